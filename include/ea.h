@@ -1,0 +1,135 @@
+/*
+ * ea.h -- C ABI of libea_b200.so: checkerboard Metropolis sweeps of the 3D +-J
+ * Edwards-Anderson model, 64 samples multispin-coded per 64-bit word, and the popcount
+ * observables C(t,t_w), C_4(r,t_w), energy, magnetisation -- hand-written sm_100a kernels.
+ *
+ * Paper: Manssen & Hartmann, arXiv:1411.5512; citations are PAPER.md:<line> + section/equation.
+ * "C-xx" are the readings of the paper listed in DESIGN.md section 2 (the stream contract).
+ *
+ * Conventions for every entry point
+ *   - Plain C types only.  "host" pointers are caller-allocated host memory, "device" pointers
+ *     are CUDA device memory.  Nothing allocated by the library is ever handed to the caller.
+ *   - Every function returns an ea_status; on any error the outputs are untouched and
+ *     ea_last_error(sim) holds a message.  No exceptions or aborts cross the boundary.
+ *   - ea_sweep / ea_snapshot are asynchronous on the sim's stream; every call that returns
+ *     host data synchronises that stream before returning.
+ *   - A handle is not thread-safe; distinct handles are independent.
+ *   - Results depend only on (L, p, T, n_replicas, seed, t): never on the GPU, the kernel
+ *     variant or the launch geometry.  ea_sweep(a); ea_sweep(b) == ea_sweep(a+b).
+ *   - There is no CPU fallback: without a CUDA device every compute call returns EA_ERR_CUDA.
+ *
+ * Canonical host format (the exchange format of ea_get_* / ea_set_*; C-A1, C-A2):
+ *   site = x + L*(y + L*z);  spins[site] : bit b = 1 <-> S = -1 of sample b;
+ *   bonds[d*N + site], d = 0,1,2 : bond between site and site + e_d (+x,+y,+z, periodic),
+ *   bit b = 1 <-> J = -1 of sample b.  n_replicas == 2: sample b (<32) = disorder b replica (a),
+ *   sample b+32 = disorder b replica (b); every bond word has hi half == lo half.
+ */
+#ifndef EA_B200_H
+#define EA_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define EA_LANES 64 /* samples per multispin word (III) */
+
+typedef struct ea_sim ea_sim; /* opaque; one batch of 64 samples on one L^3 lattice */
+
+typedef enum {
+    EA_OK = 0,
+    EA_ERR_INVALID = 1, /* bad argument (see each call)                                   */
+    EA_ERR_CUDA = 2,    /* CUDA runtime error, or no device                                */
+    EA_ERR_NOMEM = 3,   /* host or device allocation failed / workspace too small          */
+    EA_ERR_STATE = 4    /* call not valid in this state (unset slot, c4 on 1 replica, ...) */
+} ea_status;
+
+/* Sweep kernel variants (all bit-identical; selection is a performance matter only). */
+typedef enum {
+    EA_KERNEL_AUTO = 0,   /* the fastest variant valid for L                              */
+    EA_KERNEL_SCALAR = 1, /* one site per thread, 64-bit loads; any even L >= 2           */
+    EA_KERNEL_VEC2 = 2,   /* two sites per thread, 128-bit loads; L % 4 == 0              */
+    EA_KERNEL_ROWS = 3,   /* warp marches along y with a register window; L % 4 == 0      */
+    EA_KERNEL_RESIDENT = 4 /* persistent cooperative kernel, many sweeps per launch       */
+} ea_kernel;
+
+typedef struct ea_params {
+    int32_t L;          /* lattice side; even, >= 2, L^3 < 2^31 (C-A1)                     */
+    int32_t n_samples;  /* must be 64                                                      */
+    int32_t n_replicas; /* 1: 64 independent samples; 2: 32 disorders x 2 replicas (C-A2r) */
+    int32_t n_slots;    /* snapshot slots for ea_snapshot / ea_autocorr (>= 0)             */
+    double p;           /* P(J = +1), in [0,1]                              */
+    double T;           /* temperature, >= 0; 0 and +inf legal (Eq. 9)        */
+    uint64_t seed;      /* Philox key (C-A6)                                               */
+    int32_t device;     /* CUDA device ordinal; -1 = current device                        */
+    int32_t kernel;     /* ea_kernel                                                       */
+    void *stream;       /* cudaStream_t to run on (caller-owned, not the legacy default
+                           stream); NULL = the library creates and owns a stream            */
+    void *d_workspace;  /* device memory, >= ea_workspace_bytes(...), 256-byte aligned,
+                           caller-owned and alive until ea_destroy; NULL = library allocates */
+    size_t workspace_bytes;
+} ea_params;
+
+/* Bytes of device memory one sim needs (0 if the arguments are invalid). */
+size_t ea_workspace_bytes(int L, int n_replicas, int n_slots);
+
+/* Create a sim: bonds iid with P(J=+1) = p per disorder sample (C-A9), spins
+ * uniform +-1 (random start = quench from T = inf, C-A8), t = 0.
+ * ea_create: 64 independent samples (n_samples must be 64), 2 slots, current device, own stream.
+ * EA_ERR_INVALID: L odd / < 2 / too large, p outside [0,1] or NaN, T < 0 or NaN, n_samples != 64,
+ * n_replicas not 1|2, n_slots < 0, out == NULL.  The caller owns *out until ea_destroy. */
+ea_status ea_create(int L, double p, double T, int n_samples, uint64_t seed, ea_sim **out);
+ea_status ea_create_ex(const ea_params *prm, ea_sim **out);
+ea_status ea_destroy(ea_sim *sim);
+
+/* n full sweeps: each = all sites with (x+y+z)&1 == 0, then all with parity 1 (C-S2),
+ * single-spin-flip Metropolis with Eq. 9 (C-A4), one Philox4x32-10 block per (site, sweep)
+ * (C-A6, C-A7).  Asynchronous; t += n. */
+ea_status ea_sweep(ea_sim *sim, uint64_t n);
+/* One colour only (parity 0 or 1) of sweep t; does not advance t.  For tests of the half-step. */
+ea_status ea_half_sweep(ea_sim *sim, int parity);
+
+ea_status ea_get_time(const ea_sim *sim, uint64_t *t); /* completed sweeps since the random start (C-S11) */
+ea_status ea_set_time(ea_sim *sim, uint64_t t);
+ea_status ea_set_temperature(ea_sim *sim, double T);   /* recomputes the thresholds               */
+ea_status ea_get_thresholds(const ea_sim *sim, uint64_t thr[3]); /* thr[n_u], n_u = 0,1,2 (C-A4)  */
+ea_status ea_set_kernel(ea_sim *sim, int kernel);      /* EA_ERR_INVALID if not valid for this L  */
+ea_status ea_get_kernel(const ea_sim *sim, int *kernel); /* the variant AUTO resolved to          */
+ea_status ea_synchronize(ea_sim *sim);                 /* wait for the sim's stream               */
+
+/* Keep sigma(t) in slot (device copy; the paper wrote configurations to disk). */
+ea_status ea_snapshot(ea_sim *sim, int slot);
+/* A[b] = sum_i S_i,b(t_w) S_i,b(now) = N C(t,t_w) (Eq. 7); C[b] = A[b]/N or NULL.
+ * host arrays of 64.  EA_ERR_INVALID bad slot, EA_ERR_STATE unset slot. */
+ea_status ea_autocorr(ea_sim *sim, int slot, int64_t *A, double *C);
+/* Replica overlap and four-point correlation along the lattice axes (Eq. 2-3; C-S8):
+ * q[b] = sum_i q_i, q_i = S^a_i S^b_i;  B[(d*(r_max+1) + r)*32 + b] = sum_i q_i q_{i + r e_d} = N C_4.
+ * c4_avg[r] = sum_d sum_b B / (3*32*N) or NULL; q may be NULL.  0 <= r_max <= L/2.
+ * EA_ERR_STATE on a 1-replica sim. */
+ea_status ea_c4(ea_sim *sim, int r_max, int64_t *B, int64_t *q, double *c4_avg);
+/* E[b] = -sum_<ij> J_ij S_i S_j over the 3N bonds (Eq. 1); host array of 64. */
+ea_status ea_energy(ea_sim *sim, int64_t *E);
+/* M[b] = sum_i S_i,b (C-S14); host array of 64. */
+ea_status ea_magnetisation(ea_sim *sim, int64_t *M);
+
+/* Canonical packed I/O (host arrays: spins N words, bonds 3N words).
+ * ea_set_bonds on a 2-replica sim: EA_ERR_INVALID unless hi half == lo half in every word. */
+ea_status ea_get_spins(ea_sim *sim, uint64_t *host);
+ea_status ea_set_spins(ea_sim *sim, const uint64_t *host);
+ea_status ea_get_bonds(ea_sim *sim, uint64_t *host);
+ea_status ea_set_bonds(ea_sim *sim, const uint64_t *host);
+ea_status ea_get_snapshot(ea_sim *sim, int slot, uint64_t *host);
+
+/* Philox4x32-10 block on the device (one thread), for the known-answer test of the GPU side (C-A6). */
+ea_status ea_philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+
+const char *ea_strerror(ea_status s);
+const char *ea_last_error(const ea_sim *sim);
+const char *ea_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EA_B200_H */

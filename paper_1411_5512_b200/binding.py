@@ -1,0 +1,250 @@
+"""ctypes binding of libea_b200.so -- argument marshalling only; every step runs in the CUDA kernels.
+
+Function names are those of include/ea.h.  PyTorch is used for device memory (the workspace tensor handed to
+`ea_create_ex`) and streams, nothing else.  There is NO fallback: if the shared library is missing or has no
+CUDA device to run on, calls raise `EAError` / `OSError`.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libea_b200.so")
+
+EA_OK, EA_ERR_INVALID, EA_ERR_CUDA, EA_ERR_NOMEM, EA_ERR_STATE = range(5)
+EA_KERNEL_AUTO, EA_KERNEL_SCALAR, EA_KERNEL_VEC2, EA_KERNEL_ROWS, EA_KERNEL_RESIDENT = range(5)
+KERNEL_NAMES = {"auto": 0, "scalar": 1, "vec2": 2, "rows": 3, "resident": 4}
+LANES = 64
+
+
+class ea_params(C.Structure):
+    _fields_ = [("L", C.c_int32), ("n_samples", C.c_int32), ("n_replicas", C.c_int32), ("n_slots", C.c_int32),
+                ("p", C.c_double), ("T", C.c_double), ("seed", C.c_uint64), ("device", C.c_int32),
+                ("kernel", C.c_int32), ("stream", C.c_void_p), ("d_workspace", C.c_void_p),
+                ("workspace_bytes", C.c_size_t)]
+
+
+class EAError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__("ea status %d: %s" % (status, msg))
+        self.status = status
+
+
+# name -> (restype, argtypes); the -m "not gpu" suite checks that every symbol of include/ea.h is here and exported
+_vp, _i, _u64, _dbl = C.c_void_p, C.c_int, C.c_uint64, C.c_double
+SIGNATURES = {
+    "ea_workspace_bytes": (C.c_size_t, [_i, _i, _i]),
+    "ea_create": (_i, [_i, _dbl, _dbl, _i, _u64, C.POINTER(_vp)]),
+    "ea_create_ex": (_i, [C.POINTER(ea_params), C.POINTER(_vp)]),
+    "ea_destroy": (_i, [_vp]),
+    "ea_sweep": (_i, [_vp, _u64]),
+    "ea_half_sweep": (_i, [_vp, _i]),
+    "ea_get_time": (_i, [_vp, C.POINTER(_u64)]),
+    "ea_set_time": (_i, [_vp, _u64]),
+    "ea_set_temperature": (_i, [_vp, _dbl]),
+    "ea_get_thresholds": (_i, [_vp, C.POINTER(_u64)]),
+    "ea_set_kernel": (_i, [_vp, _i]),
+    "ea_get_kernel": (_i, [_vp, C.POINTER(_i)]),
+    "ea_synchronize": (_i, [_vp]),
+    "ea_snapshot": (_i, [_vp, _i]),
+    "ea_autocorr": (_i, [_vp, _i, _vp, _vp]),
+    "ea_c4": (_i, [_vp, _i, _vp, _vp, _vp]),
+    "ea_energy": (_i, [_vp, _vp]),
+    "ea_magnetisation": (_i, [_vp, _vp]),
+    "ea_get_spins": (_i, [_vp, _vp]),
+    "ea_set_spins": (_i, [_vp, _vp]),
+    "ea_get_bonds": (_i, [_vp, _vp]),
+    "ea_set_bonds": (_i, [_vp, _vp]),
+    "ea_get_snapshot": (_i, [_vp, _i, _vp]),
+    "ea_philox_selftest": (_i, [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]),
+    "ea_strerror": (C.c_char_p, [_i]),
+    "ea_last_error": (C.c_char_p, [_vp]),
+    "ea_version": (C.c_char_p, []),
+}
+
+_lib = None
+
+
+def lib():
+    """Load libea_b200.so (built by `python -m paper_1411_5512_b200.build`).  Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise OSError("libea_b200.so is not built (run `python -m paper_1411_5512_b200.build`); "
+                          "there is no CPU fallback")
+        L = C.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            f = getattr(L, name)
+            f.restype, f.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _ptr(a):
+    """Host pointer of a numpy array or a torch CPU tensor (contiguous)."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        assert a.flags["C_CONTIGUOUS"]
+        return a.ctypes.data
+    assert a.device.type == "cpu" and a.is_contiguous()  # torch tensor (possibly pinned)
+    return a.data_ptr()
+
+
+class Sim:
+    """One batch of 64 samples on an L^3 lattice on the GPU.  Methods mirror the C entry points."""
+
+    def __init__(self, L, p, T, n_replicas=1, seed=0, n_slots=2, kernel="auto", device=None, stream=None,
+                 torch_workspace=True):
+        self._h = _vp()
+        self.L, self.N, self.n_replicas, self.n_slots = int(L), int(L) ** 3, int(n_replicas), int(n_slots)
+        prm = ea_params()
+        prm.L, prm.n_samples, prm.n_replicas, prm.n_slots = int(L), LANES, int(n_replicas), int(n_slots)
+        prm.p, prm.T, prm.seed = float(p), float(T), int(seed)
+        prm.kernel = KERNEL_NAMES[kernel] if isinstance(kernel, str) else int(kernel)
+        prm.device = -1 if device is None else int(device)
+        self._ws = None
+        self._stream = stream
+        if stream is not None:  # a torch.cuda.Stream: the library launches on it
+            prm.stream = stream.cuda_stream
+        nbytes = lib().ea_workspace_bytes(int(L), int(n_replicas), int(n_slots))
+        if torch_workspace and nbytes:
+            import torch  # device memory only
+            if not torch.cuda.is_available():
+                raise EAError(EA_ERR_CUDA, "no CUDA device (there is no CPU fallback)")
+            dev = torch.device("cuda", torch.cuda.current_device() if device is None else int(device))
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev)
+            base = self._ws.data_ptr()
+            prm.d_workspace = (base + 255) & ~255
+            prm.workspace_bytes = nbytes
+        st = lib().ea_create_ex(C.byref(prm), C.byref(self._h))
+        if st != EA_OK:
+            self._h = _vp()
+            raise EAError(st, lib().ea_strerror(st).decode() + " (ea_create_ex)")
+
+    # -- plumbing -----------------------------------------------------------------------------------
+    def _ck(self, st):
+        if st != EA_OK:
+            raise EAError(st, lib().ea_last_error(self._h).decode() or lib().ea_strerror(st).decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().ea_destroy(self._h)
+            self._h = _vp()
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- dynamics -------------------------------------------------------------------------------------
+    def sweep(self, n=1):
+        self._ck(lib().ea_sweep(self._h, int(n)))
+
+    def half_sweep(self, parity):
+        self._ck(lib().ea_half_sweep(self._h, int(parity)))
+
+    def synchronize(self):
+        self._ck(lib().ea_synchronize(self._h))
+
+    @property
+    def time(self):
+        t = _u64()
+        self._ck(lib().ea_get_time(self._h, C.byref(t)))
+        return t.value
+
+    @time.setter
+    def time(self, t):
+        self._ck(lib().ea_set_time(self._h, int(t)))
+
+    def set_temperature(self, T):
+        self._ck(lib().ea_set_temperature(self._h, float(T)))
+
+    @property
+    def thresholds(self):
+        thr = (_u64 * 3)()
+        self._ck(lib().ea_get_thresholds(self._h, thr))
+        return np.array(list(thr), dtype=np.uint64)
+
+    @property
+    def kernel(self):
+        k = _i()
+        self._ck(lib().ea_get_kernel(self._h, C.byref(k)))
+        return k.value
+
+    @kernel.setter
+    def kernel(self, k):
+        self._ck(lib().ea_set_kernel(self._h, KERNEL_NAMES[k] if isinstance(k, str) else int(k)))
+
+    # -- observables ----------------------------------------------------------------------------------
+    def snapshot(self, slot):
+        self._ck(lib().ea_snapshot(self._h, int(slot)))
+
+    def autocorr(self, slot, with_C=False):
+        A = np.zeros(LANES, dtype=np.int64)
+        Cn = np.zeros(LANES, dtype=np.float64) if with_C else None
+        self._ck(lib().ea_autocorr(self._h, int(slot), _ptr(A), _ptr(Cn)))
+        return (A, Cn) if with_C else A
+
+    def c4(self, r_max, with_q=False, with_avg=False):
+        B = np.zeros((3, r_max + 1, 32), dtype=np.int64)
+        q = np.zeros(32, dtype=np.int64) if with_q else None
+        avg = np.zeros(r_max + 1, dtype=np.float64) if with_avg else None
+        self._ck(lib().ea_c4(self._h, int(r_max), _ptr(B), _ptr(q), _ptr(avg)))
+        out = (B,) + ((q,) if with_q else ()) + ((avg,) if with_avg else ())
+        return out if len(out) > 1 else B
+
+    def energy(self):
+        E = np.zeros(LANES, dtype=np.int64)
+        self._ck(lib().ea_energy(self._h, _ptr(E)))
+        return E
+
+    def magnetisation(self):
+        M = np.zeros(LANES, dtype=np.int64)
+        self._ck(lib().ea_magnetisation(self._h, _ptr(M)))
+        return M
+
+    # -- canonical packed I/O -----------------------------------------------------------------------------
+    def get_spins(self, out=None):
+        w = np.zeros(self.N, dtype=np.uint64) if out is None else out
+        self._ck(lib().ea_get_spins(self._h, _ptr(w)))
+        return w
+
+    def set_spins(self, words):
+        if isinstance(words, np.ndarray):
+            words = np.ascontiguousarray(words, dtype=np.uint64)
+            assert words.shape == (self.N,)
+        self._ck(lib().ea_set_spins(self._h, _ptr(words)))
+
+    def get_bonds(self, out=None):
+        w = np.zeros(3 * self.N, dtype=np.uint64) if out is None else out
+        self._ck(lib().ea_get_bonds(self._h, _ptr(w)))
+        return w
+
+    def set_bonds(self, words):
+        if isinstance(words, np.ndarray):
+            words = np.ascontiguousarray(words, dtype=np.uint64)
+            assert words.shape == (3 * self.N,)
+        self._ck(lib().ea_set_bonds(self._h, _ptr(words)))
+
+    def get_snapshot(self, slot):
+        w = np.zeros(self.N, dtype=np.uint64)
+        self._ck(lib().ea_get_snapshot(self._h, int(slot), _ptr(w)))
+        return w
+
+
+def philox_selftest(ctr, key):
+    c = (C.c_uint32 * 4)(*[int(x) for x in ctr])
+    k = (C.c_uint32 * 2)(*[int(x) for x in key])
+    o = (C.c_uint32 * 4)()
+    st = lib().ea_philox_selftest(c, k, o)
+    if st != EA_OK:
+        raise EAError(st, "ea_philox_selftest")
+    return [int(x) for x in o]
+
+
+def version():
+    return lib().ea_version().decode()

@@ -1,0 +1,509 @@
+// ea_api.cu -- the C ABI of libea_b200.so (declared in include/ea.h): argument checking, device memory,
+// launch sequencing.  No arithmetic of the method lives here except the acceptance thresholds (Eq. 9).
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "ea_internal.h"
+
+namespace ea {
+
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+WorkspaceLayout workspace_layout(int L, int n_replicas, int n_slots)
+{
+    WorkspaceLayout w;
+    size_t N = (size_t)L * L * L, bond_bytes = n_replicas == 2 ? 4 : 8;
+    w.n_counters = (size_t)(3 * (L / 2 + 1) + 1) * 64;
+    size_t off = 0;
+    w.off_spins = off;    off = align_up(off + N * 8);
+    w.off_bonds = off;    off = align_up(off + 3 * N * bond_bytes);
+    w.off_snaps = off;    off = align_up(off + (size_t)n_slots * N * 8);
+    w.off_stage = off;    off = align_up(off + N * 8);
+    w.off_counters = off; off = align_up(off + w.n_counters * 8);
+    w.off_time = off;     off = align_up(off + 8);
+    w.total = off;
+    return w;
+}
+
+static int ilog2_exact(unsigned v)
+{
+    if (v == 0 || (v & (v - 1))) return -1;
+    int l = 0;
+    while ((1u << l) != v) ++l;
+    return l;
+}
+
+// Eq. 9 with sum_j J_ij S_i S_j = 6 - 2 n_u:  thr[n_u] = floor(2^32 exp(-4 (3 - n_u) / T) + 0.5),
+// n_u = 0, 1, 2 (C-A4).  T = 0 -> exp(-inf) = 0;  T = +inf -> exp(-0) = 1 -> 2^32 ("always").
+static void compute_thresholds(double T, uint64_t thr[3], Thresholds &th)
+{
+    for (int k = 0; k < 3; ++k) {
+        double w = exp(-(4.0 * (double)(3 - k)) / T);
+        thr[k] = (uint64_t)floor(4294967296.0 * w + 0.5);
+        th.thr[k] = thr[k] > 0xffffffffull ? 0xffffffffu : (uint32_t)thr[k];
+        th.always[k] = thr[k] > 0xffffffffull ? 0xffffffffu : 0u;
+    }
+}
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+        changed = ok && prev != dev;
+    }
+    ~DeviceGuard() { if (changed) cudaSetDevice(prev); }
+    bool changed = false;
+};
+
+} // namespace ea
+
+using namespace ea;
+
+#define EA_FAIL(sim, code, ...)                                   \
+    do {                                                          \
+        char _b[512];                                             \
+        snprintf(_b, sizeof(_b), __VA_ARGS__);                    \
+        if (sim) (sim)->err = _b;                                 \
+        return (code);                                            \
+    } while (0)
+
+#define EA_CUDA(sim, expr)                                                                     \
+    do {                                                                                       \
+        cudaError_t _e = (expr);                                                               \
+        if (_e != cudaSuccess) EA_FAIL(sim, EA_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(_e)); \
+    } while (0)
+
+static bool valid_L(int L) { return L >= 2 && (L & 1) == 0 && (int64_t)L * L * L < ((int64_t)1 << 31); }
+
+static bool kernel_valid_for(int kernel, int L)
+{
+    switch (kernel) {
+    case EA_KERNEL_SCALAR: return true;
+    case EA_KERNEL_VEC2: return L % 4 == 0;
+    default: return false;
+    }
+}
+
+static int resolve_kernel(int kernel, int L)
+{
+    if (kernel == EA_KERNEL_AUTO) return L % 4 == 0 ? EA_KERNEL_VEC2 : EA_KERNEL_SCALAR;
+    return kernel;
+}
+
+extern "C" {
+
+const char *ea_version(void) { return "ea_b200 0.1 (sm_100a)"; }
+
+const char *ea_strerror(ea_status s)
+{
+    switch (s) {
+    case EA_OK: return "ok";
+    case EA_ERR_INVALID: return "invalid argument";
+    case EA_ERR_CUDA: return "CUDA error";
+    case EA_ERR_NOMEM: return "out of memory";
+    case EA_ERR_STATE: return "invalid state";
+    }
+    return "unknown status";
+}
+
+const char *ea_last_error(const ea_sim *sim) { return sim ? sim->err.c_str() : "null handle"; }
+
+size_t ea_workspace_bytes(int L, int n_replicas, int n_slots)
+{
+    if (!valid_L(L) || (n_replicas != 1 && n_replicas != 2) || n_slots < 0) return 0;
+    return workspace_layout(L, n_replicas, n_slots).total;
+}
+
+static void destroy_graph(ea_sim *s)
+{
+    if (s->graph_exec) cudaGraphExecDestroy(s->graph_exec);
+    s->graph_exec = nullptr;
+    s->graph_sweeps = 0;
+}
+
+ea_status ea_destroy(ea_sim *sim)
+{
+    if (!sim) return EA_OK;
+    {
+        DeviceGuard g(sim->device);
+        cudaStreamSynchronize(sim->stream);
+        destroy_graph(sim);
+        if (sim->own_ws && sim->ws) cudaFree(sim->ws);
+        if (sim->own_stream && sim->stream) cudaStreamDestroy(sim->stream);
+    }
+    delete sim;
+    return EA_OK;
+}
+
+ea_status ea_create_ex(const ea_params *prm, ea_sim **out)
+{
+    if (!prm || !out) return EA_ERR_INVALID;
+    if (!valid_L(prm->L) || prm->n_samples != EA_LANES || (prm->n_replicas != 1 && prm->n_replicas != 2) ||
+        prm->n_slots < 0 || !(prm->p >= 0.0 && prm->p <= 1.0) || !(prm->T >= 0.0))
+        return EA_ERR_INVALID;
+    int kernel = resolve_kernel(prm->kernel, prm->L);
+    if (!kernel_valid_for(kernel, prm->L)) return EA_ERR_INVALID;
+
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) return EA_ERR_CUDA; // no CPU fallback
+    int device = prm->device;
+    if (device < 0 && cudaGetDevice(&device) != cudaSuccess) return EA_ERR_CUDA;
+    if (device >= n_dev) return EA_ERR_INVALID;
+
+    ea_sim *s = new (std::nothrow) ea_sim();
+    if (!s) return EA_ERR_NOMEM;
+    const int L = prm->L;
+    s->lat.L = L;
+    s->lat.Lh = L / 2;
+    s->lat.log2L = ilog2_exact(L);
+    s->lat.log2Lh = ilog2_exact(L / 2);
+    s->N = (int64_t)L * L * L;
+    s->lat.Nh = (unsigned)(s->N / 2);
+    s->n_replicas = prm->n_replicas;
+    s->n_slots = prm->n_slots;
+    s->p = prm->p;
+    s->T = prm->T;
+    s->seed = prm->seed;
+    s->t = 0;
+    s->device = device;
+    s->kernel = kernel;
+    compute_thresholds(s->T, s->thr, s->th);
+    s->slot_set.assign(prm->n_slots, 0);
+    s->slot_t.assign(prm->n_slots, 0);
+
+    DeviceGuard g(device);
+    ea_status rc = EA_OK;
+    cudaError_t e = cudaSuccess;
+    WorkspaceLayout w = workspace_layout(L, s->n_replicas, s->n_slots);
+    do {
+        if (!g.ok) { rc = EA_ERR_CUDA; break; }
+        cudaDeviceGetAttribute(&s->n_sm, cudaDevAttrMultiProcessorCount, device);
+        if (prm->stream) {
+            s->stream = (cudaStream_t)prm->stream;
+        } else { // own stream: the legacy default stream cannot be captured into a graph
+            if ((e = cudaStreamCreateWithFlags(&s->stream, cudaStreamNonBlocking)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
+            s->own_stream = true;
+        }
+        if (prm->d_workspace) {
+            if (prm->workspace_bytes < w.total || ((uintptr_t)prm->d_workspace & 255)) { rc = EA_ERR_NOMEM; break; }
+            s->ws = (char *)prm->d_workspace;
+        } else {
+            if ((e = cudaMalloc((void **)&s->ws, w.total)) != cudaSuccess) { rc = EA_ERR_NOMEM; break; }
+            s->own_ws = true;
+        }
+        s->ws_bytes = w.total;
+        s->spins = (uint64_t *)(s->ws + w.off_spins);
+        s->bonds = (void *)(s->ws + w.off_bonds);
+        s->snaps = (uint64_t *)(s->ws + w.off_snaps);
+        s->stage = (uint64_t *)(s->ws + w.off_stage);
+        s->counters = (unsigned long long *)(s->ws + w.off_counters);
+        s->n_counters = w.n_counters;
+        s->d_time = (uint64_t *)(s->ws + w.off_time);
+        s->h_counters.resize(w.n_counters);
+        if ((e = launch_init_bonds(s)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
+        if ((e = launch_init_spins(s)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
+        if ((e = cudaMemsetAsync(s->d_time, 0, 8, s->stream)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
+        if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
+    } while (0);
+    if (rc != EA_OK) {
+        if (e != cudaSuccess) fprintf(stderr, "ea_create_ex: %s\n", cudaGetErrorString(e));
+        if (s->own_ws && s->ws) cudaFree(s->ws);
+        if (s->own_stream && s->stream) cudaStreamDestroy(s->stream);
+        delete s;
+        return rc;
+    }
+    *out = s;
+    return EA_OK;
+}
+
+ea_status ea_create(int L, double p, double T, int n_samples, uint64_t seed, ea_sim **out)
+{
+    ea_params prm;
+    memset(&prm, 0, sizeof(prm));
+    prm.L = L; prm.n_samples = n_samples; prm.n_replicas = 1; prm.n_slots = 2;
+    prm.p = p; prm.T = T; prm.seed = seed; prm.device = -1; prm.kernel = EA_KERNEL_AUTO;
+    return ea_create_ex(&prm, out);
+}
+
+// ---- dynamics -------------------------------------------------------------------------------------
+
+static const int GRAPH_SWEEPS = 32; // sweeps per CUDA-graph replay (2 kernel nodes each + the time bump)
+
+static ea_status build_graph(ea_sim *s)
+{
+    destroy_graph(s);
+    cudaGraph_t graph = nullptr;
+    EA_CUDA(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
+    cudaError_t e = cudaSuccess;
+    for (int k = 0; k < GRAPH_SWEEPS && e == cudaSuccess; ++k) {
+        e = launch_half_sweep(s, 0, 0, s->d_time, (uint32_t)k, s->stream);
+        if (e == cudaSuccess) e = launch_half_sweep(s, 1, 0, s->d_time, (uint32_t)k, s->stream);
+    }
+    if (e == cudaSuccess) e = launch_bump_time(s, GRAPH_SWEEPS, s->stream);
+    cudaError_t e2 = cudaStreamEndCapture(s->stream, &graph);
+    if (e != cudaSuccess || e2 != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        EA_FAIL(s, EA_ERR_CUDA, "graph capture: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
+    }
+    e = cudaGraphInstantiate(&s->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) {
+        s->graph_exec = nullptr;
+        EA_FAIL(s, EA_ERR_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
+    }
+    s->graph_sweeps = GRAPH_SWEEPS;
+    s->graph_kernel = s->kernel;
+    return EA_OK;
+}
+
+ea_status ea_sweep(ea_sim *sim, uint64_t n)
+{
+    if (!sim) return EA_ERR_INVALID;
+    DeviceGuard g(sim->device);
+    uint64_t left = n;
+    if (left >= (uint64_t)GRAPH_SWEEPS) {
+        if (!sim->graph_exec || sim->graph_kernel != sim->kernel) {
+            ea_status rc = build_graph(sim);
+            if (rc != EA_OK) return rc;
+        }
+        // pageable source: staged before the call returns, so &sim->t need not outlive it
+        EA_CUDA(sim, cudaMemcpyAsync(sim->d_time, &sim->t, 8, cudaMemcpyHostToDevice, sim->stream));
+        while (left >= (uint64_t)sim->graph_sweeps) {
+            EA_CUDA(sim, cudaGraphLaunch(sim->graph_exec, sim->stream));
+            sim->t += sim->graph_sweeps;
+            left -= sim->graph_sweeps;
+        }
+    }
+    for (; left; --left) {
+        EA_CUDA(sim, launch_half_sweep(sim, 0, sim->t, nullptr, 0, sim->stream));
+        EA_CUDA(sim, launch_half_sweep(sim, 1, sim->t, nullptr, 0, sim->stream));
+        sim->t += 1;
+    }
+    return EA_OK;
+}
+
+ea_status ea_half_sweep(ea_sim *sim, int parity)
+{
+    if (!sim) return EA_ERR_INVALID;
+    if (parity != 0 && parity != 1) EA_FAIL(sim, EA_ERR_INVALID, "parity must be 0 or 1");
+    DeviceGuard g(sim->device);
+    EA_CUDA(sim, launch_half_sweep(sim, parity, sim->t, nullptr, 0, sim->stream));
+    return EA_OK;
+}
+
+ea_status ea_get_time(const ea_sim *sim, uint64_t *t)
+{
+    if (!sim || !t) return EA_ERR_INVALID;
+    *t = sim->t;
+    return EA_OK;
+}
+
+ea_status ea_set_time(ea_sim *sim, uint64_t t)
+{
+    if (!sim) return EA_ERR_INVALID;
+    sim->t = t;
+    return EA_OK;
+}
+
+ea_status ea_set_temperature(ea_sim *sim, double T)
+{
+    if (!sim) return EA_ERR_INVALID;
+    if (!(T >= 0.0)) EA_FAIL(sim, EA_ERR_INVALID, "T must be >= 0");
+    sim->T = T;
+    compute_thresholds(T, sim->thr, sim->th);
+    DeviceGuard g(sim->device);
+    destroy_graph(sim); // thresholds are baked into the captured launches
+    return EA_OK;
+}
+
+ea_status ea_get_thresholds(const ea_sim *sim, uint64_t thr[3])
+{
+    if (!sim || !thr) return EA_ERR_INVALID;
+    memcpy(thr, sim->thr, sizeof(sim->thr));
+    return EA_OK;
+}
+
+ea_status ea_set_kernel(ea_sim *sim, int kernel)
+{
+    if (!sim) return EA_ERR_INVALID;
+    int k = resolve_kernel(kernel, sim->lat.L);
+    if (!kernel_valid_for(k, sim->lat.L)) EA_FAIL(sim, EA_ERR_INVALID, "kernel %d not valid for L=%d", kernel, sim->lat.L);
+    sim->kernel = k;
+    return EA_OK;
+}
+
+ea_status ea_get_kernel(const ea_sim *sim, int *kernel)
+{
+    if (!sim || !kernel) return EA_ERR_INVALID;
+    *kernel = sim->kernel;
+    return EA_OK;
+}
+
+ea_status ea_synchronize(ea_sim *sim)
+{
+    if (!sim) return EA_ERR_INVALID;
+    DeviceGuard g(sim->device);
+    EA_CUDA(sim, cudaStreamSynchronize(sim->stream));
+    return EA_OK;
+}
+
+// ---- observables ----------------------------------------------------------------------------------
+
+static ea_status fetch_counters(ea_sim *s, size_t n)
+{
+    EA_CUDA(s, cudaMemcpyAsync(s->h_counters.data(), s->counters, n * sizeof(unsigned long long),
+                               cudaMemcpyDeviceToHost, s->stream));
+    EA_CUDA(s, cudaStreamSynchronize(s->stream));
+    return EA_OK;
+}
+
+ea_status ea_snapshot(ea_sim *sim, int slot)
+{
+    if (!sim) return EA_ERR_INVALID;
+    if (slot < 0 || slot >= sim->n_slots) EA_FAIL(sim, EA_ERR_INVALID, "slot %d out of range [0,%d)", slot, sim->n_slots);
+    DeviceGuard g(sim->device);
+    EA_CUDA(sim, cudaMemcpyAsync(sim->snaps + (size_t)slot * sim->N, sim->spins, (size_t)sim->N * 8,
+                                 cudaMemcpyDeviceToDevice, sim->stream));
+    sim->slot_set[slot] = 1;
+    sim->slot_t[slot] = sim->t;
+    return EA_OK;
+}
+
+ea_status ea_autocorr(ea_sim *sim, int slot, int64_t *A, double *C)
+{
+    if (!sim || !A) return EA_ERR_INVALID;
+    if (slot < 0 || slot >= sim->n_slots) EA_FAIL(sim, EA_ERR_INVALID, "slot %d out of range [0,%d)", slot, sim->n_slots);
+    if (!sim->slot_set[slot]) EA_FAIL(sim, EA_ERR_STATE, "slot %d holds no snapshot", slot);
+    DeviceGuard g(sim->device);
+    EA_CUDA(sim, launch_count_spins(sim, sim->snaps + (size_t)slot * sim->N));
+    ea_status rc = fetch_counters(sim, 64);
+    if (rc != EA_OK) return rc;
+    for (int b = 0; b < 64; ++b) {
+        A[b] = sim->N - 2 * (int64_t)sim->h_counters[b];
+        if (C) C[b] = (double)A[b] / (double)sim->N;
+    }
+    return EA_OK;
+}
+
+ea_status ea_magnetisation(ea_sim *sim, int64_t *M)
+{
+    if (!sim || !M) return EA_ERR_INVALID;
+    DeviceGuard g(sim->device);
+    EA_CUDA(sim, launch_count_spins(sim, nullptr));
+    ea_status rc = fetch_counters(sim, 64);
+    if (rc != EA_OK) return rc;
+    for (int b = 0; b < 64; ++b) M[b] = sim->N - 2 * (int64_t)sim->h_counters[b];
+    return EA_OK;
+}
+
+ea_status ea_energy(ea_sim *sim, int64_t *E)
+{
+    if (!sim || !E) return EA_ERR_INVALID;
+    DeviceGuard g(sim->device);
+    EA_CUDA(sim, launch_count_energy(sim));
+    ea_status rc = fetch_counters(sim, 64);
+    if (rc != EA_OK) return rc;
+    for (int b = 0; b < 64; ++b) E[b] = -3 * sim->N + 2 * (int64_t)sim->h_counters[b];
+    return EA_OK;
+}
+
+ea_status ea_c4(ea_sim *sim, int r_max, int64_t *B, int64_t *q, double *c4_avg)
+{
+    if (!sim || !B) return EA_ERR_INVALID;
+    if (sim->n_replicas != 2) EA_FAIL(sim, EA_ERR_STATE, "ea_c4 needs a 2-replica sim");
+    if (r_max < 0 || r_max > sim->lat.L / 2) EA_FAIL(sim, EA_ERR_INVALID, "r_max %d outside [0, L/2]", r_max);
+    DeviceGuard g(sim->device);
+    EA_CUDA(sim, launch_count_c4(sim, r_max));
+    const size_t n_r = (size_t)r_max + 1, jobs = 3 * n_r + 1;
+    ea_status rc = fetch_counters(sim, jobs * 32);
+    if (rc != EA_OK) return rc;
+    for (size_t k = 0; k < 3 * n_r * 32; ++k) B[k] = sim->N - 2 * (int64_t)sim->h_counters[k];
+    if (q)
+        for (int b = 0; b < 32; ++b) q[b] = sim->N - 2 * (int64_t)sim->h_counters[3 * n_r * 32 + b];
+    if (c4_avg)
+        for (size_t r = 0; r < n_r; ++r) {
+            int64_t sum = 0; // integer sum first, one division (C-A10)
+            for (int d = 0; d < 3; ++d)
+                for (int b = 0; b < 32; ++b) sum += B[(d * n_r + r) * 32 + b];
+            c4_avg[r] = (double)sum / (3.0 * 32.0 * (double)sim->N);
+        }
+    return EA_OK;
+}
+
+// ---- canonical packed I/O ---------------------------------------------------------------------------
+
+ea_status ea_get_spins(ea_sim *sim, uint64_t *host)
+{
+    if (!sim || !host) return EA_ERR_INVALID;
+    DeviceGuard g(sim->device);
+    EA_CUDA(sim, launch_unpack_spins(sim, sim->spins, sim->stage));
+    EA_CUDA(sim, cudaMemcpyAsync(host, sim->stage, (size_t)sim->N * 8, cudaMemcpyDeviceToHost, sim->stream));
+    EA_CUDA(sim, cudaStreamSynchronize(sim->stream));
+    return EA_OK;
+}
+
+ea_status ea_get_snapshot(ea_sim *sim, int slot, uint64_t *host)
+{
+    if (!sim || !host) return EA_ERR_INVALID;
+    if (slot < 0 || slot >= sim->n_slots) EA_FAIL(sim, EA_ERR_INVALID, "slot %d out of range [0,%d)", slot, sim->n_slots);
+    if (!sim->slot_set[slot]) EA_FAIL(sim, EA_ERR_STATE, "slot %d holds no snapshot", slot);
+    DeviceGuard g(sim->device);
+    EA_CUDA(sim, launch_unpack_spins(sim, sim->snaps + (size_t)slot * sim->N, sim->stage));
+    EA_CUDA(sim, cudaMemcpyAsync(host, sim->stage, (size_t)sim->N * 8, cudaMemcpyDeviceToHost, sim->stream));
+    EA_CUDA(sim, cudaStreamSynchronize(sim->stream));
+    return EA_OK;
+}
+
+ea_status ea_set_spins(ea_sim *sim, const uint64_t *host)
+{
+    if (!sim || !host) return EA_ERR_INVALID;
+    DeviceGuard g(sim->device);
+    EA_CUDA(sim, cudaMemcpyAsync(sim->stage, host, (size_t)sim->N * 8, cudaMemcpyHostToDevice, sim->stream));
+    EA_CUDA(sim, launch_pack_spins(sim, sim->stage, sim->spins));
+    EA_CUDA(sim, cudaStreamSynchronize(sim->stream));
+    return EA_OK;
+}
+
+ea_status ea_get_bonds(ea_sim *sim, uint64_t *host)
+{
+    if (!sim || !host) return EA_ERR_INVALID;
+    DeviceGuard g(sim->device);
+    for (int d = 0; d < 3; ++d) {
+        EA_CUDA(sim, launch_unpack_bonds(sim, d, sim->stage));
+        EA_CUDA(sim, cudaMemcpyAsync(host + (size_t)d * sim->N, sim->stage, (size_t)sim->N * 8, cudaMemcpyDeviceToHost,
+                                     sim->stream));
+        EA_CUDA(sim, cudaStreamSynchronize(sim->stream));
+    }
+    return EA_OK;
+}
+
+ea_status ea_set_bonds(ea_sim *sim, const uint64_t *host)
+{
+    if (!sim || !host) return EA_ERR_INVALID;
+    if (sim->n_replicas == 2) // both replicas have "the same bond configuration"
+        for (int64_t k = 0; k < 3 * sim->N; ++k)
+            if ((uint32_t)host[k] != (uint32_t)(host[k] >> 32))
+                EA_FAIL(sim, EA_ERR_INVALID, "2-replica sim: bond word %lld has hi half != lo half", (long long)k);
+    DeviceGuard g(sim->device);
+    for (int d = 0; d < 3; ++d) {
+        EA_CUDA(sim, cudaMemcpyAsync(sim->stage, host + (size_t)d * sim->N, (size_t)sim->N * 8, cudaMemcpyHostToDevice,
+                                     sim->stream));
+        EA_CUDA(sim, launch_pack_bonds(sim, d, sim->stage));
+        EA_CUDA(sim, cudaStreamSynchronize(sim->stream));
+    }
+    return EA_OK;
+}
+
+ea_status ea_philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    if (!ctr || !key || !out) return EA_ERR_INVALID;
+    return philox_selftest(ctr, key, out) == cudaSuccess ? EA_OK : EA_ERR_CUDA;
+}
+
+} // extern "C"

@@ -1,0 +1,217 @@
+// ea_device.cuh -- device-side building blocks shared by the kernels of libea_b200.so.
+//
+// Everything here implements the WRITTEN stream contract of DESIGN.md section 2 (C-xx) for the
+// paper's update (Manssen & Hartmann, arXiv:1411.5512; section III).  It shares no
+// code with oracle/ (the CPU checker is written independently from the same text).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ea {
+
+// ---------------------------------------------------------------------------------------------
+// HBM layout.  Sites are split by colour c = (x+y+z)&1 and compacted along x:
+//   compact index i = xh + Lh*(y + L*z),  xh = x>>1,  Lh = L/2,  x = 2*xh + (c ^ ((y+z)&1)).
+//   spins  : uint64 [2][Nh]           (Nh = N/2)
+//   bonds  : BondT  [2][3][Nh]        forward bond (d, site) stored at the site's (colour, compact index);
+//            BondT = uint64 for 64 independent samples, uint32 for 32 disorders x 2 replicas
+//            (hi half == lo half by PAPER.md:33, so only the low half is stored and read).
+// A half-sweep of colour c reads spins[c], spins[1-c], all six bond planes once and writes spins[c].
+// ---------------------------------------------------------------------------------------------
+struct Lattice {
+    int L, Lh;       // side, side/2
+    int log2Lh;      // >= 0 if Lh is a power of two, else -1
+    int log2L;       // >= 0 if L is a power of two, else -1
+    unsigned Nh;     // L^3 / 2
+};
+
+// Philox4x32-10 (Salmon et al., SC'11), reading C-A6: multipliers 0xD2511F53 (on c0) and
+// 0xCD9E8D57 (on c2), Weyl increments 0x9E3779B9 / 0xBB67AE85 added to the key after each round.
+constexpr uint32_t PHILOX_M0 = 0xD2511F53u;
+constexpr uint32_t PHILOX_M1 = 0xCD9E8D57u;
+constexpr uint32_t PHILOX_W0 = 0x9E3779B9u;
+constexpr uint32_t PHILOX_W1 = 0xBB67AE85u;
+
+// Stream tags, 4th counter word (C-A6).
+enum : uint32_t { TAG_PARITY0 = 0, TAG_PARITY1 = 1, TAG_INIT_SPINS = 2, TAG_BONDS = 3 };
+
+__device__ __forceinline__ void mulhilo(uint32_t a, uint32_t b, uint32_t &hi, uint32_t &lo)
+{
+    unsigned long long p = (unsigned long long)a * (unsigned long long)b; // one IMAD.WIDE.U32
+    hi = (uint32_t)(p >> 32);
+    lo = (uint32_t)p;
+}
+
+// The full block function (all four outputs); used by the setup kernels and the self-test.
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t out[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        uint32_t h0, l0, h1, l1;
+        mulhilo(PHILOX_M0, c0, h0, l0);
+        mulhilo(PHILOX_M1, c2, h1, l1);
+        c0 = h1 ^ c1 ^ k0;
+        c1 = l1;
+        c2 = h0 ^ c3 ^ k1;
+        c3 = l0;
+        k0 += PHILOX_W0;
+        k1 += PHILOX_W1;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// The update stream of one half-sweep: counter (site, t lo, t hi, parity), key = seed (C-A6).
+// Only c0 = site varies inside a launch, so everything that depends on (t, parity, seed) alone is
+// folded once per launch into SweepRng (rounds 1-2 collapse to two multiplies); and only out[0]
+// (samples 0..31) and out[1] (samples 32..63) are consumed (C-A7), so round 10 needs one multiply.
+// The result is bit-identical to philox4x32_10(site, t lo, t hi, parity; seed)[0..1].
+struct SweepRng {
+    uint32_t x2;     // tag ^ k1[0]
+    uint32_t x0;     // lo(M1*t_hi) ^ k0[1]
+    uint32_t y2;     // hi(M0*U0) ^ k1[1],  U0 = hi(M1*t_hi) ^ t_lo ^ k0[0]
+    uint32_t z2;     // lo(M0*U0) ^ k1[2]
+    uint32_t k0[10]; // round keys (only [2..9] used)
+    uint32_t k1[10]; // round keys (only [3..8] used)
+};
+
+__host__ __device__ inline SweepRng make_sweep_rng(uint64_t seed, uint64_t t, uint32_t tag)
+{
+    SweepRng g;
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) {
+        g.k0[r] = k0 + (uint32_t)r * PHILOX_W0;
+        g.k1[r] = k1 + (uint32_t)r * PHILOX_W1;
+    }
+    uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
+    uint64_t p1 = (uint64_t)PHILOX_M1 * t_hi;
+    uint32_t U0 = (uint32_t)(p1 >> 32) ^ t_lo ^ g.k0[0];
+    uint32_t U1 = (uint32_t)p1;
+    uint64_t q0 = (uint64_t)PHILOX_M0 * U0;
+    g.x2 = tag ^ g.k1[0];
+    g.x0 = U1 ^ g.k0[1];
+    g.y2 = (uint32_t)(q0 >> 32) ^ g.k1[1];
+    g.z2 = (uint32_t)q0 ^ g.k1[2];
+    return g;
+}
+
+__device__ __forceinline__ void sweep_random(const SweepRng &g, uint32_t site, uint32_t &r_lo, uint32_t &r_hi)
+{
+    uint32_t h, l, h0, l0, h1, l1;
+    // round 1: (site, t_lo, t_hi, tag) -> (U0, U1, n2, n3)
+    mulhilo(PHILOX_M0, site, h, l);
+    uint32_t n2 = h ^ g.x2, n3 = l;
+    // round 2: (U0, U1, n2, n3) -> (m0, m1, m2, V3)
+    mulhilo(PHILOX_M1, n2, h, l);
+    uint32_t c0 = h ^ g.x0, c1 = l, c2 = n3 ^ g.y2;
+    // round 3: c3 = V3 is launch-uniform
+    mulhilo(PHILOX_M0, c0, h0, l0);
+    mulhilo(PHILOX_M1, c2, h1, l1);
+    c0 = h1 ^ c1 ^ g.k0[2];
+    c1 = l1;
+    c2 = h0 ^ g.z2;
+    uint32_t c3 = l0;
+    // rounds 4..9
+#pragma unroll
+    for (int r = 3; r < 9; ++r) {
+        mulhilo(PHILOX_M0, c0, h0, l0);
+        mulhilo(PHILOX_M1, c2, h1, l1);
+        c0 = h1 ^ c1 ^ g.k0[r];
+        c1 = l1;
+        c2 = h0 ^ c3 ^ g.k1[r];
+        c3 = l0;
+    }
+    // round 10: only out[0], out[1]
+    mulhilo(PHILOX_M1, c2, h1, l1);
+    r_lo = h1 ^ c1 ^ g.k0[9];
+    r_hi = l1;
+}
+
+// Acceptance thresholds of Eq. 9 (C-A4) prepared for 32-bit compares:
+// accept at n_u = k  <=>  r < thr[k]  with thr[k] in [0, 2^32];  thr == 2^32 ("always", T = inf)
+// does not fit a 32-bit compare, so it is carried as an all-ones mask OR-ed into the result.
+struct Thresholds {
+    uint32_t thr[3];    // min(thr[k], 2^32 - 1)
+    uint32_t always[3]; // 0xffffffff if thr[k] == 2^32 else 0
+};
+
+__device__ __forceinline__ uint32_t xor3(uint32_t a, uint32_t b, uint32_t c) { return a ^ b ^ c; }
+__device__ __forceinline__ uint32_t maj3(uint32_t a, uint32_t b, uint32_t c) { return (a & b) | (c & (a | b)); }
+
+// One 32-sample half of one Metropolis trial (Eq. 9; "boolean logic at the bit level").
+// u1..u6: unsatisfied-bond words j ^ sigma_i ^ sigma_nbr (C-A2, C-A3).  Bit-sliced count n_u = (c2 c1 c0),
+// nested level masks m0 <= m1 <= m2 (m_k = all ones iff r < thr[k]): flip iff n_u + level >= 3, i.e.
+//   f = [n_u>=3] | m2 & [n_u>=2] | m1 & [n_u>=1] | m0.
+__device__ __forceinline__ uint32_t flip_mask(uint32_t u1, uint32_t u2, uint32_t u3, uint32_t u4, uint32_t u5,
+                                              uint32_t u6, uint32_t m0, uint32_t m1, uint32_t m2)
+{
+    uint32_t sa = xor3(u1, u2, u3), ka = maj3(u1, u2, u3);
+    uint32_t sb = xor3(u4, u5, u6), kb = maj3(u4, u5, u6);
+    uint32_t c0 = sa ^ sb, kc = sa & sb;
+    uint32_t c1 = xor3(ka, kb, kc), c2 = maj3(ka, kb, kc);
+    uint32_t a = c1 & (c0 | m2);     // n_u = 3, or n_u = 2 with level >= 1
+    uint32_t b = a | (m1 & c0);      // n_u = 1 with level >= 2 (m1 & c1 is inside m2 & c1 because m1 <= m2)
+    return b | c2 | m0;              // n_u >= 4; level 3
+}
+
+__device__ __forceinline__ void level_masks(const Thresholds &th, uint32_t r, uint32_t &m0, uint32_t &m1, uint32_t &m2)
+{
+    m0 = (r < th.thr[0] ? 0xffffffffu : 0u) | th.always[0];
+    m1 = (r < th.thr[1] ? 0xffffffffu : 0u) | th.always[1];
+    m2 = (r < th.thr[2] ? 0xffffffffu : 0u) | th.always[2];
+}
+
+// 64-bit word <-> halves
+__device__ __forceinline__ uint32_t lo32(uint64_t w) { return (uint32_t)w; }
+__device__ __forceinline__ uint32_t hi32(uint64_t w) { return (uint32_t)(w >> 32); }
+__device__ __forceinline__ uint64_t mk64(uint32_t lo, uint32_t hi) { return (uint64_t)lo | ((uint64_t)hi << 32); }
+
+// Bond word -> the two 32-sample halves the update logic needs.
+__device__ __forceinline__ uint32_t bond_lo(uint64_t j) { return (uint32_t)j; }
+__device__ __forceinline__ uint32_t bond_hi(uint64_t j) { return (uint32_t)(j >> 32); }
+__device__ __forceinline__ uint32_t bond_lo(uint32_t j) { return j; }
+__device__ __forceinline__ uint32_t bond_hi(uint32_t j) { return j; } // replica (b) sees the same bonds
+
+// One whole Metropolis trial of a 64-sample word: returns the new spin word.
+template <typename BondT>
+__device__ __forceinline__ uint64_t metropolis_word(uint64_t s, uint64_t n1, uint64_t n2, uint64_t n3, uint64_t n4,
+                                                    uint64_t n5, uint64_t n6, BondT j1, BondT j2, BondT j3, BondT j4,
+                                                    BondT j5, BondT j6, uint32_t r_lo, uint32_t r_hi,
+                                                    const Thresholds &th)
+{
+    uint32_t sl = lo32(s), sh = hi32(s);
+    uint32_t m0, m1, m2;
+    level_masks(th, r_lo, m0, m1, m2);
+    uint32_t fl = flip_mask(bond_lo(j1) ^ sl ^ lo32(n1), bond_lo(j2) ^ sl ^ lo32(n2), bond_lo(j3) ^ sl ^ lo32(n3),
+                            bond_lo(j4) ^ sl ^ lo32(n4), bond_lo(j5) ^ sl ^ lo32(n5), bond_lo(j6) ^ sl ^ lo32(n6),
+                            m0, m1, m2);
+    level_masks(th, r_hi, m0, m1, m2);
+    uint32_t fh = flip_mask(bond_hi(j1) ^ sh ^ hi32(n1), bond_hi(j2) ^ sh ^ hi32(n2), bond_hi(j3) ^ sh ^ hi32(n3),
+                            bond_hi(j4) ^ sh ^ hi32(n4), bond_hi(j5) ^ sh ^ hi32(n5), bond_hi(j6) ^ sh ^ hi32(n6),
+                            m0, m1, m2);
+    return mk64(sl ^ fl, sh ^ fh);
+}
+
+// ---------------------------------------------------------------------------------------------
+// 32x32 bit-matrix transpose across a warp (observables: per-sample popcounts).
+// In : lane i holds w_i, bit j of w_i = sample j at site i.   Out: lane j holds bit i = sample j at site i.
+// Five butterfly stages; stage s swaps bit s of the lane index with bit s of the bit index.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t warp_transpose32(uint32_t w, unsigned lane)
+{
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) {
+        // keep-mask: bit positions whose bit-s equals the lane's bit-s stay; the others come from the partner
+        const uint32_t lowmask = (s == 16) ? 0x0000ffffu : (s == 8) ? 0x00ff00ffu : (s == 4) ? 0x0f0f0f0fu
+                                 : (s == 2)                                                 ? 0x33333333u
+                                                                                            : 0x55555555u;
+        uint32_t p = __shfl_xor_sync(0xffffffffu, w, s);
+        if (lane & s)
+            w = (w & ~lowmask) | ((p >> s) & lowmask);
+        else
+            w = (w & lowmask) | ((p << s) & ~lowmask);
+    }
+    return w;
+}
+
+} // namespace ea

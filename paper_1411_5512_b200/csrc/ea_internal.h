@@ -1,0 +1,79 @@
+// ea_internal.h -- host-side state of one sim and the launch wrappers of the kernels (not installed).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/ea.h"
+#include "ea_device.cuh"
+
+struct ea_sim {
+    ea::Lattice lat;
+    int64_t N = 0;
+    int n_replicas = 1, n_slots = 0;
+    double p = 0, T = 0;
+    uint64_t seed = 0, t = 0;
+    uint64_t thr[3] = {0, 0, 0};
+    ea::Thresholds th;
+    int device = 0;
+    int n_sm = 148;
+    cudaStream_t stream = nullptr;
+    int kernel = EA_KERNEL_SCALAR; // resolved variant
+
+    bool own_ws = false, own_stream = false;
+    char *ws = nullptr;
+    size_t ws_bytes = 0;
+    uint64_t *spins = nullptr;    // [2][Nh]
+    void *bonds = nullptr;        // BondT [2][3][Nh]
+    uint64_t *snaps = nullptr;    // [n_slots][2][Nh]
+    uint64_t *stage = nullptr;    // [N] canonical staging for get/set
+    unsigned long long *counters = nullptr; // [n_counters]
+    size_t n_counters = 0;
+    std::vector<char> slot_set;
+    std::vector<uint64_t> slot_t;
+    std::vector<unsigned long long> h_counters;
+
+    // CUDA graph of a block of sweeps (launch-bound small lattices)
+    cudaGraphExec_t graph_exec = nullptr;
+    int graph_sweeps = 0;
+    int graph_kernel = -1;
+    uint64_t *d_time = nullptr;   // device copy of t consumed by graph-launched kernels
+
+    std::string err;
+
+    int bond_bytes() const { return n_replicas == 2 ? 4 : 8; }
+    uint64_t *spins_c(int c) const { return spins + (size_t)c * lat.Nh; }
+};
+
+namespace ea {
+
+struct WorkspaceLayout {
+    size_t off_spins, off_bonds, off_snaps, off_stage, off_counters, off_time, total;
+    size_t n_counters;
+};
+WorkspaceLayout workspace_layout(int L, int n_replicas, int n_slots);
+
+// ---- launch wrappers (each returns the cudaError_t of the launch) -------------------------------
+cudaError_t launch_init_spins(ea_sim *s);
+cudaError_t launch_init_bonds(ea_sim *s);
+// one colour of sweep t.  If d_time != nullptr the kernels read t = *d_time + t_offset on the device.
+cudaError_t launch_half_sweep(ea_sim *s, int parity, uint64_t t, const uint64_t *d_time, uint32_t t_offset,
+                              cudaStream_t st);
+cudaError_t launch_bump_time(ea_sim *s, uint32_t n, cudaStream_t st);
+
+// canonical <-> internal
+cudaError_t launch_pack_spins(ea_sim *s, const uint64_t *d_canon, uint64_t *d_internal);   // canonical -> internal
+cudaError_t launch_unpack_spins(ea_sim *s, const uint64_t *d_internal, uint64_t *d_canon); // internal -> canonical
+cudaError_t launch_pack_bonds(ea_sim *s, int d, const uint64_t *d_canon);                  // one direction, N words
+cudaError_t launch_unpack_bonds(ea_sim *s, int d, uint64_t *d_canon);
+
+// observables: per-sample bit counts into s->counters (zeroed by the wrapper)
+cudaError_t launch_count_spins(ea_sim *s, const uint64_t *d_other /* nullable: XOR partner, same layout */);
+cudaError_t launch_count_energy(ea_sim *s);
+cudaError_t launch_count_c4(ea_sim *s, int r_max); // counters[(d*(r_max+1)+r)*32+b], then [3*(r_max+1)*32 + b] = overlap
+
+cudaError_t philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+
+} // namespace ea

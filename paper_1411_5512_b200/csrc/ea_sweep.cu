@@ -1,0 +1,209 @@
+// ea_sweep.cu -- the half-sweep kernels: one Metropolis trial (Eq. 9) for every site of one
+// colour, 64 samples per word, in the colour-split compact layout of ea_device.cuh.
+//
+// A kernel boundary is the colour barrier ("each half-step is performed in its own CUDA kernel call to
+// ensure global synchronization").  All variants are bit-identical (same stream contract).
+#include "ea_internal.h"
+
+namespace ea {
+
+struct SweepArgs {
+    Lattice lat;
+    int colour;                 // parity of the sites updated by this launch (C-S2)
+    uint64_t *own;              // spins[colour]      (read + written)
+    const uint64_t *oth;        // spins[1 - colour]  (read only)
+    const void *Jc;             // bonds[colour][3][Nh]     forward bonds of the updated sites
+    const void *Jo;             // bonds[1 - colour][3][Nh] forward bonds of the neighbours (our backward bonds)
+    uint64_t seed;
+    uint64_t t;                 // sweep index, used when d_time == nullptr
+    const uint64_t *d_time;     // device-resident t (CUDA-graph replays); t = *d_time + t_offset
+    uint32_t t_offset;
+    Thresholds th;
+};
+
+__device__ __forceinline__ uint64_t sweep_time(const SweepArgs &a)
+{
+    return (a.d_time ? *a.d_time : a.t) + a.t_offset;
+}
+
+template <bool POW2>
+__device__ __forceinline__ void decode_row(const Lattice &lat, unsigned tid, unsigned log2W, unsigned W, unsigned &k,
+                                           unsigned &y, unsigned &z)
+{
+    unsigned row;
+    if (POW2) {
+        k = tid & (W - 1);
+        row = tid >> log2W;
+        y = row & (lat.L - 1);
+        z = row >> lat.log2L;
+    } else {
+        k = tid % W;
+        row = tid / W;
+        y = row % lat.L;
+        z = row / lat.L;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// SCALAR: one site per thread, any even L >= 2 (L = 2: +x and -x neighbours are the same site,
+// reached through two distinct bonds -- C-S15).
+// ---------------------------------------------------------------------------------------------
+template <typename BondT, bool POW2>
+__global__ void __launch_bounds__(256) k_sweep_scalar(const SweepArgs a)
+{
+    const Lattice lat = a.lat;
+    const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= lat.Nh) return;
+    unsigned xh, y, z;
+    decode_row<POW2>(lat, tid, lat.log2Lh, lat.Lh, xh, y, z);
+    const unsigned L = lat.L, Lh = lat.Lh;
+    const unsigned s = (a.colour ^ (y + z)) & 1u;
+    const unsigned yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
+    const unsigned zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+    const unsigned rowbase = Lh * (y + L * z);
+    const unsigned i = rowbase + xh;
+    const unsigned xo = s ? ((xh + 1 == Lh) ? 0 : xh + 1) : ((xh == 0) ? Lh - 1 : xh - 1);
+    const unsigned jp = s ? rowbase + xo : i; // compact index of the +x neighbour
+    const unsigned jm = s ? i : rowbase + xo; // compact index of the -x neighbour
+    const unsigned iyp = Lh * (yp + L * z) + xh, iym = Lh * (ym + L * z) + xh;
+    const unsigned izp = Lh * (y + L * zp) + xh, izm = Lh * (y + L * zm) + xh;
+
+    const BondT *__restrict__ Jc = (const BondT *)a.Jc;
+    const BondT *__restrict__ Jo = (const BondT *)a.Jo;
+    const unsigned Nh = lat.Nh;
+    const uint64_t sg = a.own[i];
+    const uint64_t n_xp = __ldg(a.oth + jp), n_xm = __ldg(a.oth + jm);
+    const uint64_t n_yp = __ldg(a.oth + iyp), n_ym = __ldg(a.oth + iym);
+    const uint64_t n_zp = __ldg(a.oth + izp), n_zm = __ldg(a.oth + izm);
+    const BondT j_xp = __ldg(Jc + i), j_yp = __ldg(Jc + Nh + i), j_zp = __ldg(Jc + 2 * Nh + i);
+    const BondT j_xm = __ldg(Jo + jm), j_ym = __ldg(Jo + Nh + iym), j_zm = __ldg(Jo + 2 * Nh + izm);
+
+    const SweepRng g = make_sweep_rng(a.seed, sweep_time(a), (uint32_t)a.colour);
+    const uint32_t site = (2 * xh + s) + L * (y + L * z); // canonical site index = Philox counter word 0
+    uint32_t r_lo, r_hi;
+    sweep_random(g, site, r_lo, r_hi);
+    a.own[i] = metropolis_word<BondT>(sg, n_xp, n_xm, n_yp, n_ym, n_zp, n_zm, j_xp, j_xm, j_yp, j_ym, j_zp, j_zm,
+                                      r_lo, r_hi, a.th);
+}
+
+// ---------------------------------------------------------------------------------------------
+// VEC2: two x-adjacent sites of one colour per thread; every access but one neighbour word and one
+// bond word per thread is a 128-bit (uint64 pairs) or 64-bit (uint32 bond pairs) vector.  L % 4 == 0.
+// ---------------------------------------------------------------------------------------------
+template <typename T> struct Pair;
+template <> struct Pair<uint64_t> { typedef ulonglong2 type; };
+template <> struct Pair<uint32_t> { typedef uint2 type; };
+
+template <typename BondT>
+__device__ __forceinline__ void ld_pair(const BondT *p, BondT &a, BondT &b)
+{
+    typename Pair<BondT>::type v = __ldg((const typename Pair<BondT>::type *)p);
+    a = v.x;
+    b = v.y;
+}
+
+template <typename BondT, bool POW2>
+__global__ void __launch_bounds__(256) k_sweep_vec2(const SweepArgs a)
+{
+    const Lattice lat = a.lat;
+    const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= lat.Nh / 2) return;
+    const unsigned L = lat.L, Lh = lat.Lh, W = Lh >> 1;
+    unsigned k, y, z;
+    decode_row<POW2>(lat, tid, lat.log2Lh - 1, W, k, y, z);
+    const unsigned s = (a.colour ^ (y + z)) & 1u;
+    const unsigned yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
+    const unsigned zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+    const unsigned rowbase = Lh * (y + L * z);
+    const unsigned i0 = rowbase + 2 * k;
+    // the one word outside the aligned pair: oth[2k-1] (s = 0, the -x neighbour of word 0) or oth[2k+2] (s = 1)
+    const unsigned xe = s ? ((2 * k + 2 == Lh) ? 0 : 2 * k + 2) : ((k == 0) ? Lh - 1 : 2 * k - 1);
+    const unsigned ie = rowbase + xe;
+    const unsigned iyp = Lh * (yp + L * z) + 2 * k, iym = Lh * (ym + L * z) + 2 * k;
+    const unsigned izp = Lh * (y + L * zp) + 2 * k, izm = Lh * (y + L * zm) + 2 * k;
+    const unsigned Nh = lat.Nh;
+    const BondT *__restrict__ Jc = (const BondT *)a.Jc;
+    const BondT *__restrict__ Jo = (const BondT *)a.Jo;
+
+    uint64_t sg0, sg1, A0, A1, yp0, yp1, ym0, ym1, zp0, zp1, zm0, zm1;
+    {
+        ulonglong2 v = *(const ulonglong2 *)(a.own + i0);
+        sg0 = v.x; sg1 = v.y;
+    }
+    ld_pair<uint64_t>(a.oth + i0, A0, A1);
+    const uint64_t ex = __ldg(a.oth + ie);
+    ld_pair<uint64_t>(a.oth + iyp, yp0, yp1);
+    ld_pair<uint64_t>(a.oth + iym, ym0, ym1);
+    ld_pair<uint64_t>(a.oth + izp, zp0, zp1);
+    ld_pair<uint64_t>(a.oth + izm, zm0, zm1);
+    BondT jx0, jx1, jy0, jy1, jz0, jz1, B0, B1, by0, by1, bz0, bz1;
+    ld_pair<BondT>(Jc + i0, jx0, jx1);
+    ld_pair<BondT>(Jc + Nh + i0, jy0, jy1);
+    ld_pair<BondT>(Jc + 2 * Nh + i0, jz0, jz1);
+    ld_pair<BondT>(Jo + i0, B0, B1);
+    const BondT Jex = __ldg(Jo + ie);
+    ld_pair<BondT>(Jo + Nh + iym, by0, by1);
+    ld_pair<BondT>(Jo + 2 * Nh + izm, bz0, bz1);
+
+    // (+x neighbour, -x neighbour, backward x bond) of the two words, by row phase s
+    const uint64_t np0 = s ? A1 : A0, nm0 = s ? A0 : ex;
+    const uint64_t np1 = s ? ex : A1, nm1 = s ? A1 : A0;
+    const BondT jm0 = s ? B0 : Jex, jm1 = s ? B1 : B0;
+
+    const SweepRng g = make_sweep_rng(a.seed, sweep_time(a), (uint32_t)a.colour);
+    const uint32_t site0 = (4 * k + s) + L * (y + L * z);
+    uint32_t r0l, r0h, r1l, r1h;
+    sweep_random(g, site0, r0l, r0h);
+    sweep_random(g, site0 + 2, r1l, r1h);
+    ulonglong2 out;
+    out.x = metropolis_word<BondT>(sg0, np0, nm0, yp0, ym0, zp0, zm0, jx0, jm0, jy0, by0, jz0, bz0, r0l, r0h, a.th);
+    out.y = metropolis_word<BondT>(sg1, np1, nm1, yp1, ym1, zp1, zm1, jx1, jm1, jy1, by1, jz1, bz1, r1l, r1h, a.th);
+    *(ulonglong2 *)(a.own + i0) = out;
+}
+
+__global__ void k_bump_time(uint64_t *d_time, uint32_t n) { *d_time += n; }
+
+// ---------------------------------------------------------------------------------------------
+template <typename BondT>
+static cudaError_t launch_typed(ea_sim *s, const SweepArgs &a, cudaStream_t st)
+{
+    const Lattice &lat = s->lat;
+    const bool pow2 = lat.log2L >= 0;
+    if (s->kernel == EA_KERNEL_VEC2) {
+        unsigned n = lat.Nh / 2, block = 256, grid = (n + block - 1) / block;
+        if (pow2) k_sweep_vec2<BondT, true><<<grid, block, 0, st>>>(a);
+        else k_sweep_vec2<BondT, false><<<grid, block, 0, st>>>(a);
+    } else {
+        unsigned n = lat.Nh, block = 256, grid = (n + block - 1) / block;
+        if (pow2) k_sweep_scalar<BondT, true><<<grid, block, 0, st>>>(a);
+        else k_sweep_scalar<BondT, false><<<grid, block, 0, st>>>(a);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_half_sweep(ea_sim *s, int parity, uint64_t t, const uint64_t *d_time, uint32_t t_offset,
+                              cudaStream_t st)
+{
+    SweepArgs a;
+    a.lat = s->lat;
+    a.colour = parity;
+    a.own = s->spins_c(parity);
+    a.oth = s->spins_c(1 - parity);
+    const size_t plane = (size_t)3 * s->lat.Nh * s->bond_bytes();
+    a.Jc = (const char *)s->bonds + (size_t)parity * plane;
+    a.Jo = (const char *)s->bonds + (size_t)(1 - parity) * plane;
+    a.seed = s->seed;
+    a.t = t;
+    a.d_time = d_time;
+    a.t_offset = t_offset;
+    a.th = s->th;
+    return s->n_replicas == 2 ? launch_typed<uint32_t>(s, a, st) : launch_typed<uint64_t>(s, a, st);
+}
+
+cudaError_t launch_bump_time(ea_sim *s, uint32_t n, cudaStream_t st)
+{
+    k_bump_time<<<1, 1, 0, st>>>(s->d_time, n);
+    return cudaGetLastError();
+}
+
+} // namespace ea

@@ -1,0 +1,84 @@
+"""Host-side checks of the C-ABI library (no GPU needed): it builds, loads, exports every symbol that
+include/ea.h declares, and fails loudly -- never falls back -- when there is no CUDA device."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_1411_5512_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.lib()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "ea.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(ea_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_header_symbols_are_all_exported_and_bound(lib):
+    names = declared_symbols()
+    assert len(names) >= 25
+    for n in names:
+        assert hasattr(lib, n), "libea_b200.so does not export %s" % n
+        assert n in binding.SIGNATURES, "binding.py does not marshal %s" % n
+    assert sorted(binding.SIGNATURES) == names
+
+
+def test_library_links_no_python_or_torch():
+    import subprocess
+    out = subprocess.run(["ldd", binding.LIB_PATH], capture_output=True, text=True).stdout
+    names = [line.split()[0] for line in out.splitlines() if line.strip()]
+    assert names and not any("torch" in n or "python" in n or "c10" in n for n in names), names
+
+
+def test_library_holds_sm100a_code():
+    import subprocess
+    out = subprocess.run(["cuobjdump", "-lelf", binding.LIB_PATH], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+
+
+def test_workspace_bytes_and_argument_validation(lib):
+    assert lib.ea_workspace_bytes(3, 1, 0) == 0          # odd L
+    assert lib.ea_workspace_bytes(0, 1, 0) == 0
+    assert lib.ea_workspace_bytes(8, 3, 0) == 0          # n_replicas
+    assert lib.ea_workspace_bytes(8, 1, -1) == 0
+    assert lib.ea_workspace_bytes(2048, 1, 0) == 0       # L^3 >= 2^31
+    n1 = lib.ea_workspace_bytes(128, 1, 2)
+    n2 = lib.ea_workspace_bytes(128, 2, 2)
+    N = 128 ** 3
+    assert n1 >= N * 8 * (1 + 3 + 2 + 1) and n1 < N * 8 * 7 + (1 << 20)
+    assert n1 - n2 == 3 * N * 4                          # 32-bit bond words in replica mode
+    h = C.c_void_p()
+    bad = [(7, 0.5, 0.8, 64), (8, 1.5, 0.8, 64), (8, 0.5, -1.0, 64), (8, 0.5, 0.8, 32), (8, float("nan"), 0.8, 64)]
+    for L, p, T, ns in bad:
+        assert lib.ea_create(L, p, T, ns, 1, C.byref(h)) == binding.EA_ERR_INVALID
+    assert lib.ea_strerror(binding.EA_ERR_STATE) == b"invalid state"
+    assert b"sm_100a" in lib.ea_version()
+
+
+def test_no_cpu_fallback_without_a_device(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("this check is for the GPU-less box")
+    h = C.c_void_p()
+    assert lib.ea_create(8, 0.5, 0.8, 64, 1, C.byref(h)) == binding.EA_ERR_CUDA
+    with pytest.raises(binding.EAError):
+        binding.Sim(8, 0.5, 0.8)
+
+
+def test_product_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1411_5512_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src, f
+                assert "ea_oracle" not in src, f

@@ -1,0 +1,334 @@
+"""GPU parity: the sm_100a path (through the C ABI) against the CPU oracle, element by element, bit-exact.
+
+Every test here needs a CUDA device (`-m gpu`).  Inputs are seeded and synthetic: the
+lattice is drawn inside each side from the written stream definition, or injected as plain random words.
+No expected value comes from the CUDA path.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import Oracle
+from paper_1411_5512_b200 import binding
+from paper_1411_5512_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = ["scalar", "vec2"]
+
+
+def kernels_for(L):
+    return [k for k in KERNELS if k == "scalar" or L % 4 == 0]
+
+
+def make_pair(L, p, T, n_rep, seed, n_slots=2, kernel="auto"):
+    g = binding.Sim(L, p, T, n_replicas=n_rep, seed=seed, n_slots=n_slots, kernel=kernel)
+    o = Oracle(L, p, T, n_replicas=n_rep, seed=seed, n_slots=n_slots)
+    return g, o
+
+
+def assert_same_state(g, o, what=""):
+    a, b = g.get_spins(), o.get_spins()
+    if not np.array_equal(a, b):
+        bad = np.flatnonzero(a != b)
+        raise AssertionError("%s: %d of %d spin words differ, first at site %d: gpu %016x oracle %016x"
+                             % (what, bad.size, a.size, bad[0], int(a[bad[0]]), int(b[bad[0]])))
+
+
+def assert_same_observables(g, o, slot=None):
+    assert np.array_equal(g.energy(), o.energy())
+    assert np.array_equal(g.magnetisation(), o.magnetisation())
+    if slot is not None:
+        A, Cn = g.autocorr(slot, with_C=True)
+        Ao = o.autocorr(slot)
+        assert np.array_equal(A, Ao)
+        np.testing.assert_allclose(Cn, Ao.astype(np.float64) / g.N, rtol=1e-12, atol=0)
+    if g.n_replicas == 2:
+        r_max = g.L // 2
+        B, q, avg = g.c4(r_max, with_q=True, with_avg=True)
+        Bo = o.c4(r_max)
+        assert np.array_equal(B, Bo)
+        assert np.array_equal(q, o.overlap())
+        ref = Bo.sum(axis=(0, 2)).astype(np.float64) / (3.0 * 32.0 * g.N)
+        np.testing.assert_allclose(avg, ref, rtol=1e-12, atol=0)
+
+
+# ----------------------------------------------------------------------------------------------------
+def test_philox_known_answers_on_the_device():
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "philox4x32_10_kat.txt")
+    n = 0
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        lhs, rhs = line.split("->")
+        v = [int(x, 16) for x in lhs.split()]
+        want = [int(x, 16) for x in rhs.split()]
+        assert binding.philox_selftest(v[:4], v[4:6]) == want
+        n += 1
+    assert n == 3
+    rng = np.random.default_rng(5)
+    for _ in range(50):  # random counters (any tag): device block == oracle block, folded stream == block
+        v = [int(x) for x in rng.integers(0, 2 ** 32, size=6)]
+        assert binding.philox_selftest(v[:4], v[4:6]) == [int(x) for x in oracle.philox4x32_10(v[:4], v[4:6])]
+
+
+@pytest.mark.parametrize("L,p,n_rep", [(2, 0.5, 1), (2, 0.3, 2), (4, 0.5, 2), (6, 0.77, 1), (8, 0.5, 1),
+                                       (10, 0.9, 2), (12, 0.5, 2), (16, 1.0, 2), (16, 0.0, 1), (32, 0.5, 2)])
+def test_initial_lattice_matches_the_oracle(L, p, n_rep):
+    g, o = make_pair(L, p, 0.8, n_rep, wl.seed_for(9, L))
+    assert np.array_equal(g.get_bonds(), o.get_bonds())
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    assert np.array_equal(g.thresholds, o.thresholds)
+    assert g.time == 0
+    assert_same_observables(g, o)
+
+
+@pytest.mark.parametrize("T", [0.0, 0.8, 2.0, float("inf")])
+def test_thresholds_match(T):
+    g = binding.Sim(4, 0.5, T)
+    assert [int(x) for x in g.thresholds] == [int(x) for x in oracle.thresholds(T)]
+
+
+@pytest.mark.parametrize("L,n_rep,T,sweeps", [(2, 1, 2.0, 200), (2, 2, 0.8, 200), (4, 1, 0.8, 200), (4, 2, 2.0, 200),
+                                               (6, 2, 0.8, 100), (8, 2, 2.0, 100), (10, 1, 0.8, 60), (12, 2, 0.8, 60),
+                                               (16, 1, 2.0, 60), (20, 2, 0.8, 30), (24, 1, 0.8, 30)])
+def test_sweeps_bit_exact_small_lattices_every_kernel(L, n_rep, T, sweeps):
+    for kern in kernels_for(L):
+        g, o = make_pair(L, 0.6, T, n_rep, wl.seed_for(8, L), kernel=kern)
+        done = 0
+        for chunk in (1, 1, 2, 5, sweeps):  # compare after every early sweep, then in bulk (graph path for >= 32)
+            n = min(chunk, sweeps - done)
+            if n <= 0:
+                break
+            g.sweep(n)
+            o.sweep(n)
+            done += n
+            assert g.time == o.time == done
+            assert_same_state(g, o, "L=%d %s after %d sweeps" % (L, kern, done))
+        assert_same_observables(g, o)
+
+
+def test_half_sweeps_match():
+    g, o = make_pair(8, 0.5, 1.5, 2, 77)
+    for parity in (0, 1, 1, 0):
+        g.half_sweep(parity)
+        o.half_sweep(parity)
+        assert_same_state(g, o, "half sweep parity %d" % parity)
+
+
+def test_cfg1_full_horizon_with_autocorrelation():
+    """BASELINE cfg1: L=8, p=0.5, T=0.8, 64 independent samples, 1000 sweeps, C(t,t_w) at t_w = 10, 100."""
+    c = wl.CONFIGS["cfg1"]
+    g, o = make_pair(c.L, c.p, c.T, c.n_replicas, c.seed)
+    marks = {10: 0, 100: 1}
+    t = 0
+    for t_next in [1, 2, 5, 10, 11, 12, 15, 20, 50, 100, 101, 110, 150, 200, 500, 1000]:
+        g.sweep(t_next - t)
+        o.sweep(t_next - t)
+        t = t_next
+        assert_same_state(g, o, "cfg1 t=%d" % t)
+        if t in marks:
+            g.snapshot(marks[t])
+            o.snapshot(marks[t])
+        for tw, slot in marks.items():
+            if t >= tw:
+                assert np.array_equal(g.autocorr(slot), o.autocorr(slot))
+                assert np.array_equal(g.get_snapshot(slot), o.get_snapshot(slot))
+    assert_same_observables(g, o, slot=1)
+
+
+def test_cfg2_replica_lattice_with_c4():
+    """BASELINE cfg2 (L=32, 32 disorders x 2 replicas): 300 sweeps, C and C_4 at t_w = 10, 100."""
+    c = wl.CONFIGS["cfg2"]
+    g, o = make_pair(c.L, c.p, c.T, c.n_replicas, c.seed)
+    t = 0
+    for t_next, slot in [(10, 0), (100, 1), (c.parity_sweeps, None)]:
+        g.sweep(t_next - t)
+        o.sweep(t_next - t)
+        t = t_next
+        assert_same_state(g, o, "cfg2 t=%d" % t)
+        if slot is not None:
+            g.snapshot(slot)
+            o.snapshot(slot)
+        assert_same_observables(g, o, slot=0)
+    assert_same_observables(g, o, slot=1)
+
+
+@pytest.mark.parametrize("name", ["cfg3a", "cfg3b"])
+def test_cfg3_energy_and_c4(name):
+    c = wl.CONFIGS[name]
+    g, o = make_pair(c.L, c.p, c.T, c.n_replicas, c.seed, n_slots=1)
+    assert np.array_equal(g.get_bonds(), o.get_bonds())
+    for n in (1, 7, c.parity_sweeps - 8):
+        g.sweep(n)
+        o.sweep(n)
+        assert_same_state(g, o, "%s t=%d" % (name, g.time))
+        assert np.array_equal(g.energy(), o.energy())
+    assert_same_observables(g, o)
+
+
+@pytest.mark.parametrize("name", ["cfg4", "cfg5_p0.5_T0.8", "cfg5_p1.0_T2.0"])
+def test_full_size_L128_every_word(name):
+    """The bench configuration (L=128, 32 x 2 replicas), AUTO kernel as bench.py launches it: every spin word
+    and every integer observable after a few sweeps."""
+    c = wl.CONFIGS[name]
+    g, o = make_pair(c.L, c.p, c.T, c.n_replicas, c.seed, n_slots=1)
+    assert np.array_equal(g.get_bonds(), o.get_bonds())
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    g.snapshot(0)
+    o.snapshot(0)
+    n = c.parity_sweeps
+    g.sweep(n)
+    o.sweep(n)
+    assert_same_state(g, o, "%s t=%d" % (name, n))
+    assert_same_observables(g, o, slot=0)
+
+
+def test_graph_replay_path_and_composition():
+    """sweep(a); sweep(b) == sweep(a+b), including the CUDA-graph path (n >= 32) and its remainder."""
+    L, seed = 8, 4242
+    a = binding.Sim(L, 0.5, 0.8, n_replicas=2, seed=seed)
+    b = binding.Sim(L, 0.5, 0.8, n_replicas=2, seed=seed)
+    o = Oracle(L, 0.5, 0.8, n_replicas=2, seed=seed)
+    a.sweep(137)                      # 4 replays + 9 direct
+    for n in (3, 64, 1, 33, 36):      # mixed
+        b.sweep(n)
+    o.sweep(137)
+    assert a.time == b.time == 137
+    assert np.array_equal(a.get_spins(), b.get_spins())
+    assert_same_state(a, o, "graph path")
+
+
+def test_sweep_counter_beyond_32_bits():
+    """The sweep index enters the Philox counter as (t lo32, t hi32): cross 2^32 on both launch paths."""
+    L, seed, t0 = 6, 99, 2 ** 32 - 20
+    g, o = make_pair(L, 0.5, 1.0, 2, seed)
+    g.time = t0
+    o.time = t0
+    g.sweep(45)   # graph replay spans the boundary
+    o.sweep(45)
+    assert g.time == o.time == t0 + 45
+    assert_same_state(g, o, "t across 2^32")
+    g2 = binding.Sim(L, 0.5, 1.0, n_replicas=2, seed=seed)
+    o2 = Oracle(L, 0.5, 1.0, n_replicas=2, seed=seed)
+    g2.time = o2.time = 2 ** 40 + 5
+    g2.sweep(3)
+    o2.sweep(3)
+    assert_same_state(g2, o2, "t = 2^40")
+
+
+def test_injected_lattice_and_gauge_equivalence_on_the_device():
+    """set_spins / set_bonds with plain random words; and pin P7 on the GPU itself: the gauge-transformed
+    lattice follows the gauge-transformed trajectory exactly."""
+    L, N = 8, 512
+    spins = wl.random_words(N, 1)
+    bonds = wl.random_bond_words(N, 0.6, 1, 2)
+    eps = wl.random_words(N, 3)
+    g = binding.Sim(L, 0.5, 1.2, n_replicas=1, seed=5)
+    o = Oracle(L, 0.5, 1.2, n_replicas=1, seed=5)
+    g.set_spins(spins); g.set_bonds(bonds)
+    o.set_spins(spins); o.set_bonds(bonds)
+    assert np.array_equal(g.get_bonds(), bonds) and np.array_equal(g.get_spins(), spins)
+    e3 = eps.reshape(L, L, L)  # [z][y][x]
+    gb = bonds.copy().reshape(3, L, L, L)
+    for d, axis in ((0, 2), (1, 1), (2, 0)):
+        gb[d] ^= e3 ^ np.roll(e3, -1, axis=axis)
+    h = binding.Sim(L, 0.5, 1.2, n_replicas=1, seed=5)
+    h.set_spins(spins ^ eps); h.set_bonds(gb.reshape(-1))
+    for n in (1, 9, 40):
+        g.sweep(n); o.sweep(n); h.sweep(n)
+        assert_same_state(g, o, "injected lattice")
+        assert np.array_equal(h.get_spins(), g.get_spins() ^ eps)
+    assert np.array_equal(h.energy(), g.energy())
+
+
+def test_replica_bonds_must_have_equal_halves():
+    g = binding.Sim(4, 0.5, 0.8, n_replicas=2, seed=1)
+    bad = wl.random_bond_words(64, 0.5, 1, 7)
+    with pytest.raises(binding.EAError) as e:
+        g.set_bonds(bad)
+    assert e.value.status == binding.EA_ERR_INVALID
+    good = wl.random_bond_words(64, 0.5, 2, 7)
+    g.set_bonds(good)
+    assert np.array_equal(g.get_bonds(), good)
+
+
+@pytest.mark.parametrize("L", [4, 8, 12])
+def test_limits_T0_Tinf_p1(L):
+    N = L ** 3
+    # T = inf: every spin flips every sweep (thr = 2^32 path)
+    g = binding.Sim(L, 0.5, float("inf"), n_replicas=1, seed=3, n_slots=1)
+    s0 = g.get_spins()
+    g.snapshot(0)
+    g.sweep(1)
+    assert np.array_equal(g.get_spins(), ~s0)
+    assert np.all(g.autocorr(0) == -N)
+    g.sweep(35)
+    assert np.array_equal(g.get_spins(), s0)
+    # T = 0: energy never increases; matches the oracle
+    g, o = make_pair(L, 0.5, 0.0, 2, 11)
+    E = g.energy()
+    for _ in range(6):
+        g.sweep(1); o.sweep(1)
+        E2 = g.energy()
+        assert np.all(E2 <= E)
+        E = E2
+    assert_same_state(g, o, "T=0")
+    # p = 1 ferromagnet: all-up is the ground state E = -3N, a fixed point at T = 0
+    g = binding.Sim(L, 1.0, 0.0, n_replicas=1, seed=2)
+    assert not g.get_bonds().any()
+    g.set_spins(np.zeros(N, dtype=np.uint64))
+    g.sweep(3)
+    assert not g.get_spins().any()
+    assert np.all(g.energy() == -3 * N) and np.all(g.magnetisation() == N)
+
+
+def test_set_temperature_and_kernel_switch_mid_run():
+    g, o = make_pair(8, 0.5, 0.8, 2, 31)
+    g.sweep(40); o.sweep(40)
+    g.set_temperature(2.0); o.set_temperature(2.0)
+    g.kernel = "scalar"
+    g.sweep(40); o.sweep(40)
+    g.kernel = "vec2"
+    g.sweep(3); o.sweep(3)
+    assert_same_state(g, o, "after T / kernel switch")
+
+
+def test_resume_from_saved_state():
+    L, seed = 8, 17
+    a = binding.Sim(L, 0.5, 0.8, n_replicas=2, seed=seed)
+    a.sweep(50)
+    spins, bonds, t = a.get_spins(), a.get_bonds(), a.time
+    a.sweep(50)
+    b = binding.Sim(L, 0.9, 0.8, n_replicas=2, seed=seed)  # other bonds until restored
+    b.set_bonds(bonds); b.set_spins(spins); b.time = t
+    b.sweep(50)
+    assert np.array_equal(a.get_spins(), b.get_spins())
+
+
+def test_error_codes():
+    g = binding.Sim(4, 0.5, 0.8, n_replicas=1, seed=1, n_slots=1)
+    for call, status in [(lambda: g.autocorr(0), binding.EA_ERR_STATE), (lambda: g.autocorr(5), binding.EA_ERR_INVALID),
+                         (lambda: g.snapshot(1), binding.EA_ERR_INVALID), (lambda: g.c4(1), binding.EA_ERR_STATE),
+                         (lambda: g.half_sweep(2), binding.EA_ERR_INVALID),
+                         (lambda: g.set_temperature(-1.0), binding.EA_ERR_INVALID)]:
+        with pytest.raises(binding.EAError) as e:
+            call()
+        assert e.value.status == status
+    g2 = binding.Sim(6, 0.5, 0.8, n_replicas=2, seed=1)
+    with pytest.raises(binding.EAError):
+        g2.c4(4)          # r_max > L/2
+    with pytest.raises(binding.EAError):
+        g2.kernel = "vec2"  # L % 4 != 0
+    with pytest.raises(binding.EAError):
+        binding.Sim(6, 0.5, 0.8, kernel="vec2")
+
+
+def test_caller_stream_and_library_workspace():
+    import torch
+    st = torch.cuda.Stream()
+    a = binding.Sim(8, 0.5, 0.8, n_replicas=2, seed=3, stream=st)
+    b = binding.Sim(8, 0.5, 0.8, n_replicas=2, seed=3, torch_workspace=False)
+    a.sweep(70); b.sweep(70)
+    assert np.array_equal(a.get_spins(), b.get_spins())
