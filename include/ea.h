@@ -98,6 +98,8 @@ ea_status ea_get_thresholds(const ea_sim *sim, uint64_t thr[3]); /* thr[n_u], n_
 ea_status ea_set_kernel(ea_sim *sim, int kernel);      /* EA_ERR_INVALID if not valid for this L  */
 ea_status ea_get_kernel(const ea_sim *sim, int *kernel); /* the variant AUTO resolved to          */
 ea_status ea_synchronize(ea_sim *sim);                 /* wait for the sim's stream               */
+/* Kernels this sim has launched on the device since ea_create (a CUDA-graph replay counts its kernel nodes). */
+ea_status ea_get_launch_count(const ea_sim *sim, uint64_t *n);
 
 /* Keep sigma(t) in slot (device copy; the paper wrote configurations to disk). */
 ea_status ea_snapshot(ea_sim *sim, int slot);

@@ -47,6 +47,7 @@ SIGNATURES = {
     "ea_set_kernel": (_i, [_vp, _i]),
     "ea_get_kernel": (_i, [_vp, C.POINTER(_i)]),
     "ea_synchronize": (_i, [_vp]),
+    "ea_get_launch_count": (_i, [_vp, C.POINTER(_u64)]),
     "ea_snapshot": (_i, [_vp, _i]),
     "ea_autocorr": (_i, [_vp, _i, _vp, _vp]),
     "ea_c4": (_i, [_vp, _i, _vp, _vp, _vp]),
@@ -149,6 +150,12 @@ class Sim:
 
     def synchronize(self):
         self._ck(lib().ea_synchronize(self._h))
+
+    @property
+    def launch_count(self):
+        n = _u64()
+        self._ck(lib().ea_get_launch_count(self._h, C.byref(n)))
+        return n.value
 
     @property
     def time(self):

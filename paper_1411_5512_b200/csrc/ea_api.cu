@@ -241,12 +241,14 @@ static ea_status build_graph(ea_sim *s)
     cudaGraph_t graph = nullptr;
     EA_CUDA(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
     cudaError_t e = cudaSuccess;
+    s->capturing = true; // captured nodes are counted per replay, not here
     for (int k = 0; k < GRAPH_SWEEPS && e == cudaSuccess; ++k) {
         e = launch_half_sweep(s, 0, 0, s->d_time, (uint32_t)k, s->stream);
         if (e == cudaSuccess) e = launch_half_sweep(s, 1, 0, s->d_time, (uint32_t)k, s->stream);
     }
     if (e == cudaSuccess) e = launch_bump_time(s, GRAPH_SWEEPS, s->stream);
     cudaError_t e2 = cudaStreamEndCapture(s->stream, &graph);
+    s->capturing = false;
     if (e != cudaSuccess || e2 != cudaSuccess) {
         if (graph) cudaGraphDestroy(graph);
         EA_FAIL(s, EA_ERR_CUDA, "graph capture: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
@@ -276,6 +278,7 @@ ea_status ea_sweep(ea_sim *sim, uint64_t n)
         EA_CUDA(sim, cudaMemcpyAsync(sim->d_time, &sim->t, 8, cudaMemcpyHostToDevice, sim->stream));
         while (left >= (uint64_t)sim->graph_sweeps) {
             EA_CUDA(sim, cudaGraphLaunch(sim->graph_exec, sim->stream));
+            sim->count_launch(2 * sim->graph_sweeps + 1);
             sim->t += sim->graph_sweeps;
             left -= sim->graph_sweeps;
         }
@@ -342,6 +345,13 @@ ea_status ea_get_kernel(const ea_sim *sim, int *kernel)
 {
     if (!sim || !kernel) return EA_ERR_INVALID;
     *kernel = sim->kernel;
+    return EA_OK;
+}
+
+ea_status ea_get_launch_count(const ea_sim *sim, uint64_t *n)
+{
+    if (!sim || !n) return EA_ERR_INVALID;
+    *n = sim->launches;
     return EA_OK;
 }
 

@@ -41,6 +41,11 @@ struct ea_sim {
     int graph_kernel = -1;
     uint64_t *d_time = nullptr;   // device copy of t consumed by graph-launched kernels
 
+    // kernels this sim has put on the device (a graph replay counts its kernel nodes); bench.py's gpu_launches
+    uint64_t launches = 0;
+    bool capturing = false;
+    void count_launch(unsigned n = 1) { if (!capturing) launches += n; }
+
     std::string err;
 
     int bond_bytes() const { return n_replicas == 2 ? 4 : 8; }

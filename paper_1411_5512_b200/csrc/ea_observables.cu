@@ -145,6 +145,7 @@ cudaError_t launch_count_spins(ea_sim *s, const uint64_t *d_other)
     cudaError_t e = cudaMemsetAsync(s->counters, 0, 64 * sizeof(unsigned long long), s->stream);
     if (e != cudaSuccess) return e;
     k_count_spins<<<grid_for(s, s->N), 256, 0, s->stream>>>(s->lat, s->spins, d_other, s->counters);
+    s->count_launch();
     return cudaGetLastError();
 }
 
@@ -156,6 +157,7 @@ cudaError_t launch_count_energy(ea_sim *s)
         k_count_energy<uint32_t><<<grid_for(s, s->N), 256, 0, s->stream>>>(s->lat, s->spins, (const uint32_t *)s->bonds, s->counters);
     else
         k_count_energy<uint64_t><<<grid_for(s, s->N), 256, 0, s->stream>>>(s->lat, s->spins, (const uint64_t *)s->bonds, s->counters);
+    s->count_launch();
     return cudaGetLastError();
 }
 
@@ -167,6 +169,7 @@ cudaError_t launch_count_c4(ea_sim *s, int r_max)
     size_t need = ((size_t)s->N + 255) / 256, cap = (size_t)s->n_sm * 2;
     dim3 grid((unsigned)(need < cap ? need : cap), (unsigned)jobs);
     k_count_c4<<<grid, 256, 0, s->stream>>>(s->lat, s->spins, r_max, s->counters);
+    s->count_launch();
     return cudaGetLastError();
 }
 

@@ -112,6 +112,7 @@ cudaError_t launch_init_spins(ea_sim *s)
 {
     size_t n = 2 * (size_t)s->lat.Nh;
     k_init_spins<<<blocks_for(n, 256), 256, 0, s->stream>>>(s->lat, s->spins, s->seed);
+    s->count_launch();
     return cudaGetLastError();
 }
 
@@ -126,18 +127,21 @@ cudaError_t launch_init_bonds(ea_sim *s)
         k_init_bonds<uint32_t><<<blocks_for(n, 256), 256, 0, s->stream>>>(s->lat, (uint32_t *)s->bonds, s->seed, P);
     else
         k_init_bonds<uint64_t><<<blocks_for(n, 256), 256, 0, s->stream>>>(s->lat, (uint64_t *)s->bonds, s->seed, P);
+    s->count_launch();
     return cudaGetLastError();
 }
 
 cudaError_t launch_pack_spins(ea_sim *s, const uint64_t *d_canon, uint64_t *d_internal)
 {
     k_pack_spins<<<blocks_for(s->N, 256), 256, 0, s->stream>>>(s->lat, d_canon, d_internal);
+    s->count_launch();
     return cudaGetLastError();
 }
 
 cudaError_t launch_unpack_spins(ea_sim *s, const uint64_t *d_internal, uint64_t *d_canon)
 {
     k_unpack_spins<<<blocks_for(s->N, 256), 256, 0, s->stream>>>(s->lat, d_internal, d_canon);
+    s->count_launch();
     return cudaGetLastError();
 }
 
@@ -147,6 +151,7 @@ cudaError_t launch_pack_bonds(ea_sim *s, int d, const uint64_t *d_canon)
         k_pack_bonds<uint32_t><<<blocks_for(s->N, 256), 256, 0, s->stream>>>(s->lat, d, d_canon, (uint32_t *)s->bonds);
     else
         k_pack_bonds<uint64_t><<<blocks_for(s->N, 256), 256, 0, s->stream>>>(s->lat, d, d_canon, (uint64_t *)s->bonds);
+    s->count_launch();
     return cudaGetLastError();
 }
 
@@ -156,6 +161,7 @@ cudaError_t launch_unpack_bonds(ea_sim *s, int d, uint64_t *d_canon)
         k_unpack_bonds<uint32_t><<<blocks_for(s->N, 256), 256, 0, s->stream>>>(s->lat, d, (const uint32_t *)s->bonds, d_canon);
     else
         k_unpack_bonds<uint64_t><<<blocks_for(s->N, 256), 256, 0, s->stream>>>(s->lat, d, (const uint64_t *)s->bonds, d_canon);
+    s->count_launch();
     return cudaGetLastError();
 }
 

@@ -178,6 +178,7 @@ static cudaError_t launch_typed(ea_sim *s, const SweepArgs &a, cudaStream_t st)
         if (pow2) k_sweep_scalar<BondT, true><<<grid, block, 0, st>>>(a);
         else k_sweep_scalar<BondT, false><<<grid, block, 0, st>>>(a);
     }
+    s->count_launch();
     return cudaGetLastError();
 }
 
@@ -203,6 +204,7 @@ cudaError_t launch_half_sweep(ea_sim *s, int parity, uint64_t t, const uint64_t 
 cudaError_t launch_bump_time(ea_sim *s, uint32_t n, cudaStream_t st)
 {
     k_bump_time<<<1, 1, 0, st>>>(s->d_time, n);
+    s->count_launch();
     return cudaGetLastError();
 }
 
