@@ -86,13 +86,15 @@ static bool kernel_valid_for(int kernel, int L)
     switch (kernel) {
     case EA_KERNEL_SCALAR: return true;
     case EA_KERNEL_VEC2: return L % 4 == 0;
+    case EA_KERNEL_ROWS: return L == 16 || L == 32 || L == 64 || L == 128;
     default: return false;
     }
 }
 
 static int resolve_kernel(int kernel, int L)
 {
-    if (kernel == EA_KERNEL_AUTO) return L % 4 == 0 ? EA_KERNEL_VEC2 : EA_KERNEL_SCALAR;
+    if (kernel == EA_KERNEL_AUTO)
+        return kernel_valid_for(EA_KERNEL_ROWS, L) ? EA_KERNEL_ROWS : L % 4 == 0 ? EA_KERNEL_VEC2 : EA_KERNEL_SCALAR;
     return kernel;
 }
 

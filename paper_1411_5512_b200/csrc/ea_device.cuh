@@ -139,26 +139,26 @@ __device__ __forceinline__ uint32_t xor3(uint32_t a, uint32_t b, uint32_t c) { r
 __device__ __forceinline__ uint32_t maj3(uint32_t a, uint32_t b, uint32_t c) { return (a & b) | (c & (a | b)); }
 
 // One 32-sample half of one Metropolis trial (Eq. 9; "boolean logic at the bit level").
-// u1..u6: unsatisfied-bond words j ^ sigma_i ^ sigma_nbr (C-A2, C-A3).  Bit-sliced count n_u = (c2 c1 c0),
-// nested level masks m0 <= m1 <= m2 (m_k = all ones iff r < thr[k]): flip iff n_u + level >= 3, i.e.
-//   f = [n_u>=3] | m2 & [n_u>=2] | m1 & [n_u>=1] | m0.
-__device__ __forceinline__ uint32_t flip_mask(uint32_t u1, uint32_t u2, uint32_t u3, uint32_t u4, uint32_t u5,
-                                              uint32_t u6, uint32_t m0, uint32_t m1, uint32_t m2)
+// u1..u6: unsatisfied-bond words j ^ sigma_i ^ sigma_nbr (C-A2, C-A3).  Two full adders give
+// a = u1+u2+u3 = sa + 2 ka and b = u4+u5+u6 = sb + 2 kb, n_u = a + b.  With t = sa | sb:
+//   [n_u >= 3] = maj(ka, kb, t),  [n_u >= 2] = ka | kb | (sa & sb),  [n_u >= 1] = ka | kb | t.
+// The thresholds are nested (thr[0] <= thr[1] <= thr[2]), so
+//   f = [n_u >= 3] | [r < thr[2]] [n_u >= 2] | [r < thr[1]] [n_u >= 1] | [r < thr[0]]
+// and each rare term is one or two predicated LOP3 behind an ISETP (no masks are materialised).
+// ALWAYS: some thr[k] == 2^32 (T = inf), which a 32-bit compare cannot express -- OR-ed in as masks.
+template <bool ALWAYS>
+__device__ __forceinline__ uint32_t flip_half(uint32_t u1, uint32_t u2, uint32_t u3, uint32_t u4, uint32_t u5,
+                                              uint32_t u6, uint32_t r, const Thresholds &th)
 {
-    uint32_t sa = xor3(u1, u2, u3), ka = maj3(u1, u2, u3);
-    uint32_t sb = xor3(u4, u5, u6), kb = maj3(u4, u5, u6);
-    uint32_t c0 = sa ^ sb, kc = sa & sb;
-    uint32_t c1 = xor3(ka, kb, kc), c2 = maj3(ka, kb, kc);
-    uint32_t a = c1 & (c0 | m2);     // n_u = 3, or n_u = 2 with level >= 1
-    uint32_t b = a | (m1 & c0);      // n_u = 1 with level >= 2 (m1 & c1 is inside m2 & c1 because m1 <= m2)
-    return b | c2 | m0;              // n_u >= 4; level 3
-}
-
-__device__ __forceinline__ void level_masks(const Thresholds &th, uint32_t r, uint32_t &m0, uint32_t &m1, uint32_t &m2)
-{
-    m0 = (r < th.thr[0] ? 0xffffffffu : 0u) | th.always[0];
-    m1 = (r < th.thr[1] ? 0xffffffffu : 0u) | th.always[1];
-    m2 = (r < th.thr[2] ? 0xffffffffu : 0u) | th.always[2];
+    const uint32_t sa = xor3(u1, u2, u3), ka = maj3(u1, u2, u3);
+    const uint32_t sb = xor3(u4, u5, u6), kb = maj3(u4, u5, u6);
+    const uint32_t t = sa | sb;
+    uint32_t f = maj3(ka, kb, t);
+    if (r < th.thr[2]) f = ka | kb | (sa & sb);
+    if (r < th.thr[1]) f = ka | kb | t;
+    if (r < th.thr[0]) f = 0xffffffffu;
+    if (ALWAYS) f |= (th.always[2] & (ka | kb | (sa & sb))) | (th.always[1] & (ka | kb | t)) | th.always[0];
+    return f;
 }
 
 // 64-bit word <-> halves
@@ -172,23 +172,21 @@ __device__ __forceinline__ uint32_t bond_hi(uint64_t j) { return (uint32_t)(j >>
 __device__ __forceinline__ uint32_t bond_lo(uint32_t j) { return j; }
 __device__ __forceinline__ uint32_t bond_hi(uint32_t j) { return j; } // replica (b) sees the same bonds
 
-// One whole Metropolis trial of a 64-sample word: returns the new spin word.
-template <typename BondT>
+// One whole Metropolis trial of a 64-sample word: returns the new spin word.  (n_d, j_d), d = 1..6: the six
+// neighbour words with the bond word that couples each to this site, in any order (n_u is a count).
+template <typename BondT, bool ALWAYS>
 __device__ __forceinline__ uint64_t metropolis_word(uint64_t s, uint64_t n1, uint64_t n2, uint64_t n3, uint64_t n4,
                                                     uint64_t n5, uint64_t n6, BondT j1, BondT j2, BondT j3, BondT j4,
                                                     BondT j5, BondT j6, uint32_t r_lo, uint32_t r_hi,
                                                     const Thresholds &th)
 {
-    uint32_t sl = lo32(s), sh = hi32(s);
-    uint32_t m0, m1, m2;
-    level_masks(th, r_lo, m0, m1, m2);
-    uint32_t fl = flip_mask(bond_lo(j1) ^ sl ^ lo32(n1), bond_lo(j2) ^ sl ^ lo32(n2), bond_lo(j3) ^ sl ^ lo32(n3),
-                            bond_lo(j4) ^ sl ^ lo32(n4), bond_lo(j5) ^ sl ^ lo32(n5), bond_lo(j6) ^ sl ^ lo32(n6),
-                            m0, m1, m2);
-    level_masks(th, r_hi, m0, m1, m2);
-    uint32_t fh = flip_mask(bond_hi(j1) ^ sh ^ hi32(n1), bond_hi(j2) ^ sh ^ hi32(n2), bond_hi(j3) ^ sh ^ hi32(n3),
-                            bond_hi(j4) ^ sh ^ hi32(n4), bond_hi(j5) ^ sh ^ hi32(n5), bond_hi(j6) ^ sh ^ hi32(n6),
-                            m0, m1, m2);
+    const uint32_t sl = lo32(s), sh = hi32(s);
+    const uint32_t fl = flip_half<ALWAYS>(bond_lo(j1) ^ sl ^ lo32(n1), bond_lo(j2) ^ sl ^ lo32(n2),
+                                          bond_lo(j3) ^ sl ^ lo32(n3), bond_lo(j4) ^ sl ^ lo32(n4),
+                                          bond_lo(j5) ^ sl ^ lo32(n5), bond_lo(j6) ^ sl ^ lo32(n6), r_lo, th);
+    const uint32_t fh = flip_half<ALWAYS>(bond_hi(j1) ^ sh ^ hi32(n1), bond_hi(j2) ^ sh ^ hi32(n2),
+                                          bond_hi(j3) ^ sh ^ hi32(n3), bond_hi(j4) ^ sh ^ hi32(n4),
+                                          bond_hi(j5) ^ sh ^ hi32(n5), bond_hi(j6) ^ sh ^ hi32(n6), r_hi, th);
     return mk64(sl ^ fl, sh ^ fh);
 }
 

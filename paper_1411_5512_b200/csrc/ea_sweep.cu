@@ -48,7 +48,7 @@ __device__ __forceinline__ void decode_row(const Lattice &lat, unsigned tid, uns
 // SCALAR: one site per thread, any even L >= 2 (L = 2: +x and -x neighbours are the same site,
 // reached through two distinct bonds -- C-S15).
 // ---------------------------------------------------------------------------------------------
-template <typename BondT, bool POW2>
+template <typename BondT, bool POW2, bool ALWAYS>
 __global__ void __launch_bounds__(256) k_sweep_scalar(const SweepArgs a)
 {
     const Lattice lat = a.lat;
@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(256) k_sweep_scalar(const SweepArgs a)
     const uint32_t site = (2 * xh + s) + L * (y + L * z); // canonical site index = Philox counter word 0
     uint32_t r_lo, r_hi;
     sweep_random(g, site, r_lo, r_hi);
-    a.own[i] = metropolis_word<BondT>(sg, n_xp, n_xm, n_yp, n_ym, n_zp, n_zm, j_xp, j_xm, j_yp, j_ym, j_zp, j_zm,
+    a.own[i] = metropolis_word<BondT, ALWAYS>(sg, n_xp, n_xm, n_yp, n_ym, n_zp, n_zm, j_xp, j_xm, j_yp, j_ym, j_zp, j_zm,
                                       r_lo, r_hi, a.th);
 }
 
@@ -102,7 +102,7 @@ __device__ __forceinline__ void ld_pair(const BondT *p, BondT &a, BondT &b)
     b = v.y;
 }
 
-template <typename BondT, bool POW2>
+template <typename BondT, bool POW2, bool ALWAYS>
 __global__ void __launch_bounds__(256) k_sweep_vec2(const SweepArgs a)
 {
     const Lattice lat = a.lat;
@@ -156,30 +156,161 @@ __global__ void __launch_bounds__(256) k_sweep_vec2(const SweepArgs a)
     sweep_random(g, site0, r0l, r0h);
     sweep_random(g, site0 + 2, r1l, r1h);
     ulonglong2 out;
-    out.x = metropolis_word<BondT>(sg0, np0, nm0, yp0, ym0, zp0, zm0, jx0, jm0, jy0, by0, jz0, bz0, r0l, r0h, a.th);
-    out.y = metropolis_word<BondT>(sg1, np1, nm1, yp1, ym1, zp1, zm1, jx1, jm1, jy1, by1, jz1, bz1, r1l, r1h, a.th);
+    out.x = metropolis_word<BondT, ALWAYS>(sg0, np0, nm0, yp0, ym0, zp0, zm0, jx0, jm0, jy0, by0, jz0, bz0, r0l, r0h, a.th);
+    out.y = metropolis_word<BondT, ALWAYS>(sg1, np1, nm1, yp1, ym1, zp1, zm1, jx1, jm1, jy1, by1, jz1, bz1, r1l, r1h, a.th);
     *(ulonglong2 *)(a.own + i0) = out;
 }
 
 __global__ void k_bump_time(uint64_t *d_time, uint32_t n) { *d_time += n; }
 
 // ---------------------------------------------------------------------------------------------
+// ROWS: a warp owns whole x-rows (L/4 lanes per row, two words per lane) and marches M rows along y, keeping
+// the other colour's rows y-1, y, y+1 in registers (each is loaded once instead of three times).  The row
+// phase s = (colour ^ (y + z)) & 1 alternates along y, so the march is unrolled by two with s a compile-time
+// constant: no selects, and the one x-neighbour word outside the lane's aligned pair comes from the adjacent
+// lane by a warp shuffle (the periodic wrap in x is a rotation inside the row's lane group).
+// L in {16, 32, 64, 128} (L/4 lanes per row must divide the warp), L a compile-time constant so every row
+// stride is an immediate.  A warp with several rows (L < 128) takes rows of equal z parity, which keeps s
+// warp-uniform.
+// ---------------------------------------------------------------------------------------------
 template <typename BondT>
+__device__ __forceinline__ typename Pair<BondT>::type ldg_pair(const BondT *p)
+{
+    return __ldg((const typename Pair<BondT>::type *)p);
+}
+
+__device__ __forceinline__ uint64_t shfl64(uint64_t v, int src)
+{
+    uint32_t lo = __shfl_sync(0xffffffffu, lo32(v), src), hi = __shfl_sync(0xffffffffu, hi32(v), src);
+    return mk64(lo, hi);
+}
+__device__ __forceinline__ uint32_t shfl_bond(uint32_t v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+__device__ __forceinline__ uint64_t shfl_bond(uint64_t v, int src) { return shfl64(v, src); }
+
+template <int S, typename BondT, bool ALWAYS>
+__device__ __forceinline__ ulonglong2 update_pair(const ulonglong2 own, const ulonglong2 P0, const ulonglong2 Pm,
+                                                  const ulonglong2 Pp, const ulonglong2 Zm, const ulonglong2 Zp,
+                                                  const typename Pair<BondT>::type jx,
+                                                  const typename Pair<BondT>::type jy,
+                                                  const typename Pair<BondT>::type jz,
+                                                  const typename Pair<BondT>::type bx,
+                                                  const typename Pair<BondT>::type by,
+                                                  const typename Pair<BondT>::type bz, const uint32_t site0,
+                                                  const SweepRng &g, const Thresholds &th, const int lane_m,
+                                                  const int lane_p)
+{
+    uint32_t r0l, r0h, r1l, r1h;
+    sweep_random(g, site0, r0l, r0h);
+    sweep_random(g, site0 + 2, r1l, r1h);
+    ulonglong2 out;
+    if (S == 0) { // own x = 4k, 4k+2; other colour at 4k+1 (P0.x), 4k+3 (P0.y), 4k-1 (left lane's P0.y)
+        const uint64_t ex = shfl64(P0.y, lane_m);
+        const BondT jex = shfl_bond((BondT)bx.y, lane_m);
+        out.x = metropolis_word<BondT, ALWAYS>(own.x, P0.x, ex, Pp.x, Pm.x, Zp.x, Zm.x, (BondT)jx.x, jex, (BondT)jy.x,
+                                               (BondT)by.x, (BondT)jz.x, (BondT)bz.x, r0l, r0h, th);
+        out.y = metropolis_word<BondT, ALWAYS>(own.y, P0.y, P0.x, Pp.y, Pm.y, Zp.y, Zm.y, (BondT)jx.y, (BondT)bx.x,
+                                               (BondT)jy.y, (BondT)by.y, (BondT)jz.y, (BondT)bz.y, r1l, r1h, th);
+    } else {      // own x = 4k+1, 4k+3; other colour at 4k (P0.x), 4k+2 (P0.y), 4k+4 (right lane's P0.x)
+        const uint64_t ex = shfl64(P0.x, lane_p);
+        out.x = metropolis_word<BondT, ALWAYS>(own.x, P0.y, P0.x, Pp.x, Pm.x, Zp.x, Zm.x, (BondT)jx.x, (BondT)bx.x,
+                                               (BondT)jy.x, (BondT)by.x, (BondT)jz.x, (BondT)bz.x, r0l, r0h, th);
+        out.y = metropolis_word<BondT, ALWAYS>(own.y, ex, P0.y, Pp.y, Pm.y, Zp.y, Zm.y, (BondT)jx.y, (BondT)bx.y,
+                                               (BondT)jy.y, (BondT)by.y, (BondT)jz.y, (BondT)bz.y, r1l, r1h, th);
+    }
+    return out;
+}
+
+template <int L, int M, int S0, typename BondT, bool ALWAYS>
+__device__ __forceinline__ void march_rows(const SweepArgs &a, const SweepRng &g, const unsigned y0, const unsigned z,
+                                           const unsigned k, const int lane_m, const int lane_p)
+{
+    constexpr unsigned Lh = L / 2, Nh = (unsigned)L * L * L / 2, ZS = Lh * L; // row and plane strides (words)
+    const BondT *__restrict__ Jc = (const BondT *)a.Jc;
+    const BondT *__restrict__ Jo = (const BondT *)a.Jo;
+    const unsigned zb = ZS * z + 2 * k, zbm = ZS * ((z - 1) & (L - 1)) + 2 * k, zbp = ZS * ((z + 1) & (L - 1)) + 2 * k;
+    ulonglong2 Pm = ldg_pair<uint64_t>(a.oth + zb + Lh * ((y0 - 1) & (L - 1)));
+    ulonglong2 P0 = ldg_pair<uint64_t>(a.oth + zb + Lh * y0);
+#pragma unroll
+    for (int m = 0; m < M; ++m) {
+        const unsigned y = y0 + m, row = zb + Lh * y;
+        const ulonglong2 own = *(const ulonglong2 *)(a.own + row);
+        const ulonglong2 Pp = ldg_pair<uint64_t>(a.oth + zb + Lh * ((y + 1) & (L - 1)));
+        const ulonglong2 Zm = ldg_pair<uint64_t>(a.oth + zbm + Lh * y);
+        const ulonglong2 Zp = ldg_pair<uint64_t>(a.oth + zbp + Lh * y);
+        const typename Pair<BondT>::type jx = ldg_pair<BondT>(Jc + row), jy = ldg_pair<BondT>(Jc + Nh + row),
+                                         jz = ldg_pair<BondT>(Jc + 2 * Nh + row), bx = ldg_pair<BondT>(Jo + row),
+                                         by = ldg_pair<BondT>(Jo + Nh + zb + Lh * ((y - 1) & (L - 1))),
+                                         bz = ldg_pair<BondT>(Jo + 2 * Nh + zbm + Lh * y);
+        const uint32_t site0 = 4 * k + L * (y + L * z);
+        ulonglong2 out;
+        if (((m & 1) ^ S0) == 0)
+            out = update_pair<0, BondT, ALWAYS>(own, P0, Pm, Pp, Zm, Zp, jx, jy, jz, bx, by, bz, site0, g, a.th, lane_m, lane_p);
+        else
+            out = update_pair<1, BondT, ALWAYS>(own, P0, Pm, Pp, Zm, Zp, jx, jy, jz, bx, by, bz, site0 + 1, g, a.th, lane_m, lane_p);
+        *(ulonglong2 *)(a.own + row) = out;
+        Pm = P0;
+        P0 = Pp;
+    }
+}
+
+template <int L, int M, typename BondT, bool ALWAYS>
+__global__ void __launch_bounds__(128) k_sweep_rows(const SweepArgs a)
+{
+    constexpr unsigned RL = L / 4, G = 32 / RL; // lanes per row, rows per warp
+    constexpr unsigned YC = L / M;              // y-chunks
+    const unsigned lane = threadIdx.x & 31, warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned k = lane % RL, grp = lane / RL;
+    const unsigned zg = warp / YC, yc = warp - zg * YC; // consecutive warps: the y-chunks of one z group
+    if (zg >= L / G) return;
+    const unsigned zpar = zg & 1, z = 2 * (G * (zg >> 1) + grp) + zpar, y0 = yc * M;
+    const int lane_m = (int)((lane & ~(RL - 1)) | ((k - 1) & (RL - 1))), lane_p = (int)((lane & ~(RL - 1)) | ((k + 1) & (RL - 1)));
+    const SweepRng g = make_sweep_rng(a.seed, sweep_time(a), (uint32_t)a.colour);
+    if ((a.colour ^ zpar) == 0) // phase of row y0 (even): warp-uniform
+        march_rows<L, M, 0, BondT, ALWAYS>(a, g, y0, z, k, lane_m, lane_p);
+    else
+        march_rows<L, M, 1, BondT, ALWAYS>(a, g, y0, z, k, lane_m, lane_p);
+}
+
+template <int L, typename BondT, bool ALWAYS>
+static void launch_rows(const SweepArgs &a, cudaStream_t st)
+{
+    constexpr int M = (L >= 128) ? 4 : 2, G = 32 / (L / 4);
+    constexpr unsigned warps = (L / M) * (L / G), block = 128, grid = (warps * 32 + block - 1) / block;
+    k_sweep_rows<L, M, BondT, ALWAYS><<<grid, block, 0, st>>>(a);
+}
+
+// ---------------------------------------------------------------------------------------------
+template <typename BondT, bool ALWAYS>
 static cudaError_t launch_typed(ea_sim *s, const SweepArgs &a, cudaStream_t st)
 {
     const Lattice &lat = s->lat;
     const bool pow2 = lat.log2L >= 0;
-    if (s->kernel == EA_KERNEL_VEC2) {
+    if (s->kernel == EA_KERNEL_ROWS) {
+        switch (lat.L) {
+        case 16: launch_rows<16, BondT, ALWAYS>(a, st); break;
+        case 32: launch_rows<32, BondT, ALWAYS>(a, st); break;
+        case 64: launch_rows<64, BondT, ALWAYS>(a, st); break;
+        case 128: launch_rows<128, BondT, ALWAYS>(a, st); break;
+        default: return cudaErrorInvalidValue;
+        }
+    } else if (s->kernel == EA_KERNEL_VEC2) {
         unsigned n = lat.Nh / 2, block = 256, grid = (n + block - 1) / block;
-        if (pow2) k_sweep_vec2<BondT, true><<<grid, block, 0, st>>>(a);
-        else k_sweep_vec2<BondT, false><<<grid, block, 0, st>>>(a);
+        if (pow2) k_sweep_vec2<BondT, true, ALWAYS><<<grid, block, 0, st>>>(a);
+        else k_sweep_vec2<BondT, false, ALWAYS><<<grid, block, 0, st>>>(a);
     } else {
         unsigned n = lat.Nh, block = 256, grid = (n + block - 1) / block;
-        if (pow2) k_sweep_scalar<BondT, true><<<grid, block, 0, st>>>(a);
-        else k_sweep_scalar<BondT, false><<<grid, block, 0, st>>>(a);
+        if (pow2) k_sweep_scalar<BondT, true, ALWAYS><<<grid, block, 0, st>>>(a);
+        else k_sweep_scalar<BondT, false, ALWAYS><<<grid, block, 0, st>>>(a);
     }
     s->count_launch();
     return cudaGetLastError();
+}
+
+template <typename BondT>
+static cudaError_t launch_typed(ea_sim *s, const SweepArgs &a, cudaStream_t st)
+{
+    const bool always = a.th.always[0] | a.th.always[1] | a.th.always[2]; // T = inf: some thr == 2^32
+    return always ? launch_typed<BondT, true>(s, a, st) : launch_typed<BondT, false>(s, a, st);
 }
 
 cudaError_t launch_half_sweep(ea_sim *s, int parity, uint64_t t, const uint64_t *d_time, uint32_t t_offset,
