@@ -46,8 +46,8 @@ LANES = 64
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE half-sweep launch at the bench configuration, from the
-# `ncu --set full` capture summarised in profiles/ (see profiles/README.md for the command); None = not captured.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+# `ncu --set full` capture summarised in profiles/ (the .md names the command); None = not captured.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 41996032  # profiles/r01_ncu_full_k_sweep_rows.md (cold L2: ncu flushes caches per launch)
 
 
 def algorithmic_bytes_per_half_sweep(N, n_replicas):
