@@ -134,6 +134,133 @@ __global__ void __launch_bounds__(256) k_count_c4(Lattice lat, const uint64_t *_
     flush_counts(k, out + (size_t)job * 32, false);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Fast C_4 path for L in {64, 128} (L/2 a multiple of 32), 2 replicas.
+// Pass 1 (k_q_transpose): Q_i = sigma^a_i ^ sigma^b_i (Eq. 2), every block of 32 consecutive compact sites
+// transposed once into sample-major words:  Tq[c][row][xb][b], row = y + L z, xb = block of 32 compact x
+// positions; bit k of the word = Q of sample b at compact xh = 32 xb + k.  Also counts the overlap q.
+// Pass 2: B_b(d, r) = N - 2 sum popc(own ^ partner): along y / z the partner of (c, row) at distance r is the
+// word of colour c ^ (r & 1) in the row r further on (same xh: the row phase flips with the colour);
+// along x it is the partner row's bits rotated by r/2 (r even, same colour) or (r-1)/2 + s (r odd, other
+// colour, s = row phase of the own colour).  One POPC then counts 32 sites of one sample; lane = sample, so
+// no cross-lane reduction is needed.
+// ---------------------------------------------------------------------------------------------
+template <int L>
+__global__ void __launch_bounds__(256) k_q_transpose(const uint64_t *__restrict__ spins, uint32_t *__restrict__ Tq,
+                                                     unsigned long long *out_overlap)
+{
+    constexpr unsigned NW = (unsigned)L * L * L / 32; // 32-site blocks over both colours
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
+    unsigned cnt = 0;
+    for (unsigned w = warp; w < NW; w += nwarps) { // warp-uniform trip count
+        const uint64_t sg = spins[(size_t)w * 32 + lane];
+        const uint32_t t = warp_transpose32(lo32(sg) ^ hi32(sg), lane);
+        Tq[(size_t)w * 32 + lane] = t;
+        cnt += __popc(t);
+    }
+    __shared__ unsigned acc[32];
+    if (threadIdx.x < 32) acc[threadIdx.x] = 0;
+    __syncthreads();
+    atomicAdd(&acc[lane], cnt);
+    __syncthreads();
+    if (threadIdx.x < 32) atomicAdd(&out_overlap[threadIdx.x], (unsigned long long)acc[threadIdx.x]);
+}
+
+template <int NR>
+__device__ __forceinline__ void flush_r_counts(const unsigned (&cnt)[NR], unsigned lane, int r_max,
+                                               unsigned long long *out /* [r][32] */)
+{
+    __shared__ unsigned acc[NR][32];
+    for (unsigned k = threadIdx.x; k < NR * 32; k += blockDim.x) (&acc[0][0])[k] = 0;
+    __syncthreads();
+#pragma unroll
+    for (int r = 1; r < NR; ++r) atomicAdd(&acc[r][lane], cnt[r]);
+    __syncthreads();
+    for (unsigned k = threadIdx.x; k < NR * 32; k += blockDim.x)
+        if ((int)(k >> 5) <= r_max && (&acc[0][0])[k]) atomicAdd(&out[k], (unsigned long long)(&acc[0][0])[k]);
+}
+
+// AXIS = 1 (y) or 2 (z)
+template <int L, int AXIS>
+__global__ void __launch_bounds__(256) k_c4_yz(const uint32_t *__restrict__ Tq, int r_max, unsigned long long *out)
+{
+    constexpr unsigned XB = L / 64, RW = XB * 32, PL = L * RW, CW = L * PL, NT = 2 * L * L * XB;
+    constexpr int NR = L / 2 + 1;
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
+    unsigned cnt[NR];
+#pragma unroll
+    for (int r = 0; r < NR; ++r) cnt[r] = 0;
+    for (unsigned t = warp; t < NT; t += nwarps) {
+        const unsigned xb = t % XB, y = (t / XB) % L, z = (t / (XB * L)) % L, c = t / (XB * L * L);
+        const uint32_t own = __ldg(Tq + c * CW + z * PL + y * RW + xb * 32 + lane);
+#pragma unroll
+        for (int r = 1; r < NR; ++r) {
+            const unsigned cp = c ^ (r & 1);
+            const unsigned yy = AXIS == 1 ? ((y + r) & (L - 1)) : y, zz = AXIS == 2 ? ((z + r) & (L - 1)) : z;
+            cnt[r] += __popc(own ^ __ldg(Tq + cp * CW + zz * PL + yy * RW + xb * 32 + lane));
+        }
+    }
+    flush_r_counts<NR>(cnt, lane, r_max, out);
+}
+
+template <int L> struct RowBits;
+template <> struct RowBits<128> {
+    typedef uint64_t type;
+    static __device__ __forceinline__ uint64_t load(const uint32_t *p) { return mk64(__ldg(p), __ldg(p + 32)); }
+    static __device__ __forceinline__ uint64_t rotr(uint64_t v, unsigned d) { return (v >> d) | (v << ((64 - d) & 63)); }
+    static __device__ __forceinline__ unsigned popc(uint64_t v) { return __popcll(v); }
+};
+template <> struct RowBits<64> {
+    typedef uint32_t type;
+    static __device__ __forceinline__ uint32_t load(const uint32_t *p) { return __ldg(p); }
+    static __device__ __forceinline__ uint32_t rotr(uint32_t v, unsigned d) { return (v >> d) | (v << ((32 - d) & 31)); }
+    static __device__ __forceinline__ unsigned popc(uint32_t v) { return __popc(v); }
+};
+
+template <int L>
+__global__ void __launch_bounds__(256) k_c4_x(const uint32_t *__restrict__ Tq, int r_max, unsigned long long *out)
+{
+    constexpr unsigned XB = L / 64, RW = XB * 32, CW = (unsigned)L * L * RW, NT = L * L;
+    constexpr int NR = L / 2 + 1;
+    typedef RowBits<L> RB;
+    const unsigned lane = threadIdx.x & 31;
+    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
+    unsigned cnt[NR];
+#pragma unroll
+    for (int r = 0; r < NR; ++r) cnt[r] = 0;
+    for (unsigned row = warp; row < NT; row += nwarps) {
+        const unsigned y = row % L, z = row / L, s0 = (y + z) & 1u; // row phase of colour 0; colour 1 has 1 - s0
+        const typename RB::type R0 = RB::load(Tq + row * RW + lane), R1 = RB::load(Tq + CW + row * RW + lane);
+#pragma unroll
+        for (int r = 1; r < NR; ++r) {
+            const unsigned e = r >> 1;
+            if ((r & 1) == 0)
+                cnt[r] += RB::popc(R0 ^ RB::rotr(R0, e)) + RB::popc(R1 ^ RB::rotr(R1, e));
+            else
+                cnt[r] += RB::popc(R0 ^ RB::rotr(R1, e + s0)) + RB::popc(R1 ^ RB::rotr(R0, e + 1 - s0));
+        }
+    }
+    flush_r_counts<NR>(cnt, lane, r_max, out);
+}
+
+template <int L>
+static cudaError_t launch_c4_fast(ea_sim *s, int r_max)
+{
+    const size_t n_r = (size_t)r_max + 1;
+    uint32_t *Tq = (uint32_t *)s->stage; // N words of 4 B in the 8 N-byte canonical staging buffer
+    const unsigned grid = (unsigned)s->n_sm * 2;
+    k_q_transpose<L><<<grid, 256, 0, s->stream>>>(s->spins, Tq, s->counters + 3 * n_r * 32);
+    s->count_launch();
+    k_c4_x<L><<<grid, 256, 0, s->stream>>>(Tq, r_max, s->counters);
+    s->count_launch();
+    k_c4_yz<L, 1><<<grid, 256, 0, s->stream>>>(Tq, r_max, s->counters + n_r * 32);
+    s->count_launch();
+    k_c4_yz<L, 2><<<grid, 256, 0, s->stream>>>(Tq, r_max, s->counters + 2 * n_r * 32);
+    return cudaGetLastError();
+}
+
 static unsigned grid_for(const ea_sim *s, size_t items)
 {
     size_t need = (items + 255) / 256, cap = (size_t)s->n_sm * 8;
@@ -166,6 +293,11 @@ cudaError_t launch_count_c4(ea_sim *s, int r_max)
     size_t jobs = 3 * (size_t)(r_max + 1) + 1;
     cudaError_t e = cudaMemsetAsync(s->counters, 0, jobs * 32 * sizeof(unsigned long long), s->stream);
     if (e != cudaSuccess) return e;
+    if (s->lat.L == 128 || s->lat.L == 64) { // r = 0 is B = N exactly: its counters stay 0
+        e = s->lat.L == 128 ? launch_c4_fast<128>(s, r_max) : launch_c4_fast<64>(s, r_max);
+        s->count_launch();
+        return e;
+    }
     size_t need = ((size_t)s->N + 255) / 256, cap = (size_t)s->n_sm * 2;
     dim3 grid((unsigned)(need < cap ? need : cap), (unsigned)jobs);
     k_count_c4<<<grid, 256, 0, s->stream>>>(s->lat, s->spins, r_max, s->counters);

@@ -186,6 +186,26 @@ def test_full_size_L128_every_word(name):
     assert_same_observables(g, o, slot=0)
 
 
+@pytest.mark.parametrize("L", [16, 64, 128])
+def test_c4_partial_r_max_and_injected_spins(L):
+    """C_4 with r_max < L/2 and on injected random spins (both the generic and the L = 64 / 128 fast path);
+    identical replicas give B = q = N exactly."""
+    N = L ** 3
+    g, o = make_pair(L, 0.5, 0.8, 2, wl.seed_for(7, L), n_slots=1)
+    spins = wl.random_words(N, 100 + L)
+    g.set_spins(spins)
+    o.set_spins(spins)
+    for r_max in (0, 1, 5, L // 2):
+        B, q = g.c4(r_max, with_q=True)
+        assert np.array_equal(B, o.c4(r_max))
+        assert np.array_equal(q, o.overlap())
+    same = (spins & np.uint64(0xffffffff))
+    same = same | (same << np.uint64(32))
+    g.set_spins(same)
+    B, q = g.c4(L // 2, with_q=True)
+    assert np.all(B == N) and np.all(q == N)
+
+
 def test_graph_replay_path_and_composition():
     """sweep(a); sweep(b) == sweep(a+b), including the CUDA-graph path (n >= 32) and its remainder."""
     L, seed = 8, 4242
