@@ -24,6 +24,7 @@ WorkspaceLayout workspace_layout(int L, int n_replicas, int n_slots)
     w.off_stage = off;    off = align_up(off + N * 8);
     w.off_counters = off; off = align_up(off + w.n_counters * 8);
     w.off_time = off;     off = align_up(off + 8);
+    w.off_flags = off;    off = align_up(off + resident_flag_bytes());
     w.total = off;
     return w;
 }
@@ -79,6 +80,33 @@ using namespace ea;
         if (_e != cudaSuccess) EA_FAIL(sim, EA_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(_e)); \
     } while (0)
 
+// Wait for the sim's stream; if a RESIDENT launch ran since the last check, read its abort word (a CTA whose
+// neighbour never published its step gives up after 2 s instead of hanging the device).
+static ea_status stream_sync(ea_sim *s)
+{
+    EA_CUDA(s, cudaStreamSynchronize(s->stream));
+    if (s->resident_used) {
+        s->resident_used = false;
+        unsigned *d_abort = s->resident_flags + (resident_flag_bytes() / sizeof(unsigned) - 32);
+        unsigned aborted = 0;
+        EA_CUDA(s, cudaMemcpy(&aborted, d_abort, sizeof(aborted), cudaMemcpyDeviceToHost));
+        if (aborted) {
+            cudaMemset(s->resident_flags, 0, resident_flag_bytes());
+            s->resident_epoch = 0;
+            EA_FAIL(s, EA_ERR_CUDA, "resident sweep kernel: neighbour wait timed out; the spin state is invalid");
+        }
+    }
+    return EA_OK;
+}
+#define EA_SYNC(sim)                          \
+    do {                                      \
+        ea_status _rc = stream_sync(sim);     \
+        if (_rc != EA_OK) return _rc;         \
+    } while (0)
+
+static const uint64_t RESIDENT_AUTO_MIN_SWEEPS = 8;     // AUTO: below this the prologue/epilogue of the persistent kernel does not pay
+static const uint64_t RESIDENT_MAX_SWEEPS = 1u << 20;   // sweeps per persistent launch (about 10 s of device time)
+
 static bool valid_L(int L) { return L >= 2 && (L & 1) == 0 && (int64_t)L * L * L < ((int64_t)1 << 31); }
 
 static bool kernel_valid_for(int kernel, int L)
@@ -87,6 +115,7 @@ static bool kernel_valid_for(int kernel, int L)
     case EA_KERNEL_SCALAR: return true;
     case EA_KERNEL_VEC2: return L % 4 == 0;
     case EA_KERNEL_ROWS: return L == 16 || L == 32 || L == 64 || L == 128;
+    case EA_KERNEL_RESIDENT: return L == 128; // plus a device check (resident_supported) once the sim exists
     default: return false;
     }
 }
@@ -207,6 +236,15 @@ ea_status ea_create_ex(const ea_params *prm, ea_sim **out)
         s->counters = (unsigned long long *)(s->ws + w.off_counters);
         s->n_counters = w.n_counters;
         s->d_time = (uint64_t *)(s->ws + w.off_time);
+        s->resident_flags = (unsigned *)(s->ws + w.off_flags);
+        if ((e = cudaMemsetAsync(s->resident_flags, 0, resident_flag_bytes(), s->stream)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
+        if (prm->kernel == EA_KERNEL_AUTO && kernel_valid_for(EA_KERNEL_RESIDENT, L) && resident_supported(s)) {
+            s->kernel = EA_KERNEL_RESIDENT; // long runs in one persistent launch, short ones as ROWS launches
+            s->resident_min_sweeps = RESIDENT_AUTO_MIN_SWEEPS;
+        } else if (s->kernel == EA_KERNEL_RESIDENT && !resident_supported(s)) {
+            rc = EA_ERR_INVALID;
+            break;
+        }
         s->h_counters.resize(w.n_counters);
         if ((e = launch_init_bonds(s)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
         if ((e = launch_init_spins(s)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
@@ -271,6 +309,16 @@ ea_status ea_sweep(ea_sim *sim, uint64_t n)
     if (!sim) return EA_ERR_INVALID;
     DeviceGuard g(sim->device);
     uint64_t left = n;
+    if (sim->kernel == EA_KERNEL_RESIDENT && n >= sim->resident_min_sweeps) {
+        while (left) {
+            const uint32_t chunk = (uint32_t)(left < RESIDENT_MAX_SWEEPS ? left : RESIDENT_MAX_SWEEPS);
+            EA_CUDA(sim, launch_sweeps_resident(sim, sim->t, chunk, sim->stream));
+            sim->resident_used = true;
+            sim->t += chunk;
+            left -= chunk;
+        }
+        return EA_OK;
+    }
     if (left >= (uint64_t)GRAPH_SWEEPS) {
         if (!sim->graph_exec || sim->graph_kernel != sim->kernel) {
             ea_status rc = build_graph(sim);
@@ -339,6 +387,13 @@ ea_status ea_set_kernel(ea_sim *sim, int kernel)
     if (!sim) return EA_ERR_INVALID;
     int k = resolve_kernel(kernel, sim->lat.L);
     if (!kernel_valid_for(k, sim->lat.L)) EA_FAIL(sim, EA_ERR_INVALID, "kernel %d not valid for L=%d", kernel, sim->lat.L);
+    sim->resident_min_sweeps = 1;
+    if (kernel == EA_KERNEL_AUTO && kernel_valid_for(EA_KERNEL_RESIDENT, sim->lat.L) && resident_supported(sim)) {
+        k = EA_KERNEL_RESIDENT;
+        sim->resident_min_sweeps = RESIDENT_AUTO_MIN_SWEEPS;
+    }
+    if (k == EA_KERNEL_RESIDENT && !resident_supported(sim))
+        EA_FAIL(sim, EA_ERR_INVALID, "resident kernel: device lacks cooperative launch, >= 128 SMs or 181 KB of shared memory per CTA");
     sim->kernel = k;
     return EA_OK;
 }
@@ -361,7 +416,7 @@ ea_status ea_synchronize(ea_sim *sim)
 {
     if (!sim) return EA_ERR_INVALID;
     DeviceGuard g(sim->device);
-    EA_CUDA(sim, cudaStreamSynchronize(sim->stream));
+    EA_SYNC(sim);
     return EA_OK;
 }
 
@@ -371,7 +426,7 @@ static ea_status fetch_counters(ea_sim *s, size_t n)
 {
     EA_CUDA(s, cudaMemcpyAsync(s->h_counters.data(), s->counters, n * sizeof(unsigned long long),
                                cudaMemcpyDeviceToHost, s->stream));
-    EA_CUDA(s, cudaStreamSynchronize(s->stream));
+    EA_SYNC(s);
     return EA_OK;
 }
 
@@ -456,7 +511,7 @@ ea_status ea_get_spins(ea_sim *sim, uint64_t *host)
     DeviceGuard g(sim->device);
     EA_CUDA(sim, launch_unpack_spins(sim, sim->spins, sim->stage));
     EA_CUDA(sim, cudaMemcpyAsync(host, sim->stage, (size_t)sim->N * 8, cudaMemcpyDeviceToHost, sim->stream));
-    EA_CUDA(sim, cudaStreamSynchronize(sim->stream));
+    EA_SYNC(sim);
     return EA_OK;
 }
 
@@ -468,7 +523,7 @@ ea_status ea_get_snapshot(ea_sim *sim, int slot, uint64_t *host)
     DeviceGuard g(sim->device);
     EA_CUDA(sim, launch_unpack_spins(sim, sim->snaps + (size_t)slot * sim->N, sim->stage));
     EA_CUDA(sim, cudaMemcpyAsync(host, sim->stage, (size_t)sim->N * 8, cudaMemcpyDeviceToHost, sim->stream));
-    EA_CUDA(sim, cudaStreamSynchronize(sim->stream));
+    EA_SYNC(sim);
     return EA_OK;
 }
 
@@ -478,7 +533,7 @@ ea_status ea_set_spins(ea_sim *sim, const uint64_t *host)
     DeviceGuard g(sim->device);
     EA_CUDA(sim, cudaMemcpyAsync(sim->stage, host, (size_t)sim->N * 8, cudaMemcpyHostToDevice, sim->stream));
     EA_CUDA(sim, launch_pack_spins(sim, sim->stage, sim->spins));
-    EA_CUDA(sim, cudaStreamSynchronize(sim->stream));
+    EA_SYNC(sim);
     return EA_OK;
 }
 
@@ -490,7 +545,7 @@ ea_status ea_get_bonds(ea_sim *sim, uint64_t *host)
         EA_CUDA(sim, launch_unpack_bonds(sim, d, sim->stage));
         EA_CUDA(sim, cudaMemcpyAsync(host + (size_t)d * sim->N, sim->stage, (size_t)sim->N * 8, cudaMemcpyDeviceToHost,
                                      sim->stream));
-        EA_CUDA(sim, cudaStreamSynchronize(sim->stream));
+        EA_SYNC(sim);
     }
     return EA_OK;
 }
@@ -507,7 +562,7 @@ ea_status ea_set_bonds(ea_sim *sim, const uint64_t *host)
         EA_CUDA(sim, cudaMemcpyAsync(sim->stage, host + (size_t)d * sim->N, (size_t)sim->N * 8, cudaMemcpyHostToDevice,
                                      sim->stream));
         EA_CUDA(sim, launch_pack_bonds(sim, d, sim->stage));
-        EA_CUDA(sim, cudaStreamSynchronize(sim->stream));
+        EA_SYNC(sim);
     }
     return EA_OK;
 }

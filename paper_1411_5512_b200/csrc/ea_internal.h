@@ -41,6 +41,12 @@ struct ea_sim {
     int graph_kernel = -1;
     uint64_t *d_time = nullptr;   // device copy of t consumed by graph-launched kernels
 
+    // RESIDENT kernel (L = 128): per-CTA step flags + abort word in the workspace, and the flag epoch
+    unsigned *resident_flags = nullptr;
+    uint32_t resident_epoch = 0;
+    uint64_t resident_min_sweeps = 1; // shorter ea_sweep calls use the ROWS launches (AUTO: 8)
+    bool resident_used = false;       // a resident launch is in flight / unchecked: see check_resident()
+
     // kernels this sim has put on the device (a graph replay counts its kernel nodes); bench.py's gpu_launches
     uint64_t launches = 0;
     bool capturing = false;
@@ -55,7 +61,7 @@ struct ea_sim {
 namespace ea {
 
 struct WorkspaceLayout {
-    size_t off_spins, off_bonds, off_snaps, off_stage, off_counters, off_time, total;
+    size_t off_spins, off_bonds, off_snaps, off_stage, off_counters, off_time, off_flags, total;
     size_t n_counters;
 };
 WorkspaceLayout workspace_layout(int L, int n_replicas, int n_slots);
@@ -67,6 +73,10 @@ cudaError_t launch_init_bonds(ea_sim *s);
 cudaError_t launch_half_sweep(ea_sim *s, int parity, uint64_t t, const uint64_t *d_time, uint32_t t_offset,
                               cudaStream_t st);
 cudaError_t launch_bump_time(ea_sim *s, uint32_t n, cudaStream_t st);
+// RESIDENT (ea_sweep_resident.cu): n sweeps from sweep index t0 in one cooperative launch
+bool resident_supported(const ea_sim *s);
+size_t resident_flag_bytes();
+cudaError_t launch_sweeps_resident(ea_sim *s, uint64_t t0, uint32_t n, cudaStream_t st);
 
 // canonical <-> internal
 cudaError_t launch_pack_spins(ea_sim *s, const uint64_t *d_canon, uint64_t *d_internal);   // canonical -> internal

@@ -4,6 +4,7 @@
 // A kernel boundary is the colour barrier ("each half-step is performed in its own CUDA kernel call to
 // ensure global synchronization").  All variants are bit-identical (same stream contract).
 #include "ea_internal.h"
+#include "ea_sweep_common.cuh"
 
 namespace ea {
 
@@ -90,17 +91,6 @@ __global__ void __launch_bounds__(256) k_sweep_scalar(const SweepArgs a)
 // VEC2: two x-adjacent sites of one colour per thread; every access but one neighbour word and one
 // bond word per thread is a 128-bit (uint64 pairs) or 64-bit (uint32 bond pairs) vector.  L % 4 == 0.
 // ---------------------------------------------------------------------------------------------
-template <typename T> struct Pair;
-template <> struct Pair<uint64_t> { typedef ulonglong2 type; };
-template <> struct Pair<uint32_t> { typedef uint2 type; };
-
-template <typename BondT>
-__device__ __forceinline__ void ld_pair(const BondT *p, BondT &a, BondT &b)
-{
-    typename Pair<BondT>::type v = __ldg((const typename Pair<BondT>::type *)p);
-    a = v.x;
-    b = v.y;
-}
 
 template <typename BondT, bool POW2, bool ALWAYS>
 __global__ void __launch_bounds__(256) k_sweep_vec2(const SweepArgs a)
@@ -173,52 +163,6 @@ __global__ void k_bump_time(uint64_t *d_time, uint32_t n) { *d_time += n; }
 // stride is an immediate.  A warp with several rows (L < 128) takes rows of equal z parity, which keeps s
 // warp-uniform.
 // ---------------------------------------------------------------------------------------------
-template <typename BondT>
-__device__ __forceinline__ typename Pair<BondT>::type ldg_pair(const BondT *p)
-{
-    return __ldg((const typename Pair<BondT>::type *)p);
-}
-
-__device__ __forceinline__ uint64_t shfl64(uint64_t v, int src)
-{
-    uint32_t lo = __shfl_sync(0xffffffffu, lo32(v), src), hi = __shfl_sync(0xffffffffu, hi32(v), src);
-    return mk64(lo, hi);
-}
-__device__ __forceinline__ uint32_t shfl_bond(uint32_t v, int src) { return __shfl_sync(0xffffffffu, v, src); }
-__device__ __forceinline__ uint64_t shfl_bond(uint64_t v, int src) { return shfl64(v, src); }
-
-template <int S, typename BondT, bool ALWAYS>
-__device__ __forceinline__ ulonglong2 update_pair(const ulonglong2 own, const ulonglong2 P0, const ulonglong2 Pm,
-                                                  const ulonglong2 Pp, const ulonglong2 Zm, const ulonglong2 Zp,
-                                                  const typename Pair<BondT>::type jx,
-                                                  const typename Pair<BondT>::type jy,
-                                                  const typename Pair<BondT>::type jz,
-                                                  const typename Pair<BondT>::type bx,
-                                                  const typename Pair<BondT>::type by,
-                                                  const typename Pair<BondT>::type bz, const uint32_t site0,
-                                                  const SweepRng &g, const Thresholds &th, const int lane_m,
-                                                  const int lane_p)
-{
-    uint32_t r0l, r0h, r1l, r1h;
-    sweep_random(g, site0, r0l, r0h);
-    sweep_random(g, site0 + 2, r1l, r1h);
-    ulonglong2 out;
-    if (S == 0) { // own x = 4k, 4k+2; other colour at 4k+1 (P0.x), 4k+3 (P0.y), 4k-1 (left lane's P0.y)
-        const uint64_t ex = shfl64(P0.y, lane_m);
-        const BondT jex = shfl_bond((BondT)bx.y, lane_m);
-        out.x = metropolis_word<BondT, ALWAYS>(own.x, P0.x, ex, Pp.x, Pm.x, Zp.x, Zm.x, (BondT)jx.x, jex, (BondT)jy.x,
-                                               (BondT)by.x, (BondT)jz.x, (BondT)bz.x, r0l, r0h, th);
-        out.y = metropolis_word<BondT, ALWAYS>(own.y, P0.y, P0.x, Pp.y, Pm.y, Zp.y, Zm.y, (BondT)jx.y, (BondT)bx.x,
-                                               (BondT)jy.y, (BondT)by.y, (BondT)jz.y, (BondT)bz.y, r1l, r1h, th);
-    } else {      // own x = 4k+1, 4k+3; other colour at 4k (P0.x), 4k+2 (P0.y), 4k+4 (right lane's P0.x)
-        const uint64_t ex = shfl64(P0.x, lane_p);
-        out.x = metropolis_word<BondT, ALWAYS>(own.x, P0.y, P0.x, Pp.x, Pm.x, Zp.x, Zm.x, (BondT)jx.x, (BondT)bx.x,
-                                               (BondT)jy.x, (BondT)by.x, (BondT)jz.x, (BondT)bz.x, r0l, r0h, th);
-        out.y = metropolis_word<BondT, ALWAYS>(own.y, ex, P0.y, Pp.y, Pm.y, Zp.y, Zm.y, (BondT)jx.y, (BondT)bx.y,
-                                               (BondT)jy.y, (BondT)by.y, (BondT)jz.y, (BondT)bz.y, r1l, r1h, th);
-    }
-    return out;
-}
 
 template <int L, int M, int S0, typename BondT, bool ALWAYS>
 __device__ __forceinline__ void march_rows(const SweepArgs &a, const SweepRng &g, const unsigned y0, const unsigned z,
@@ -285,7 +229,7 @@ static cudaError_t launch_typed(ea_sim *s, const SweepArgs &a, cudaStream_t st)
 {
     const Lattice &lat = s->lat;
     const bool pow2 = lat.log2L >= 0;
-    if (s->kernel == EA_KERNEL_ROWS) {
+    if (s->kernel == EA_KERNEL_ROWS || s->kernel == EA_KERNEL_RESIDENT) { // RESIDENT: single half-sweeps go as ROWS
         switch (lat.L) {
         case 16: launch_rows<16, BondT, ALWAYS>(a, st); break;
         case 32: launch_rows<32, BondT, ALWAYS>(a, st); break;
