@@ -95,6 +95,20 @@ __host__ __device__ inline SweepRng make_sweep_rng(uint64_t seed, uint64_t t, ui
     return g;
 }
 
+// Same folding when the round keys are already in place (RESIDENT: keys arrive as kernel parameters).
+__host__ __device__ inline void sweep_rng_set_time(SweepRng &g, uint64_t t, uint32_t tag)
+{
+    uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
+    uint64_t p1 = (uint64_t)PHILOX_M1 * t_hi;
+    uint32_t U0 = (uint32_t)(p1 >> 32) ^ t_lo ^ g.k0[0];
+    uint32_t U1 = (uint32_t)p1;
+    uint64_t q0 = (uint64_t)PHILOX_M0 * U0;
+    g.x2 = tag ^ g.k1[0];
+    g.x0 = U1 ^ g.k0[1];
+    g.y2 = (uint32_t)(q0 >> 32) ^ g.k1[1];
+    g.z2 = (uint32_t)q0 ^ g.k1[2];
+}
+
 __device__ __forceinline__ void sweep_random(const SweepRng &g, uint32_t site, uint32_t &r_lo, uint32_t &r_hi)
 {
     uint32_t h, l, h0, l0, h1, l1;

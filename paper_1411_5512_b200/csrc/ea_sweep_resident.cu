@@ -16,7 +16,10 @@
 //     dependency whose latency is hidden behind the interior update -- no grid-wide barrier, no relaunch.
 //   * global memory always holds the current boundary rows; interior rows are written back once at the end,
 //     so after the launch the global array is the full state at time t0 + n.
-#include <cooperative_groups.h>
+#include <stdlib.h>
+
+#include <utility>
+#include <vector>
 
 #include "ea_internal.h"
 #include "ea_sweep_common.cuh"
@@ -26,7 +29,7 @@ namespace ea {
 struct ResidentArgs {
     uint64_t *spins;     // [2][Nh]
     const void *bonds;   // BondT [2][3][Nh]
-    uint64_t seed;
+    uint32_t k0[10], k1[10]; // Philox round keys of the seed (C-A6)
     uint64_t t0;         // first sweep index
     uint32_t n_half;     // half-steps to run (2 per sweep)
     uint32_t epoch0;     // flag value before this launch; step h publishes epoch0 + h + 1
@@ -47,7 +50,7 @@ template <int L_, int TY_, int TZ_> struct ResidentGeom {
     static constexpr int NB = ROWS - (TY - 2) * (TZ - 2); // boundary rows
     static constexpr unsigned HALO_BYTES = (2 * TY + 2 * TZ) * Lh * 8;
     static constexpr size_t SPIN_BYTES = (size_t)2 * HZ * HY * Lh * 8;
-    static constexpr size_t SMEM_BYTES = SPIN_BYTES + 16 /*mbarrier*/ + ROWS * 4 /*row table*/;
+    static constexpr size_t SMEM_BYTES = SPIN_BYTES + 16 /*mbarrier*/ + ROWS * 16 /*row descriptors*/;
     static_assert(Lh == 64, "a warp covers one colour row with two words per lane");
     static_assert(ROWS % CW == 0, "equal number of rows per compute warp");
 };
@@ -101,54 +104,138 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
 enum { BAR_BOUNDARY = 1, BAR_STEP = 2 };
 constexpr unsigned long long RESIDENT_TIMEOUT_NS = 2000000000ull; // a neighbour that never shows up: give up after 2 s
 
+// Row schedule of one CTA (built on the host, build_row_table): compute warp w updates rows row[w][0..RPW-1]
+// (yy | zz << 8, tile coordinates 1..TY, 1..TZ), boundary rows first (n_bnd[w] of them), and consecutive rows
+// of a warp alternate in (yy + zz) parity starting from phi[w] -- so the row phase s = (colour ^ y ^ z) & 1 of
+// every row is a compile-time constant once the warp-uniform (colour ^ phi[w]) is known.
+template <typename G> struct RowTable {
+    uint16_t row[G::CW][G::ROWS / G::CW];
+    uint8_t n_bnd[G::CW];
+    uint8_t phi[G::CW];
+};
+
 template <typename BondT> struct RowBonds { typename Pair<BondT>::type jx, jy, jz, bx, by, bz; };
 
-template <typename G, typename BondT>
-__device__ __forceinline__ RowBonds<BondT> load_row_bonds(const BondT *__restrict__ Jc, const BondT *__restrict__ Jo,
-                                                          unsigned y, unsigned z, unsigned k)
+// Row descriptor (shared memory, one per (compute warp, row slot), written once in the prologue):
+//   x = byte offset of row (zz, yy) inside a colour plane of the tile
+//   y = word offset of row (y, z) inside a colour plane of the global arrays, Lh * (y + L * z)
+//   z = Nh + offset of row (y-1, z),  w = 2 Nh + offset of row (y, z-1)    (periodic) -- the backward y / z bonds
+template <typename G>
+__device__ __forceinline__ uint4 make_row_desc(unsigned yy, unsigned zz, unsigned y0, unsigned z0)
 {
     constexpr unsigned Lh = G::Lh, L = G::L, Nh = (unsigned)L * L * L / 2;
-    const unsigned row = Lh * (y + L * z) + 2 * k;
-    const unsigned rowym = Lh * (((y - 1) & (L - 1)) + L * z) + 2 * k;
-    const unsigned rowzm = Lh * (y + L * ((z - 1) & (L - 1))) + 2 * k;
+    const unsigned y = y0 + yy - 1, z = z0 + zz - 1;
+    uint4 d;
+    d.x = (zz * G::HY + yy) * Lh * 8;
+    d.y = Lh * (y + L * z);
+    d.z = Nh + Lh * (((y - 1) & (L - 1)) + L * z);
+    d.w = 2 * Nh + Lh * (y + L * ((z - 1) & (L - 1)));
+    return d;
+}
+
+// The kernel is bound by the alu pipe (LOP3), and 64-bit address arithmetic costs IADD3 / LEA.HI.X pairs on that
+// pipe for every row.  The host guarantees (resident_supported) that neither the bond nor the spin array
+// straddles a 4 GiB boundary, so inside the row loop an address is {constant high word, low word + offset}.
+struct Ptr32 {
+    uint32_t lo, hi;
+    __device__ __forceinline__ Ptr32() {}
+    __device__ __forceinline__ explicit Ptr32(const void *p) : lo((uint32_t)(uintptr_t)p), hi((uint32_t)((uintptr_t)p >> 32)) {}
+    template <typename T> __device__ __forceinline__ T *at(unsigned elem_off) const
+    {
+        return (T *)(((uintptr_t)hi << 32) | (uintptr_t)(lo + elem_off * (unsigned)sizeof(T)));
+    }
+};
+
+// Jc_l / Jo_l: bond planes of the updated / the other colour, already offset by the lane's 2k words
+template <typename BondT>
+__device__ __forceinline__ RowBonds<BondT> load_row_bonds(const Ptr32 Jc_l, const Ptr32 Jo_l, const uint4 d,
+                                                          const unsigned Nh)
+{
     RowBonds<BondT> b;
-    b.jx = ldg_pair<BondT>(Jc + row);
-    b.jy = ldg_pair<BondT>(Jc + Nh + row);
-    b.jz = ldg_pair<BondT>(Jc + 2 * Nh + row);
-    b.bx = ldg_pair<BondT>(Jo + row);
-    b.by = ldg_pair<BondT>(Jo + Nh + rowym);
-    b.bz = ldg_pair<BondT>(Jo + 2 * Nh + rowzm);
+    const BondT *pc = Jc_l.at<const BondT>(d.y);
+    b.jx = ldg_pair<BondT>(pc);
+    b.jy = ldg_pair<BondT>(pc + Nh);
+    b.jz = ldg_pair<BondT>(pc + 2 * Nh);
+    b.bx = ldg_pair<BondT>(Jo_l.at<const BondT>(d.y));
+    b.by = ldg_pair<BondT>(Jo_l.at<const BondT>(d.z));
+    b.bz = ldg_pair<BondT>(Jo_l.at<const BondT>(d.w));
     return b;
 }
 
+// per-step, per-lane context of a compute warp
+struct ResidentStep {
+    const unsigned char *s_oth; // tile plane of colour 1-c + 16 * lane
+    unsigned char *s_own;       // tile plane of colour c + 16 * lane
+    Ptr32 g_own;                // global plane of colour c + 2 * lane
+    unsigned k;
+    int lane_m, lane_p;
+};
+
+// one row of colour c with compile-time phase S; publishes it to global when `publish`
+template <int S, typename G, typename BondT, bool ALWAYS>
+__device__ __forceinline__ void resident_row(const ResidentStep &x, const uint4 d, const RowBonds<BondT> &bd,
+                                             const SweepRng &g, const Thresholds &th, const bool publish)
+{
+    constexpr int ROWB = G::Lh * 8, PLANEB = G::HY * G::Lh * 8; // smem strides: next y row, next z plane
+    unsigned char *own_row = x.s_own + d.x;
+    const unsigned char *o = x.s_oth + d.x;
+    const ulonglong2 own = *(const ulonglong2 *)own_row;
+    const ulonglong2 P0 = *(const ulonglong2 *)o;
+    const ulonglong2 Pm = *(const ulonglong2 *)(o - ROWB);
+    const ulonglong2 Pp = *(const ulonglong2 *)(o + ROWB);
+    const ulonglong2 Zm = *(const ulonglong2 *)(o - PLANEB);
+    const ulonglong2 Zp = *(const ulonglong2 *)(o + PLANEB);
+    const uint32_t site0 = 4 * x.k + S + 2 * d.y; // canonical site = x + L (y + L z), L = 2 Lh
+    const ulonglong2 out = update_pair<S, BondT, ALWAYS>(own, P0, Pm, Pp, Zm, Zp, bd.jx, bd.jy, bd.jz, bd.bx, bd.by, bd.bz,
+                                                         site0, g, th, x.lane_m, x.lane_p);
+    *(ulonglong2 *)own_row = out;
+    if (publish) *x.g_own.at<ulonglong2>(d.y / 2) = out;
+}
+
+// all rows of one compute warp for one half-step; S0 = phase of the warp's first row
+template <int S0, typename G, typename BondT, bool ALWAYS>
+__device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4 *__restrict__ desc, const int n_bnd,
+                                              RowBonds<BondT> &nxt, const Ptr32 Jc_l, const Ptr32 Jo_l,
+                                              const SweepRng &g, const Thresholds &th)
+{
+    constexpr int RPW = G::ROWS / G::CW;
+    constexpr unsigned Nh = (unsigned)G::L * G::L * G::L / 2;
+    static_assert(RPW % 2 == 0, "rows are taken two at a time (phases S0, 1 - S0)");
+#pragma unroll 1
+    for (int i = 0; i < RPW; i += 2) {
+        const uint4 d0 = desc[i], d1 = desc[i + 1], d2 = desc[(i + 2) % RPW];
+        const RowBonds<BondT> b0 = nxt;
+        const RowBonds<BondT> b1 = load_row_bonds<BondT>(Jc_l, Jo_l, d1, Nh);
+        resident_row<S0, G, BondT, ALWAYS>(x, d0, b0, g, th, i < n_bnd);
+        if (i + 1 == n_bnd) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
+        // the row after next: first row of the next half-step (colours swap roles) when this is the last pair
+        if (i + 2 < RPW) nxt = load_row_bonds<BondT>(Jc_l, Jo_l, d2, Nh);
+        else nxt = load_row_bonds<BondT>(Jo_l, Jc_l, d2, Nh);
+        resident_row<1 - S0, G, BondT, ALWAYS>(x, d1, b1, g, th, i + 1 < n_bnd);
+        if (i + 2 == n_bnd) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
+    }
+}
+
 template <typename G, typename BondT, bool ALWAYS>
-__global__ void __launch_bounds__(G::THREADS, 1) k_sweep_resident(const ResidentArgs a)
+__global__ void __launch_bounds__(G::THREADS, 1) k_sweep_resident(const ResidentArgs a, const RowTable<G> tab)
 {
     constexpr int L = G::L, Lh = G::Lh, TY = G::TY, TZ = G::TZ, HY = G::HY, HZ = G::HZ, CW = G::CW, ROWS = G::ROWS;
     constexpr unsigned Nh = (unsigned)L * L * L / 2;
     constexpr int RPW = ROWS / CW; // rows per compute warp per half-step
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    uint64_t *tile = (uint64_t *)smem_raw;                          // [2][HZ][HY][Lh]
-    uint64_t *halo_bar = (uint64_t *)(smem_raw + G::SPIN_BYTES);    // mbarrier: halo of the next step has landed
-    uint32_t *rowtab = (uint32_t *)(smem_raw + G::SPIN_BYTES + 16); // [ROWS]: yy | zz << 8, boundary rows first
+    uint64_t *tile = (uint64_t *)smem_raw;                       // [2][HZ][HY][Lh]
+    uint64_t *halo_bar = (uint64_t *)(smem_raw + G::SPIN_BYTES); // mbarrier: halo of the next step has landed
+    uint4 *rowdesc = (uint4 *)(smem_raw + G::SPIN_BYTES + 16);   // [CW][RPW] row descriptors
 
-    const unsigned tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const unsigned tid = threadIdx.x, lane = tid & 31;
+    const unsigned warp = __shfl_sync(0xffffffffu, tid >> 5, 0); // provably warp-uniform: no divergence guards around the shuffles
     const unsigned b = blockIdx.x, ty = b % G::NTY, tz = b / G::NTY;
     const unsigned y0 = ty * TY, z0 = tz * TZ;
     auto tile_at = [&](int c, int zz, int yy) -> uint64_t * { return tile + ((size_t)(c * HZ + zz) * HY + yy) * Lh; };
 
-    // ---- prologue: row table, barrier, tile + halo ring of both colours from global -------------------
-    if (tid < (unsigned)ROWS) {
-        const int yy = 1 + (int)tid % TY, zz = 1 + (int)tid / TY;
-        const bool isB = yy == 1 || yy == TY || zz == 1 || zz == TZ;
-        int before_same = 0;
-        for (int j = 0; j < (int)tid; ++j) {
-            const int y2 = 1 + j % TY, z2 = 1 + j / TY;
-            const bool b2 = y2 == 1 || y2 == TY || z2 == 1 || z2 == TZ;
-            before_same += (b2 == isB);
-        }
-        rowtab[isB ? before_same : G::NB + before_same] = (uint32_t)yy | ((uint32_t)zz << 8);
-    }
+    // ---- prologue: barrier, tile + halo ring of both colours from global -------------------------------
+    if (tid < (unsigned)ROWS)
+        rowdesc[tid] = make_row_desc<G>(tab.row[tid / RPW][tid % RPW] & 0xff, tab.row[tid / RPW][tid % RPW] >> 8, y0, z0);
     if (tid == 0) {
         mbar_init(halo_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -170,14 +257,26 @@ __global__ void __launch_bounds__(G::THREADS, 1) k_sweep_resident(const Resident
                                  : lane == 1 ? ((ty + G::NTY - 1) % G::NTY) + G::NTY * tz
                                  : lane == 2 ? ty + G::NTY * ((tz + 1) % G::NTZ)
                                              : ty + G::NTY * ((tz + G::NTZ - 1) % G::NTZ);
+        // the halo copy of this lane (2 z-faces of TY rows, then 2 y-face rows per tile plane): offsets within a colour
+        const unsigned zlo = (z0 - 1) & (L - 1), zhi = (z0 + TZ) & (L - 1);
+        const unsigned ylo = (y0 - 1) & (L - 1), yhi = (y0 + TY) & (L - 1);
+        unsigned cp_src = 0, cp_dst = 0, cp_bytes = 0; // word offsets
+        if (lane < 2) {
+            cp_src = Lh * (y0 + L * (lane ? zhi : zlo));
+            cp_dst = ((lane ? HZ - 1 : 0) * HY + 1) * Lh;
+            cp_bytes = TY * Lh * 8;
+        } else if (lane < 2 + 2 * TZ) {
+            const unsigned j = lane - 2, zz = 1 + (j >> 1), hi = j & 1;
+            cp_src = Lh * ((hi ? yhi : ylo) + L * (z0 + zz - 1));
+            cp_dst = (zz * HY + (hi ? HY - 1 : 0)) * Lh;
+            cp_bytes = Lh * 8;
+        }
+        static_assert(2 + 2 * TZ <= 32, "one halo copy per producer lane");
         for (uint32_t h = 0; h < a.n_half; ++h) {
             const int c = h & 1;
             named_bar_sync(BAR_BOUNDARY, G::THREADS); // boundary rows of step h are in smem and in global
             const unsigned epoch = a.epoch0 + h + 1;
-            if (lane == 0) {
-                __threadfence();
-                st_release_gpu(a.flags + b * 32, epoch);
-            }
+            if (lane == 0) st_release_gpu(a.flags + b * 32, epoch); // release: cumulative over the CTA's stores
             if (h + 1 == a.n_half) break;
             bool ok = true;
             if (lane < 4) {
@@ -194,98 +293,113 @@ __global__ void __launch_bounds__(G::THREADS, 1) k_sweep_resident(const Resident
                 }
             }
             ok = __all_sync(0xffffffffu, ok);
-            if (!ok) {
-                if (lane == 0) atomicExch(a.abort_flag, 1u);
-                // leave the halo stale; everybody notices the abort flag below and the host reports the error
-            }
-            if (lane == 0) {
+            // on a time-out: raise the abort flag (every CTA stops waiting), keep going with stale halos so that
+            // all barriers still complete; the host finds the flag at its next synchronisation and reports it
+            if (!ok && lane == 0) atomicExch(a.abort_flag, 1u);
+            if (lane == 0) mbar_arrive_expect_tx(halo_bar, G::HALO_BYTES);
+            __syncwarp();
+            if (cp_bytes) {
                 asm volatile("fence.proxy.async;" ::: "memory");
-                mbar_arrive_expect_tx(halo_bar, G::HALO_BYTES);
-                const uint64_t *src = a.spins + (size_t)c * Nh;
-                const unsigned zlo = (z0 - 1) & (L - 1), zhi = (z0 + TZ) & (L - 1);
-                const unsigned ylo = (y0 - 1) & (L - 1), yhi = (y0 + TY) & (L - 1);
-                bulk_g2s(tile_at(c, 0, 1), src + Lh * (y0 + L * zlo), TY * Lh * 8, halo_bar);
-                bulk_g2s(tile_at(c, HZ - 1, 1), src + Lh * (y0 + L * zhi), TY * Lh * 8, halo_bar);
-                for (int zz = 1; zz <= TZ; ++zz) {
-                    const unsigned z = z0 + zz - 1;
-                    bulk_g2s(tile_at(c, zz, 0), src + Lh * (ylo + L * z), Lh * 8, halo_bar);
-                    bulk_g2s(tile_at(c, zz, HY - 1), src + Lh * (yhi + L * z), Lh * 8, halo_bar);
-                }
+                bulk_g2s(tile + (size_t)c * HZ * HY * Lh + cp_dst, a.spins + (size_t)c * Nh + cp_src, cp_bytes, halo_bar);
             }
         }
     } else {
         // ---- compute warps -----------------------------------------------------------------------------
-        const unsigned k = lane;
-        const int lane_m = (int)((k - 1) & 31), lane_p = (int)((k + 1) & 31);
-        int n_bnd = 0; // boundary rows of this warp: indices warp + CW*i < NB
-        for (int i = 0; i < RPW; ++i) n_bnd += ((int)warp + CW * i < G::NB);
-        uint32_t rt[RPW];
+        const int n_bnd = tab.n_bnd[warp];
+        const unsigned phi = tab.phi[warp];
+        const uint4 *__restrict__ desc = rowdesc + warp * RPW;
+        ResidentStep x;
+        x.k = lane;
+        x.lane_m = (int)((lane - 1) & 31);
+        x.lane_p = (int)((lane + 1) & 31);
+        SweepRng g;
 #pragma unroll
-        for (int i = 0; i < RPW; ++i) rt[i] = rowtab[warp + CW * i];
+        for (int r = 0; r < 10; ++r) { g.k0[r] = a.k0[r]; g.k1[r] = a.k1[r]; }
 
-        RowBonds<BondT> nxt; // software pipeline: the bond words of the next row are in flight during this row
-        {
-            const unsigned yy = rt[0] & 0xff, zz = rt[0] >> 8;
-            nxt = load_row_bonds<G, BondT>(bonds, bonds + (size_t)3 * Nh, y0 + yy - 1, z0 + zz - 1, k);
-        }
+        // software pipeline: the bond words of the next row are always in flight
+        RowBonds<BondT> nxt = load_row_bonds<BondT>(Ptr32(bonds + 2 * lane), Ptr32(bonds + (size_t)3 * Nh + 2 * lane), desc[0], Nh);
         for (uint32_t h = 0; h < a.n_half; ++h) {
             const int c = h & 1;
-            const SweepRng g = make_sweep_rng(a.seed, a.t0 + (h >> 1), (uint32_t)c);
-            const BondT *__restrict__ Jc = bonds + (size_t)c * 3 * Nh;
-            const BondT *__restrict__ Jo = bonds + (size_t)(1 - c) * 3 * Nh;
-            uint64_t *gown = a.spins + (size_t)c * Nh;
+            sweep_rng_set_time(g, a.t0 + (h >> 1), (uint32_t)c);
+            const Ptr32 Jc_l(bonds + (size_t)c * 3 * Nh + 2 * lane), Jo_l(bonds + (size_t)(1 - c) * 3 * Nh + 2 * lane);
+            x.s_own = (unsigned char *)(tile + (size_t)c * HZ * HY * Lh) + 16 * lane;
+            x.s_oth = (const unsigned char *)(tile + (size_t)(1 - c) * HZ * HY * Lh) + 16 * lane;
+            x.g_own = Ptr32(a.spins + (size_t)c * Nh + 2 * lane);
             if (h > 0) { // halo of colour 1-c, pulled in during step h-1
                 const unsigned parity = (h - 1) & 1;
                 while (!mbar_try_wait(halo_bar, parity)) { } // always completes: the producer arms it even on abort
             }
             if (n_bnd == 0) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
-#pragma unroll
-            for (int i = 0; i < RPW; ++i) {
-                const unsigned yy = rt[i] & 0xff, zz = rt[i] >> 8;
-                const unsigned y = y0 + yy - 1, z = z0 + zz - 1;
-                const RowBonds<BondT> cur = nxt;
-                { // prefetch the next row's bonds (next half-step's first row at the end of this one)
-                    const uint32_t e = rt[(i + 1) % RPW];
-                    const unsigned yn = y0 + (e & 0xff) - 1, zn = z0 + (e >> 8) - 1;
-                    if (i + 1 < RPW) nxt = load_row_bonds<G, BondT>(Jc, Jo, yn, zn, k);
-                    else nxt = load_row_bonds<G, BondT>(Jo, Jc, yn, zn, k); // colours swap roles next step
-                }
-                uint64_t *own_row = tile_at(c, zz, yy) + 2 * k;
-                const ulonglong2 own = *(const ulonglong2 *)own_row;
-                const ulonglong2 P0 = *(const ulonglong2 *)(tile_at(1 - c, zz, yy) + 2 * k);
-                const ulonglong2 Pm = *(const ulonglong2 *)(tile_at(1 - c, zz, yy - 1) + 2 * k);
-                const ulonglong2 Pp = *(const ulonglong2 *)(tile_at(1 - c, zz, yy + 1) + 2 * k);
-                const ulonglong2 Zm = *(const ulonglong2 *)(tile_at(1 - c, zz - 1, yy) + 2 * k);
-                const ulonglong2 Zp = *(const ulonglong2 *)(tile_at(1 - c, zz + 1, yy) + 2 * k);
-                const unsigned s = ((unsigned)c ^ (y + z)) & 1u;
-                const uint32_t site0 = 4 * k + s + L * (y + L * z);
-                ulonglong2 out;
-                if (s == 0)
-                    out = update_pair<0, BondT, ALWAYS>(own, P0, Pm, Pp, Zm, Zp, cur.jx, cur.jy, cur.jz, cur.bx, cur.by,
-                                                       cur.bz, site0, g, a.th, lane_m, lane_p);
-                else
-                    out = update_pair<1, BondT, ALWAYS>(own, P0, Pm, Pp, Zm, Zp, cur.jx, cur.jy, cur.jz, cur.bx, cur.by,
-                                                       cur.bz, site0, g, a.th, lane_m, lane_p);
-                *(ulonglong2 *)own_row = out;
-                if (i < n_bnd) {
-                    *(ulonglong2 *)(gown + Lh * (y + L * z) + 2 * k) = out;
-                    if (i == n_bnd - 1) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
-                }
-            }
+            // y0, z0 are even, so the phase of row i is (c ^ phi ^ i) & 1
+            if (((unsigned)c ^ phi) & 1u) resident_step<1, G, BondT, ALWAYS>(x, desc, n_bnd, nxt, Jc_l, Jo_l, g, a.th);
+            else resident_step<0, G, BondT, ALWAYS>(x, desc, n_bnd, nxt, Jc_l, Jo_l, g, a.th);
             named_bar_sync(BAR_STEP, CW * 32); // colour c of the tile is complete before anyone reads it
         }
         // ---- epilogue: interior rows were never stored; write them back (boundary rows are current) ----
-#pragma unroll
-        for (int i = 0; i < RPW; ++i) {
-            if (i < n_bnd) continue;
-            const unsigned yy = rt[i] & 0xff, zz = rt[i] >> 8;
-            const unsigned y = y0 + yy - 1, z = z0 + zz - 1;
+        for (int i = n_bnd; i < RPW; ++i) {
+            const uint4 d = desc[i];
 #pragma unroll
             for (int c = 0; c < 2; ++c)
-                *(ulonglong2 *)(a.spins + (size_t)c * Nh + Lh * (y + L * z) + 2 * k) =
-                    *(const ulonglong2 *)(tile_at(c, zz, yy) + 2 * k);
+                *(ulonglong2 *)(a.spins + (size_t)c * Nh + d.y + 2 * lane) =
+                    *(const ulonglong2 *)((const unsigned char *)(tile + (size_t)c * HZ * HY * Lh) + d.x + 16 * lane);
         }
     }
+}
+
+// Host side of the row schedule (see RowTable).  Boundary rows are dealt out along the ring, interior rows along a
+// boustrophedon path, so consecutive rows of a warp are lattice neighbours and alternate in (yy + zz) parity.
+template <typename G> static bool build_row_table(RowTable<G> &t)
+{
+    constexpr int TY = G::TY, TZ = G::TZ, CW = G::CW, RPW = G::ROWS / G::CW;
+    static_assert(TY % 2 == 0 && TZ % 2 == 0, "tile origin parity must be even");
+    std::vector<std::pair<int, int>> ring, snake;
+    for (int yy = 1; yy <= TY; ++yy) ring.push_back({yy, 1});
+    for (int zz = 2; zz <= TZ; ++zz) ring.push_back({TY, zz});
+    for (int yy = TY - 1; yy >= 1; --yy) ring.push_back({yy, TZ});
+    for (int zz = TZ - 1; zz >= 2; --zz) ring.push_back({1, zz});
+    for (int zz = 2; zz <= TZ - 1; ++zz)
+        for (int j = 0; j < TY - 2; ++j) snake.push_back({(zz & 1) ? TY - 1 - j : 2 + j, zz});
+    if ((int)ring.size() != G::NB || (int)(ring.size() + snake.size()) != G::ROWS) return false;
+    // boundary rows: the first (NB % CW) warps... every warp gets floor or ceil of NB / CW consecutive ring rows
+    const int lo = G::NB / CW, n_hi = G::NB % CW; // n_hi warps take lo + 1
+    int pos = 0;
+    int need[CW], len[CW];
+    for (int w = 0; w < CW; ++w) {
+        const int nb = lo + (w < n_hi ? 1 : 0);
+        t.n_bnd[w] = (uint8_t)nb;
+        t.phi[w] = nb ? (uint8_t)((ring[pos].first + ring[pos].second) & 1) : 0;
+        for (int i = 0; i < nb; ++i, ++pos) t.row[w][i] = (uint16_t)(ring[pos].first | (ring[pos].second << 8));
+        need[w] = (t.phi[w] + nb) & 1; // parity the first interior row must have
+        len[w] = RPW - nb;
+    }
+    // interior rows: walk the snake, each time handing the next segment to a warp whose parity fits
+    bool done[CW] = {};
+    pos = 0;
+    for (int n = 0; n < CW; ++n) {
+        int pick = -1;
+        for (int w = 0; w < CW && pick < 0; ++w) {
+            if (done[w]) continue;
+            if (len[w] == 0) pick = w;
+            else if (pos < (int)snake.size() && ((snake[pos].first + snake[pos].second) & 1) == need[w]) pick = w;
+        }
+        if (pick < 0) return false;
+        done[pick] = true;
+        for (int i = 0; i < len[pick]; ++i, ++pos) {
+            if (pos >= (int)snake.size()) return false;
+            t.row[pick][t.n_bnd[pick] + i] = (uint16_t)(snake[pos].first | (snake[pos].second << 8));
+        }
+    }
+    if (pos != (int)snake.size()) return false;
+    // check: every row once, alternating parity from phi, boundary rows first
+    std::vector<int> seen((TY + 2) * (TZ + 2), 0);
+    for (int w = 0; w < CW; ++w)
+        for (int i = 0; i < RPW; ++i) {
+            const int yy = t.row[w][i] & 0xff, zz = t.row[w][i] >> 8;
+            const bool isB = yy == 1 || yy == TY || zz == 1 || zz == TZ;
+            if (yy < 1 || yy > TY || zz < 1 || zz > TZ || seen[zz * (TY + 2) + yy]++) return false;
+            if (((yy + zz) & 1) != ((t.phi[w] + i) & 1) || isB != (i < t.n_bnd[w])) return false;
+        }
+    return true;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -294,10 +408,13 @@ typedef ResidentGeom<128, 16, 8> Geom128;
 template <typename BondT, bool ALWAYS>
 static cudaError_t launch_resident_typed(ea_sim *s, ResidentArgs &a, cudaStream_t st)
 {
+    static RowTable<Geom128> tab;
+    static const bool tab_ok = build_row_table<Geom128>(tab);
+    if (!tab_ok) return cudaErrorInvalidConfiguration;
     auto kern = k_sweep_resident<Geom128, BondT, ALWAYS>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Geom128::SMEM_BYTES);
     if (e != cudaSuccess) return e;
-    void *args[] = {&a};
+    void *args[] = {&a, &tab};
     return cudaLaunchCooperativeKernel((void *)kern, dim3(Geom128::G), dim3(Geom128::THREADS), args, Geom128::SMEM_BYTES, st);
 }
 
@@ -306,6 +423,10 @@ bool resident_supported(const ea_sim *s)
     if (s->lat.L != 128) return false;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) return false;
+    // the row loop does 32-bit address arithmetic (Ptr32): no array may straddle a 4 GiB boundary
+    const uintptr_t b0 = (uintptr_t)s->bonds, b1 = b0 + (size_t)6 * s->lat.Nh * s->bond_bytes() - 1;
+    const uintptr_t s0 = (uintptr_t)s->spins, s1 = s0 + (size_t)2 * s->lat.Nh * 8 - 1;
+    if ((b0 >> 32) != (b1 >> 32) || (s0 >> 32) != (s1 >> 32)) return false;
     return prop.cooperativeLaunch && prop.multiProcessorCount >= Geom128::G &&
            prop.sharedMemPerBlockOptin >= Geom128::SMEM_BYTES;
 }
@@ -318,7 +439,8 @@ cudaError_t launch_sweeps_resident(ea_sim *s, uint64_t t0, uint32_t n, cudaStrea
     ResidentArgs a;
     a.spins = s->spins;
     a.bonds = s->bonds;
-    a.seed = s->seed;
+    { const SweepRng g0 = make_sweep_rng(s->seed, 0, 0);
+      for (int r = 0; r < 10; ++r) { a.k0[r] = g0.k0[r]; a.k1[r] = g0.k1[r]; } }
     a.t0 = t0;
     a.n_half = 2 * n;
     a.epoch0 = s->resident_epoch;
