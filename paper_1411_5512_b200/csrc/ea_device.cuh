@@ -160,18 +160,34 @@ __device__ __forceinline__ uint32_t maj3(uint32_t a, uint32_t b, uint32_t c) { r
 //   f = [n_u >= 3] | [r < thr[2]] [n_u >= 2] | [r < thr[1]] [n_u >= 1] | [r < thr[0]]
 // and each rare term is one or two predicated LOP3 behind an ISETP (no masks are materialised).
 // ALWAYS: some thr[k] == 2^32 (T = inf), which a 32-bit compare cannot express -- OR-ed in as masks.
+struct HalfCount { uint32_t sa, ka, sb, kb; };
+
+__device__ __forceinline__ HalfCount count_half(uint32_t u1, uint32_t u2, uint32_t u3, uint32_t u4, uint32_t u5, uint32_t u6)
+{
+    HalfCount h;
+    h.sa = xor3(u1, u2, u3); h.ka = maj3(u1, u2, u3);
+    h.sb = xor3(u4, u5, u6); h.kb = maj3(u4, u5, u6);
+    return h;
+}
+
+// the energy-raising levels of one half, given that r < thr[2] is possible
+__device__ __forceinline__ uint32_t raise_half(uint32_t f, const HalfCount &h, uint32_t r, const Thresholds &th)
+{
+    const uint32_t t = h.sa | h.sb;
+    if (r < th.thr[2]) f = h.ka | h.kb | (h.sa & h.sb);
+    if (r < th.thr[1]) f = h.ka | h.kb | t;
+    if (r < th.thr[0]) f = 0xffffffffu;
+    return f;
+}
+
 template <bool ALWAYS>
 __device__ __forceinline__ uint32_t flip_half(uint32_t u1, uint32_t u2, uint32_t u3, uint32_t u4, uint32_t u5,
                                               uint32_t u6, uint32_t r, const Thresholds &th)
 {
-    const uint32_t sa = xor3(u1, u2, u3), ka = maj3(u1, u2, u3);
-    const uint32_t sb = xor3(u4, u5, u6), kb = maj3(u4, u5, u6);
-    const uint32_t t = sa | sb;
-    uint32_t f = maj3(ka, kb, t);
-    if (r < th.thr[2]) f = ka | kb | (sa & sb);
-    if (r < th.thr[1]) f = ka | kb | t;
-    if (r < th.thr[0]) f = 0xffffffffu;
-    if (ALWAYS) f |= (th.always[2] & (ka | kb | (sa & sb))) | (th.always[1] & (ka | kb | t)) | th.always[0];
+    const HalfCount h = count_half(u1, u2, u3, u4, u5, u6);
+    const uint32_t t = h.sa | h.sb;
+    uint32_t f = raise_half(maj3(h.ka, h.kb, t), h, r, th);
+    if (ALWAYS) f |= (th.always[2] & (h.ka | h.kb | (h.sa & h.sb))) | (th.always[1] & (h.ka | h.kb | t)) | th.always[0];
     return f;
 }
 
@@ -188,13 +204,28 @@ __device__ __forceinline__ uint32_t bond_hi(uint32_t j) { return j; } // replica
 
 // One whole Metropolis trial of a 64-sample word: returns the new spin word.  (n_d, j_d), d = 1..6: the six
 // neighbour words with the bond word that couples each to this site, in any order (n_u is a count).
-template <typename BondT, bool ALWAYS>
+// RARE (low temperature, thr[2] << 2^32): the three energy-raising levels sit behind ONE warp-level branch per
+// word, taken only if some lane drew r < thr[2] in either half (T = 0.8: 0.7 % per draw, 35 % per warp and word),
+// instead of six compares and eight predicated LOP3 on the alu pipe that binds these kernels.  Same result.
+template <typename BondT, bool ALWAYS, bool RARE = false>
 __device__ __forceinline__ uint64_t metropolis_word(uint64_t s, uint64_t n1, uint64_t n2, uint64_t n3, uint64_t n4,
                                                     uint64_t n5, uint64_t n6, BondT j1, BondT j2, BondT j3, BondT j4,
                                                     BondT j5, BondT j6, uint32_t r_lo, uint32_t r_hi,
                                                     const Thresholds &th)
 {
     const uint32_t sl = lo32(s), sh = hi32(s);
+    if (RARE && !ALWAYS) {
+        const HalfCount hl = count_half(bond_lo(j1) ^ sl ^ lo32(n1), bond_lo(j2) ^ sl ^ lo32(n2), bond_lo(j3) ^ sl ^ lo32(n3),
+                                        bond_lo(j4) ^ sl ^ lo32(n4), bond_lo(j5) ^ sl ^ lo32(n5), bond_lo(j6) ^ sl ^ lo32(n6));
+        const HalfCount hh = count_half(bond_hi(j1) ^ sh ^ hi32(n1), bond_hi(j2) ^ sh ^ hi32(n2), bond_hi(j3) ^ sh ^ hi32(n3),
+                                        bond_hi(j4) ^ sh ^ hi32(n4), bond_hi(j5) ^ sh ^ hi32(n5), bond_hi(j6) ^ sh ^ hi32(n6));
+        uint32_t fl = maj3(hl.ka, hl.kb, hl.sa | hl.sb), fh = maj3(hh.ka, hh.kb, hh.sa | hh.sb);
+        if (min(r_lo, r_hi) < th.thr[2]) {
+            fl = raise_half(fl, hl, r_lo, th);
+            fh = raise_half(fh, hh, r_hi, th);
+        }
+        return mk64(sl ^ fl, sh ^ fh);
+    }
     const uint32_t fl = flip_half<ALWAYS>(bond_lo(j1) ^ sl ^ lo32(n1), bond_lo(j2) ^ sl ^ lo32(n2),
                                           bond_lo(j3) ^ sl ^ lo32(n3), bond_lo(j4) ^ sl ^ lo32(n4),
                                           bond_lo(j5) ^ sl ^ lo32(n5), bond_lo(j6) ^ sl ^ lo32(n6), r_lo, th);

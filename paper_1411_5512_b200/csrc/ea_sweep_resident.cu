@@ -102,6 +102,7 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
 }
 
 enum { BAR_BOUNDARY = 1, BAR_STEP = 2 };
+constexpr uint32_t RARE_THR2_MAX = 0x04000000u; // P(r < thr[2]) < 1/64: the warp-level branch of metropolis_word pays
 constexpr unsigned long long RESIDENT_TIMEOUT_NS = 2000000000ull; // a neighbour that never shows up: give up after 2 s
 
 // Row schedule of one CTA (built on the host, build_row_table): compute warp w updates rows row[w][0..RPW-1]
@@ -171,10 +172,22 @@ struct ResidentStep {
     int lane_m, lane_p;
 };
 
+// the four random numbers of the lane's two words of a row (d.y = row offset, S = row phase): independent of the
+// spins, so they are drawn one row ahead and their IMAD.WIDE chain (fma pipe) overlaps the LOP3 logic (alu pipe)
+// of the row before
+__device__ __forceinline__ uint4 row_random(const SweepRng &g, const unsigned k, const unsigned S, const uint4 d)
+{
+    const uint32_t site0 = 4 * k + S + 2 * d.y; // canonical site = x + L (y + L z), L = 2 Lh
+    uint4 r;
+    sweep_random(g, site0, r.x, r.y);
+    sweep_random(g, site0 + 2, r.z, r.w);
+    return r;
+}
+
 // one row of colour c with compile-time phase S; publishes it to global when `publish`
-template <int S, typename G, typename BondT, bool ALWAYS>
+template <int S, typename G, typename BondT, bool ALWAYS, bool RARE>
 __device__ __forceinline__ void resident_row(const ResidentStep &x, const uint4 d, const RowBonds<BondT> &bd,
-                                             const SweepRng &g, const Thresholds &th, const bool publish)
+                                             const uint4 r, const Thresholds &th, const bool publish)
 {
     constexpr int ROWB = G::Lh * 8, PLANEB = G::HY * G::Lh * 8; // smem strides: next y row, next z plane
     unsigned char *own_row = x.s_own + d.x;
@@ -185,38 +198,47 @@ __device__ __forceinline__ void resident_row(const ResidentStep &x, const uint4 
     const ulonglong2 Pp = *(const ulonglong2 *)(o + ROWB);
     const ulonglong2 Zm = *(const ulonglong2 *)(o - PLANEB);
     const ulonglong2 Zp = *(const ulonglong2 *)(o + PLANEB);
-    const uint32_t site0 = 4 * x.k + S + 2 * d.y; // canonical site = x + L (y + L z), L = 2 Lh
-    const ulonglong2 out = update_pair<S, BondT, ALWAYS>(own, P0, Pm, Pp, Zm, Zp, bd.jx, bd.jy, bd.jz, bd.bx, bd.by, bd.bz,
-                                                         site0, g, th, x.lane_m, x.lane_p);
+    const ulonglong2 out = update_pair_r<S, BondT, ALWAYS, RARE>(own, P0, Pm, Pp, Zm, Zp, bd.jx, bd.jy, bd.jz, bd.bx, bd.by,
+                                                                 bd.bz, r, th, x.lane_m, x.lane_p);
     *(ulonglong2 *)own_row = out;
     if (publish) *x.g_own.at<ulonglong2>(d.y / 2) = out;
 }
 
-// all rows of one compute warp for one half-step; S0 = phase of the warp's first row
-template <int S0, typename G, typename BondT, bool ALWAYS>
+// all rows of one compute warp for one half-step; S0 = phase of the warp's first row.  Carried across rows and
+// steps: nxt = bond words of the next row, rnx = random numbers of the next row (gn = stream of the next step).
+template <int S0, typename G, typename BondT, bool ALWAYS, bool RARE>
 __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4 *__restrict__ desc, const int n_bnd,
-                                              RowBonds<BondT> &nxt, const Ptr32 Jc_l, const Ptr32 Jo_l,
-                                              const SweepRng &g, const Thresholds &th)
+                                              RowBonds<BondT> &nxt, uint4 &rnx, const Ptr32 Jc_l, const Ptr32 Jo_l,
+                                              const SweepRng &g, const SweepRng &gn, const Thresholds &th)
 {
     constexpr int RPW = G::ROWS / G::CW;
     constexpr unsigned Nh = (unsigned)G::L * G::L * G::L / 2;
     static_assert(RPW % 2 == 0, "rows are taken two at a time (phases S0, 1 - S0)");
 #pragma unroll 1
     for (int i = 0; i < RPW; i += 2) {
-        const uint4 d0 = desc[i], d1 = desc[i + 1], d2 = desc[(i + 2) % RPW];
+        const bool last = i + 2 >= RPW;
+        const uint4 d0 = desc[i], d1 = desc[i + 1], d2 = desc[last ? 0 : i + 2];
         const RowBonds<BondT> b0 = nxt;
+        const uint4 r0 = rnx;
         const RowBonds<BondT> b1 = load_row_bonds<BondT>(Jc_l, Jo_l, d1, Nh);
-        resident_row<S0, G, BondT, ALWAYS>(x, d0, b0, g, th, i < n_bnd);
+        const uint4 r1 = row_random(g, x.k, 1 - S0, d1);
+        resident_row<S0, G, BondT, ALWAYS, RARE>(x, d0, b0, r0, th, i < n_bnd);
         if (i + 1 == n_bnd) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
-        // the row after next: first row of the next half-step (colours swap roles) when this is the last pair
-        if (i + 2 < RPW) nxt = load_row_bonds<BondT>(Jc_l, Jo_l, d2, Nh);
-        else nxt = load_row_bonds<BondT>(Jo_l, Jc_l, d2, Nh);
-        resident_row<1 - S0, G, BondT, ALWAYS>(x, d1, b1, g, th, i + 1 < n_bnd);
+        // the row after next; for the last pair that is the first row of the next half-step: the colours swap
+        // roles, the stream moves on, and the phase of row 0 flips with the colour
+        if (!last) {
+            nxt = load_row_bonds<BondT>(Jc_l, Jo_l, d2, Nh);
+            rnx = row_random(g, x.k, S0, d2);
+        } else {
+            nxt = load_row_bonds<BondT>(Jo_l, Jc_l, d2, Nh);
+            rnx = row_random(gn, x.k, 1 - S0, d2);
+        }
+        resident_row<1 - S0, G, BondT, ALWAYS, RARE>(x, d1, b1, r1, th, i + 1 < n_bnd);
         if (i + 2 == n_bnd) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
     }
 }
 
-template <typename G, typename BondT, bool ALWAYS>
+template <typename G, typename BondT, bool ALWAYS, bool RARE>
 __global__ void __launch_bounds__(G::THREADS, 1) k_sweep_resident(const ResidentArgs a, const RowTable<G> tab)
 {
     constexpr int L = G::L, Lh = G::Lh, TY = G::TY, TZ = G::TZ, HY = G::HY, HZ = G::HZ, CW = G::CW, ROWS = G::ROWS;
@@ -318,9 +340,13 @@ __global__ void __launch_bounds__(G::THREADS, 1) k_sweep_resident(const Resident
 
         // software pipeline: the bond words of the next row are always in flight
         RowBonds<BondT> nxt = load_row_bonds<BondT>(Ptr32(bonds + 2 * lane), Ptr32(bonds + (size_t)3 * Nh + 2 * lane), desc[0], Nh);
+        sweep_rng_set_time(g, a.t0, 0u);
+        uint4 rnx = row_random(g, lane, phi & 1u, desc[0]); // phase of row 0 in step 0 (colour 0) is phi
         for (uint32_t h = 0; h < a.n_half; ++h) {
             const int c = h & 1;
             sweep_rng_set_time(g, a.t0 + (h >> 1), (uint32_t)c);
+            SweepRng gn = g;
+            sweep_rng_set_time(gn, a.t0 + ((h + 1) >> 1), (uint32_t)(1 - c));
             const Ptr32 Jc_l(bonds + (size_t)c * 3 * Nh + 2 * lane), Jo_l(bonds + (size_t)(1 - c) * 3 * Nh + 2 * lane);
             x.s_own = (unsigned char *)(tile + (size_t)c * HZ * HY * Lh) + 16 * lane;
             x.s_oth = (const unsigned char *)(tile + (size_t)(1 - c) * HZ * HY * Lh) + 16 * lane;
@@ -331,8 +357,8 @@ __global__ void __launch_bounds__(G::THREADS, 1) k_sweep_resident(const Resident
             }
             if (n_bnd == 0) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
             // y0, z0 are even, so the phase of row i is (c ^ phi ^ i) & 1
-            if (((unsigned)c ^ phi) & 1u) resident_step<1, G, BondT, ALWAYS>(x, desc, n_bnd, nxt, Jc_l, Jo_l, g, a.th);
-            else resident_step<0, G, BondT, ALWAYS>(x, desc, n_bnd, nxt, Jc_l, Jo_l, g, a.th);
+            if (((unsigned)c ^ phi) & 1u) resident_step<1, G, BondT, ALWAYS, RARE>(x, desc, n_bnd, nxt, rnx, Jc_l, Jo_l, g, gn, a.th);
+            else resident_step<0, G, BondT, ALWAYS, RARE>(x, desc, n_bnd, nxt, rnx, Jc_l, Jo_l, g, gn, a.th);
             named_bar_sync(BAR_STEP, CW * 32); // colour c of the tile is complete before anyone reads it
         }
         // ---- epilogue: interior rows were never stored; write them back (boundary rows are current) ----
@@ -405,13 +431,13 @@ template <typename G> static bool build_row_table(RowTable<G> &t)
 // ---------------------------------------------------------------------------------------------
 typedef ResidentGeom<128, 16, 8> Geom128;
 
-template <typename BondT, bool ALWAYS>
+template <typename BondT, bool ALWAYS, bool RARE>
 static cudaError_t launch_resident_typed(ea_sim *s, ResidentArgs &a, cudaStream_t st)
 {
     static RowTable<Geom128> tab;
     static const bool tab_ok = build_row_table<Geom128>(tab);
     if (!tab_ok) return cudaErrorInvalidConfiguration;
-    auto kern = k_sweep_resident<Geom128, BondT, ALWAYS>;
+    auto kern = k_sweep_resident<Geom128, BondT, ALWAYS, RARE>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Geom128::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     void *args[] = {&a, &tab};
@@ -448,11 +474,17 @@ cudaError_t launch_sweeps_resident(ea_sim *s, uint64_t t0, uint32_t n, cudaStrea
     a.abort_flag = s->resident_flags + Geom128::G * 32;
     a.th = s->th;
     const bool always = a.th.always[0] | a.th.always[1] | a.th.always[2];
+    // low temperature: energy-raising moves are rare enough for a warp-level branch (see metropolis_word)
+    const bool rare = !always && a.th.thr[2] < RARE_THR2_MAX;
     cudaError_t e;
     if (s->n_replicas == 2)
-        e = always ? launch_resident_typed<uint32_t, true>(s, a, st) : launch_resident_typed<uint32_t, false>(s, a, st);
+        e = always ? launch_resident_typed<uint32_t, true, false>(s, a, st)
+            : rare ? launch_resident_typed<uint32_t, false, true>(s, a, st)
+                   : launch_resident_typed<uint32_t, false, false>(s, a, st);
     else
-        e = always ? launch_resident_typed<uint64_t, true>(s, a, st) : launch_resident_typed<uint64_t, false>(s, a, st);
+        e = always ? launch_resident_typed<uint64_t, true, false>(s, a, st)
+            : rare ? launch_resident_typed<uint64_t, false, true>(s, a, st)
+                   : launch_resident_typed<uint64_t, false, false>(s, a, st);
     if (e == cudaSuccess) {
         s->resident_epoch += 2 * n;
         s->count_launch();
