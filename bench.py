@@ -45,9 +45,18 @@ UNIT = "ps/attempt"
 LANES = 64
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE half-sweep launch at the bench configuration, from the
-# `ncu --set full` capture summarised in profiles/ (the .md names the command); None = not captured.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 41996032  # profiles/r01_ncu_full_k_sweep_rows.md (cold L2: ncu flushes caches per launch)
+# From the `ncu --set full` captures summarised in profiles/ (each .md names its command), per kernel variant:
+#   traffic  = dram__bytes_read.sum + dram__bytes_write.sum of ONE launch at the bench configuration (cold L2: ncu
+#              flushes the caches before the launch).  ROWS: one launch = one half-sweep.  RESIDENT: one launch =
+#              the whole ea_sweep(S) call (2 S half-sweeps): the lattice is read once and written back once.
+#   alu_inst = sm__inst_executed_pipe_alu.sum per half-sweep (warp instructions on the LOP3/ISETP pipe).
+NCU = {
+    "rows": {"traffic": 41996032, "alu_inst": None, "profile": "profiles/r01_ncu_full_k_sweep_rows.md"},
+    "resident": {"traffic": None, "alu_inst": None, "profile": None},
+}
+# alu pipe: one warp instruction per 2 clocks per SM sub-partition (B300_MICROARCH "Pipe rates": rt_SMSP = 2),
+# 4 sub-partitions x 148 SMs, at the max SM clock of MEASURED_PEAKS.json (1965 MHz): DESIGN.md section 6
+ALU_PEAK_WARP_INST_PER_S = 148 * 4 * 0.5 * 1.965e9
 
 
 def algorithmic_bytes_per_half_sweep(N, n_replicas):
@@ -298,14 +307,26 @@ def run_ours(args, cfg):
     t_half = t_sweeps / (2.0 * S * K)
     alg = algorithmic_bytes_per_half_sweep(N, cfg.n_replicas)
     achieved = alg / t_half / 1e9
-    roofline = {"bound": "hbm", "kernel": "half-sweep (%s)" % binding_kernel_name(sim.kernel),
+    kname = binding_kernel_name(sim.kernel)
+    resident = kname == "resident" and S >= 8  # AUTO sends shorter calls through the ROWS launches
+    hs_per_launch = 2 * S if resident else 1
+    ncu = NCU.get(kname, {})
+    roofline = {"bound": "hbm", "kernel": "half-sweep (%s)" % kname,
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "algorithmic_bytes_per_launch": alg,
-                "us_per_launch": 1e6 * t_half, "peak_source": peak_src,
-                "share_of_step": t_sweeps / t_steps,
-                "note": "achieved = algorithmic bytes / mean half-sweep duration (CUDA events on the sim's stream "
-                        "around ea_sweep(S), / 2S). The lattice is L2-resident inside a step, so frac can exceed "
-                        "what DRAM alone allows; DESIGN.md section 6 gives the L2 and integer-pipe bounds"}
+                "traffic": ncu.get("traffic"), "half_sweeps_per_launch": hs_per_launch,
+                "algorithmic_bytes_per_launch": alg * hs_per_launch,
+                "us_per_launch": 1e6 * t_half * hs_per_launch, "us_per_half_sweep": 1e6 * t_half,
+                "peak_source": peak_src, "share_of_step": t_sweeps / t_steps, "profile": ncu.get("profile"),
+                "note": "achieved = algorithmic bytes per launch / mean launch duration (CUDA events on the sim's "
+                        "stream around ea_sweep(S)). north_star: the roofline is the slower of bytes / HBM bandwidth "
+                        "and integer ops / issue rate -- HBM (7.7 us per half-sweep) is the slower one, so bound = "
+                        "hbm; the lattice is L2-resident (ROWS) or shared-memory-resident (RESIDENT) inside a step, "
+                        "so frac exceeds 1 and the alu figure below is the bound that then applies (DESIGN.md 6)"}
+    if ncu.get("alu_inst"):
+        alu_rate = ncu["alu_inst"] / t_half
+        roofline["alu"] = {"achieved": alu_rate / 1e9, "peak": ALU_PEAK_WARP_INST_PER_S / 1e9,
+                           "unit": "G warp-inst/s (alu pipe)", "frac": alu_rate / ALU_PEAK_WARP_INST_PER_S,
+                           "alu_warp_inst_per_half_sweep": ncu["alu_inst"]}
     sim.close()
 
     cpu_baseline = None

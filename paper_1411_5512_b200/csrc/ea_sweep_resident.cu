@@ -38,14 +38,15 @@ struct ResidentArgs {
     Thresholds th;
 };
 
-template <int L_, int TY_, int TZ_> struct ResidentGeom {
+template <int L_, int TY_, int TZ_, int CW_, bool UNROLL_> struct ResidentGeom {
     static constexpr int L = L_, TY = TY_, TZ = TZ_;
     static constexpr int Lh = L / 2;                 // words per colour row
     static constexpr int NTY = L / TY, NTZ = L / TZ; // tiles along y, z
     static constexpr int G = NTY * NTZ;              // CTAs
     static constexpr int ROWS = TY * TZ;             // rows updated per CTA per half-step
     static constexpr int HY = TY + 2, HZ = TZ + 2;   // with halo ring
-    static constexpr int CW = 16;                    // compute warps
+    static constexpr int CW = CW_;                   // compute warps
+    static constexpr bool UNROLL = UNROLL_;          // unroll the row loop of a half-step (code size vs. selects)
     static constexpr int THREADS = (CW + 1) * 32;    // + one producer warp
     static constexpr int NB = ROWS - (TY - 2) * (TZ - 2); // boundary rows
     static constexpr unsigned HALO_BYTES = (2 * TY + 2 * TZ) * Lh * 8;
@@ -214,7 +215,7 @@ __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4
     constexpr int RPW = G::ROWS / G::CW;
     constexpr unsigned Nh = (unsigned)G::L * G::L * G::L / 2;
     static_assert(RPW % 2 == 0, "rows are taken two at a time (phases S0, 1 - S0)");
-#pragma unroll 1
+#pragma unroll(G::UNROLL ? RPW / 2 : 1)
     for (int i = 0; i < RPW; i += 2) {
         const bool last = i + 2 >= RPW;
         const uint4 d0 = desc[i], d1 = desc[i + 1], d2 = desc[last ? 0 : i + 2];
@@ -429,19 +430,25 @@ template <typename G> static bool build_row_table(RowTable<G> &t)
 }
 
 // ---------------------------------------------------------------------------------------------
-typedef ResidentGeom<128, 16, 8> Geom128;
+// 32-bit bond words (2 replicas): 16 compute warps, row loop unrolled (89 -> 96 registers, no spills).
+// 64-bit bond words: twice the bond registers in flight, so 8 compute warps with up to 168 registers each.
+template <typename BondT> struct Geom128Of { typedef ResidentGeom<128, 16, 8, 16, true> type; };
+template <> struct Geom128Of<uint64_t> { typedef ResidentGeom<128, 16, 8, 8, false> type; };
+typedef Geom128Of<uint32_t>::type Geom128; // tile shape, grid and flag layout are the same for both
 
 template <typename BondT, bool ALWAYS, bool RARE>
 static cudaError_t launch_resident_typed(ea_sim *s, ResidentArgs &a, cudaStream_t st)
 {
-    static RowTable<Geom128> tab;
-    static const bool tab_ok = build_row_table<Geom128>(tab);
+    typedef typename Geom128Of<BondT>::type G;
+    static_assert(G::G == Geom128::G && G::SMEM_BYTES == Geom128::SMEM_BYTES, "one flag / shared-memory layout");
+    static RowTable<G> tab;
+    static const bool tab_ok = build_row_table<G>(tab);
     if (!tab_ok) return cudaErrorInvalidConfiguration;
-    auto kern = k_sweep_resident<Geom128, BondT, ALWAYS, RARE>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Geom128::SMEM_BYTES);
+    auto kern = k_sweep_resident<G, BondT, ALWAYS, RARE>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     void *args[] = {&a, &tab};
-    return cudaLaunchCooperativeKernel((void *)kern, dim3(Geom128::G), dim3(Geom128::THREADS), args, Geom128::SMEM_BYTES, st);
+    return cudaLaunchCooperativeKernel((void *)kern, dim3(G::G), dim3(G::THREADS), args, G::SMEM_BYTES, st);
 }
 
 bool resident_supported(const ea_sim *s)

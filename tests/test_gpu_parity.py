@@ -186,6 +186,52 @@ def test_full_size_L128_every_word(name):
     assert_same_observables(g, o, slot=0)
 
 
+@pytest.mark.parametrize("n_rep,T,p", [(2, 0.8, 0.77), (1, 0.8, 0.5), (2, 2.0, 0.9), (2, float("inf"), 0.5), (1, 0.0, 0.6)])
+def test_resident_kernel_L128_against_the_oracle(n_rep, T, p):
+    """RESIDENT (persistent cooperative kernel, spins in shared memory, neighbour-flag colour barrier): every spin
+    word after 3 and after 3 + 5 sweeps (two launches: flag epochs carry over), both bond widths, the three
+    acceptance code paths (rare-branch T = 0.8, predicated T = 2, always-masks T = inf) and T = 0."""
+    L = 128
+    g, o = make_pair(L, p, T, n_rep, wl.seed_for(6, L) + n_rep, n_slots=1, kernel="resident")
+    assert g.kernel == binding.EA_KERNEL_RESIDENT
+    g.snapshot(0)
+    o.snapshot(0)
+    for n in (3, 5):
+        g.sweep(n)
+        o.sweep(n)
+        assert g.time == o.time
+        assert_same_state(g, o, "resident n_rep=%d T=%s t=%d" % (n_rep, T, g.time))
+    assert_same_observables(g, o, slot=0)
+
+
+def test_resident_kernel_long_run_is_identical_to_the_per_colour_launches():
+    """Kernel variants are bit-identical by contract: 3000 sweeps of the bench configuration through RESIDENT
+    (launches of 1, 7, 500 and 2492 sweeps) against the ROWS launches (oracle-checked above and too slow to
+    follow this far on the CPU); then AUTO, which mixes both, continues both to the same state."""
+    c = wl.CONFIGS["cfg4"]
+    a = binding.Sim(c.L, c.p, c.T, n_replicas=c.n_replicas, seed=c.seed, n_slots=1, kernel="rows")
+    b = binding.Sim(c.L, c.p, c.T, n_replicas=c.n_replicas, seed=c.seed, n_slots=1, kernel="resident")
+    for n in (1, 7, 500, 2492):
+        a.sweep(n)
+        b.sweep(n)
+        assert np.array_equal(a.get_spins(), b.get_spins()), "after %d sweeps" % a.time
+    assert np.array_equal(a.energy(), b.energy())
+    a.kernel = "auto"
+    assert a.kernel == binding.EA_KERNEL_RESIDENT
+    for n in (3, 40):  # AUTO: short calls as ROWS launches, long ones as one persistent launch
+        a.sweep(n)
+        b.sweep(n)
+    assert a.time == b.time == 3043
+    assert np.array_equal(a.get_spins(), b.get_spins())
+
+
+def test_resident_kernel_only_where_it_fits():
+    with pytest.raises(Exception):
+        binding.Sim(64, 0.5, 0.8, n_replicas=2, kernel="resident")
+    g = binding.Sim(128, 0.5, 0.8, n_replicas=2, n_slots=0)
+    assert g.kernel == binding.EA_KERNEL_RESIDENT  # AUTO at L = 128
+
+
 @pytest.mark.parametrize("L", [16, 64, 128])
 def test_c4_partial_r_max_and_injected_spins(L):
     """C_4 with r_max < L/2 and on injected random spins (both the generic and the L = 64 / 128 fast path);
