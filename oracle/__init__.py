@@ -52,6 +52,8 @@ def lib():
             "oracle_overlap": (i32, [vp, pi64]),
             "oracle_c4_one": (i32, [vp, i32, i32, pi64]),
             "oracle_c4": (i32, [vp, i32, pi64]),
+            "oracle_c4_vector": (i32, [vp, i32, i32, i32, pi64]),
+            "oracle_c4_shells": (i32, [vp, i32, pi64, pi64]),
             "oracle_get_spins": (None, [vp, pu64]),
             "oracle_set_spins": (None, [vp, pu64]),
             "oracle_get_bonds": (None, [vp, pu64]),
@@ -201,6 +203,23 @@ class Oracle:
             raise ValueError("bad c4 arguments")
         return B
 
+    def c4_vector(self, dx, dy, dz):
+        """B_b(r) = sum_i q_i q_{i+r} for the lattice vector r = (dx, dy, dz) (Eq. 3; reading C-S8v)."""
+        B = np.zeros(32, dtype=np.int64)
+        if lib().oracle_c4_vector(self._h, int(dx), int(dy), int(dz), _p(B, C.c_int64)):
+            raise ValueError("c4_vector needs n_replicas == 2")
+        return B
+
+    def c4_shells(self, r_max):
+        """(S, mult): S[d2, b] = sum of B_b(r) over all vectors with |r|^2 = d2 and components in
+        [-r_max, r_max]; mult[d2] = their number; d2 = 0..3 r_max^2."""
+        n_bins = 3 * r_max * r_max + 1
+        S = np.zeros((n_bins, 32), dtype=np.int64)
+        mult = np.zeros(n_bins, dtype=np.int64)
+        if lib().oracle_c4_shells(self._h, int(r_max), _p(S, C.c_int64), _p(mult, C.c_int64)):
+            raise ValueError("bad c4_shells arguments")
+        return S, mult
+
     # --- canonical packed words ---------------------------------------------------------
     def get_spins(self):
         w = np.zeros(self.N, dtype=np.uint64)
@@ -226,3 +245,53 @@ class Oracle:
         w = np.zeros(self.N, dtype=np.uint64)
         lib().oracle_get_snapshot(self._h, int(slot), _p(w, C.c_uint64))
         return w
+
+
+# ----------------------------------------------------------------------------------------------------
+# Integral estimator of the coherence length (Eq. 5-6; procedure PAPER.md:116).
+# Plain fp64, in the paper's order; reading C-S12:
+#   curve   : points (r_j, c_j, e_j), r ascending from r_0 = 0, c = sample mean of C_4, e = its standard error
+#             over the disorder samples, restricted to r <= r_lim (Eq. 5 integrates to L/2)
+#   cut-off : the integrals run "up to the point, where the value of C_4 first becomes smaller than three times
+#             its error" (:116): j* = first j >= 1 with c_j < 3 e_j, points 0 .. j*-1 are used (all if none)
+#   rule    : trapezoid on the (non-uniform) r grid:  I_k = sum_j (r_j^k c_j + r_{j+1}^k c_{j+1}) (r_{j+1} - r_j) / 2
+#   the paper then adds the tail of its fitted function (4); fits are out of scope, so NO tail is added
+#   xi_k = I_{k+1} / I_k
+# ----------------------------------------------------------------------------------------------------
+def c4_curve(S, mult, N, r_lim):
+    """Shell sums -> (r, c, e).  c_b(d2) = S[d2, b] / (mult[d2] N) per disorder sample b; c = mean over b;
+    e = sqrt(sum_b (c_b - c)^2 / (n (n - 1)))."""
+    S = np.asarray(S, dtype=np.int64)
+    mult = np.asarray(mult, dtype=np.int64)
+    r, c, e = [], [], []
+    n = S.shape[1]
+    for d2 in range(S.shape[0]):
+        if mult[d2] == 0 or d2 > r_lim * r_lim:
+            continue
+        cb = S[d2].astype(np.float64) / (float(mult[d2]) * float(N))
+        mean = float(np.sum(cb)) / n
+        var = float(np.sum((cb - mean) ** 2)) / (n * (n - 1))
+        r.append(float(np.sqrt(float(d2))))
+        c.append(mean)
+        e.append(float(np.sqrt(var)))
+    return np.array(r), np.array(c), np.array(e)
+
+
+def integral_estimator(r, c, e, k):
+    """(I_k, I_{k+1}, xi_k, r_cut) of Eq. 5-6 with the 3-sigma cut-off and the trapezoid rule stated above."""
+    r = np.asarray(r, dtype=np.float64)
+    c = np.asarray(c, dtype=np.float64)
+    e = np.asarray(e, dtype=np.float64)
+    n_use = len(r)
+    for j in range(1, len(r)):
+        if c[j] < 3.0 * e[j]:
+            n_use = j
+            break
+    I = [0.0, 0.0]
+    for m, kk in enumerate((k, k + 1)):
+        acc = 0.0
+        for j in range(n_use - 1):
+            acc += 0.5 * (r[j] ** kk * c[j] + r[j + 1] ** kk * c[j + 1]) * (r[j + 1] - r[j])
+        I[m] = acc
+    xi = I[1] / I[0] if I[0] != 0.0 else float("nan")
+    return I[0], I[1], xi, float(r[n_use - 1])

@@ -428,6 +428,59 @@ int oracle_c4(const oracle_sim *s, int r_max, int64_t *B)
 }
 
 /* ------------------------------------------------------------------------------------
+ * Full-vector four-point correlation.  Eq. 3: "With
+ * i + r we denote a spin which has a spacial distance r from spin i" -- reading C-S8v: r is
+ * any lattice vector (dx, dy, dz), periodic; the axis values above are the special case
+ * the paper prefers for its fits, the full set is its "all r >= 3" reference (:112) and the
+ * merged points of Fig. 2.
+ *   B_b(r) = sum_i q_i q_{i+r},  q_i = S_i^(a) S_i^(b).
+ * ---------------------------------------------------------------------------------- */
+int oracle_c4_vector(const oracle_sim *s, int dx, int dy, int dz, int64_t B[32])
+{
+    if (s->n_replicas != 2) return 1;
+    const int L = s->L;
+#pragma omp parallel for schedule(static)
+    for (int b = 0; b < 32; ++b) {
+        const int8_t *Sa = s->S + (int64_t)b * s->N;
+        const int8_t *Sb = s->S + (int64_t)(b + 32) * s->N;
+        int64_t acc = 0;
+        for (int z = 0; z < L; ++z)
+            for (int y = 0; y < L; ++y)
+                for (int x = 0; x < L; ++x) {
+                    int64_t i = site_of(L, x, y, z);
+                    int64_t j = site_of(L, wrap(x + dx, L), wrap(y + dy, L), wrap(z + dz, L));
+                    acc += (Sa[i] * Sb[i]) * (Sa[j] * Sb[j]);
+                }
+        B[b] = acc;
+    }
+    return 0;
+}
+
+/* Shell sums: every vector with |dx|, |dy|, |dz| <= r_max, collected by squared length
+ * d2 = dx^2 + dy^2 + dz^2 = 0 .. 3 r_max^2:
+ *   S[d2*32 + b] = sum_{|r|^2 = d2} B_b(r),   mult[d2] = number of those vectors
+ * so that C_4(|r| = sqrt(d2)) = S / (mult N) is the average over all directions (Fig. 2).
+ * No symmetry is used: r and -r are both visited.  r_max = L/2 visits +L/2 and -L/2 (the
+ * same displacement on the torus) as two vectors; the average is unaffected. */
+int oracle_c4_shells(const oracle_sim *s, int r_max, int64_t *S, int64_t *mult)
+{
+    if (s->n_replicas != 2 || r_max < 0 || r_max > s->L / 2) return 1;
+    const int n_bins = 3 * r_max * r_max + 1;
+    memset(S, 0, sizeof(int64_t) * 32 * (size_t)n_bins);
+    memset(mult, 0, sizeof(int64_t) * (size_t)n_bins);
+    for (int dz = -r_max; dz <= r_max; ++dz)
+        for (int dy = -r_max; dy <= r_max; ++dy)
+            for (int dx = -r_max; dx <= r_max; ++dx) {
+                int64_t B[32];
+                if (oracle_c4_vector(s, dx, dy, dz, B)) return 1;
+                int d2 = dx * dx + dy * dy + dz * dz;
+                for (int b = 0; b < 32; ++b) S[(int64_t)d2 * 32 + b] += B[b];
+                mult[d2] += 1;
+            }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------
  * Canonical packed I/O (C-A2): word[site] bit b = 1 <-> S_b = -1;
  * bond word[d*N + site] bit b = 1 <-> J_b = -1.  This is the exchange format of the
  * library boundary (include/ea.h), written out here independently.

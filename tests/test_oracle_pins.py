@@ -518,6 +518,126 @@ def test_P11_identical_replicas_give_full_correlation():
 
 
 # ----------------------------------------------------------------------------------------
+# P14  full-vector C_4 (Eq. 3 with r a lattice vector, reading C-S8v)
+# ----------------------------------------------------------------------------------------
+def _pack_replica_q(q):
+    """spin words whose replica overlap field is q (+-1 array [N]) in every disorder lane: replica (a) all up,
+    replica (b) = q."""
+    hi = np.where(q < 0, np.uint64(0xFFFFFFFF00000000), np.uint64(0)).astype(np.uint64)
+    return hi
+
+
+def test_P14_vector_c4_against_the_3d_fft_and_its_symmetries():
+    L, R = 6, 3
+    o = Oracle(L, 0.5, 1.2, 2, seed=wl.seed_for(2, 5))
+    o.sweep(4)
+    S = unpack(o.get_spins())
+    q3 = (S[:32] * S[32:]).reshape(32, L, L, L).astype(np.float64)         # [b][z][y][x]
+    F = np.fft.fftn(q3, axes=(1, 2, 3))
+    corr = np.rint(np.fft.ifftn(F * np.conj(F), axes=(1, 2, 3)).real).astype(np.int64)  # [b][dz][dy][dx] circular
+    for dz in range(-R, R + 1):
+        for dy in range(-R, R + 1):
+            for dx in range(-R, R + 1):
+                B = o.c4_vector(dx, dy, dz)
+                assert (B == corr[:, dz % L, dy % L, dx % L]).all(), (dx, dy, dz)  # library routine (Wiener-Khinchin)
+                assert (B == o.c4_vector(-dx, -dy, -dz)).all()                      # B(r) = B(-r)
+    assert (o.c4_vector(0, 0, 0) == o.N).all()
+    for d, e in enumerate(((1, 0, 0), (0, 1, 0), (0, 0, 1))):
+        for r in range(R + 1):
+            assert (o.c4_vector(r * e[0], r * e[1], r * e[2]) == o.c4_one(d, r)).all()  # the axis special case
+    total = sum(o.c4_vector(dx, dy, dz) for dz in range(L) for dy in range(L) for dx in range(L))
+    assert (total == o.overlap() ** 2).all()                               # sum over the torus = (sum_i q_i)^2
+
+
+def test_P14_vector_c4_on_hand_made_overlap_fields():
+    """Anisotropic fields whose correlation is known in closed form: a transposed or mis-signed displacement
+    component, or a wrong wrap, changes the value."""
+    L = 6
+    N = L ** 3
+    x, y, z = np.meshgrid(np.arange(L), np.arange(L), np.arange(L), indexing="ij")
+    site = (x + L * (y + L * z)).ravel()
+    o = Oracle(L, 0.5, 0.8, 2, seed=1)
+    for name, field, expect in (
+            ("stripes along x", (-1) ** x, lambda dx, dy, dz: N * (-1) ** dx),
+            ("period-3 along y", np.where(y % 3 == 0, -1, 1), lambda dx, dy, dz: N if dy % 3 == 0 else -N // 3),
+            ("planes z<2", np.where(z < 2, -1, 1), lambda dx, dy, dz: N - 4 * L * L * min(abs(dz) % L, L - abs(dz) % L, 2)),
+    ):
+        q = np.empty(N, dtype=np.int64)
+        q[site] = np.asarray(field).ravel()
+        o.set_spins(_pack_replica_q(q))
+        for (dx, dy, dz) in ((1, 0, 0), (0, 1, 0), (0, 0, 1), (2, 1, 0), (-1, 2, 3), (3, -2, 1), (0, 3, -2), (1, 1, 1)):
+            assert (o.c4_vector(dx, dy, dz) == expect(dx, dy, dz)).all(), (name, dx, dy, dz)
+    q = np.ones(N, dtype=np.int64)
+    q[4 + L * (1 + L * 3)] = -1                                                # one defect: two terms change sign
+    o.set_spins(_pack_replica_q(q))
+    assert (o.c4_vector(2, -1, 3) == N - 4).all() and (o.c4_vector(0, 0, 0) == N).all()
+
+
+def test_P14_shell_sums_and_multiplicities():
+    L, R = 8, 3
+    o = Oracle(L, 0.6, 1.0, 2, seed=wl.seed_for(2, 6))
+    o.sweep(3)
+    S, mult = o.c4_shells(R)
+    assert S.shape == (3 * R * R + 1, 32)
+    count = {}
+    for dz in range(-R, R + 1):
+        for dy in range(-R, R + 1):
+            for dx in range(-R, R + 1):
+                count[dx * dx + dy * dy + dz * dz] = count.get(dx * dx + dy * dy + dz * dz, 0) + 1
+    assert [int(m) for m in mult] == [count.get(d2, 0) for d2 in range(3 * R * R + 1)]
+    assert [int(m) for m in mult[:7]] == [1, 6, 12, 8, 6, 24, 24]          # r^2 = 0..6: the cubic-lattice shells
+    assert int(mult[7]) == 0 and (S[7] == 0).all()                         # 7 is not a sum of three squares
+    assert (S[0] == o.N).all()
+    B = o.c4(R)
+    assert (S[1] == 2 * (B[0][1] + B[1][1] + B[2][1])).all()               # shell 1 = the six axis neighbours
+    assert (S[3] == sum(o.c4_vector(a, b, c) for a in (-1, 1) for b in (-1, 1) for c in (-1, 1))).all()
+    assert int(mult.sum()) == (2 * R + 1) ** 3
+    full, _ = o.c4_shells(L // 2)                                          # +-L/2 are visited as two vectors
+    assert (full[3 * (L // 2) ** 2] == 8 * o.c4_vector(L // 2, L // 2, L // 2)).all()
+
+
+# ----------------------------------------------------------------------------------------
+# P15  integral estimator of the coherence length (Eq. 5-6; reading C-S12)
+# ----------------------------------------------------------------------------------------
+def test_P15_c4_curve_is_mean_and_standard_error_over_the_disorder_samples():
+    rng = np.random.default_rng(3)
+    N, R = 512, 2
+    mult = np.array([1, 6, 12, 8, 6, 24, 24, 0, 12, 30, 24, 24, 8], dtype=np.int64)
+    S = rng.integers(-50, 400, size=(13, 32)) * mult[:, None]
+    r, c, e = oracle.c4_curve(S, mult, N, R)
+    d2s = [d2 for d2 in range(13) if mult[d2] and d2 <= R * R]
+    assert np.allclose(r, np.sqrt(d2s), rtol=0, atol=1e-15)
+    per = np.array([S[d2] / (mult[d2] * N) for d2 in d2s])
+    assert np.allclose(c, per.mean(axis=1), rtol=1e-14)
+    assert np.allclose(e, per.std(axis=1, ddof=1) / math.sqrt(32), rtol=1e-12)   # library routine
+
+
+def test_P15_integral_estimator_closed_forms_and_cut_off():
+    R = 8.0
+    r = np.linspace(0.0, R, 9)
+    c = 1.0 - r / R                                                        # linear: trapezoid is exact for k = 0
+    I0, I1, xi, r_cut = oracle.integral_estimator(r, c, np.zeros_like(r), 0)
+    assert abs(I0 - R / 2) < 1e-14 and r_cut == R
+    assert abs(I1 - (R * R / 6 - 1.0 / 6)) < 1e-12                         # trapezoid of r(1 - r/R) with h = 1: exact - h^2 R/(6 R)... = R^2/6 - 1/6
+    assert abs(xi - I1 / I0) < 1e-15
+    xi0 = 2.5
+    r = np.linspace(0.0, 60.0, 6001)                                       # fine grid: trapezoid -> the integral
+    c = np.exp(-r / xi0)
+    I1, I2, xi1, _ = oracle.integral_estimator(r, c, np.zeros_like(r), 1)
+    assert abs(I1 - xi0 ** 2) < 1e-4 and abs(I2 - 2 * xi0 ** 3) < 1e-3 and abs(xi1 - 2 * xi0) < 1e-4  # int r^k e^{-r/xi} = k! xi^{k+1}
+    assert np.isclose(I1, np.trapezoid(r * c, r), rtol=1e-12)              # library routine on the same grid
+    e = np.full_like(r, 1e-3)                                              # 3 e = 3e-3 is crossed at r = xi0 ln(1/3e-3) = 14.52
+    I1c, I2c, _, r_cut = oracle.integral_estimator(r, c, e, 1)
+    j = int(np.argmax(c < 3e-3))
+    assert r_cut == r[j - 1] and abs(r_cut - xi0 * math.log(1 / 3e-3)) < 0.02
+    assert np.isclose(I1c, np.trapezoid((r * c)[:j], r[:j]), rtol=1e-12)
+    assert np.isclose(I2c, np.trapezoid((r * r * c)[:j], r[:j]), rtol=1e-12)
+    c2 = c.copy()
+    c2[5] = -1.0                                                           # a dip below 3 e ends the integral there, even if C_4 recovers
+    assert oracle.integral_estimator(r, c2, e, 1)[3] == r[4]
+
+
+# ----------------------------------------------------------------------------------------
 # P12  initial state
 # ----------------------------------------------------------------------------------------
 def test_P12_initial_state_statistics_and_replica_structure():
