@@ -111,6 +111,28 @@ ea_status ea_autocorr(ea_sim *sim, int slot, int64_t *A, double *C);
  * c4_avg[r] = sum_d sum_b B / (3*32*N) or NULL; q may be NULL.  0 <= r_max <= L/2.
  * EA_ERR_STATE on a 1-replica sim. */
 ea_status ea_c4(ea_sim *sim, int r_max, int64_t *B, int64_t *q, double *c4_avg);
+/* Four-point correlation for arbitrary lattice vectors (Eq. 3, with "i + r" read as any lattice
+ * vector, periodic -- reading C-S8v; the paper's "all r >= 3" reference set, and Fig. 2):
+ *   B[v*32 + b] = sum_i q_i q_{i + r_v},  r_v = (dxyz[3v], dxyz[3v+1], dxyz[3v+2]), any integers.
+ * host arrays: dxyz 3 n_vec int32, B 32 n_vec int64.  EA_ERR_STATE on a 1-replica sim; EA_ERR_INVALID unless
+ * L <= 32 or L in {64, 128}. */
+ea_status ea_c4_vectors(ea_sim *sim, int64_t n_vec, const int32_t *dxyz, int64_t *B);
+/* Shell sums over the cube |dx|, |dy|, |dz| <= r_max (0 <= r_max <= L/2), by squared length d2 = 0 .. 3 r_max^2:
+ *   S[d2*32 + b] = sum_{|r|^2 = d2} B_b(r),  mult[d2] = number of those vectors (0 for an empty shell),
+ * so C_4(|r| = sqrt(d2)) = S / (mult N).  r and -r are both counted; with r_max = L/2 the components +L/2 and
+ * -L/2 (one displacement on the torus) count as two vectors.  host arrays of (3 r_max^2 + 1) * 32 and 3 r_max^2 + 1. */
+ea_status ea_c4_shells(ea_sim *sim, int r_max, int64_t *S, int64_t *mult);
+/* Host arithmetic in double (no device work), the post-processing of PAPER.md:116 -- reading C-S12:
+ * ea_c4_curve: shell sums -> points with mult > 0 and d2 <= r_lim^2, ascending: r = sqrt(d2), c = mean over the
+ *   n_samples disorder samples of S/(mult N), e = its standard error sqrt(sum (c_b - c)^2 / (n (n-1))).
+ *   r, c, e: host arrays of n_bins; *n_pts = points written.
+ * ea_integral_estimator (Eq. 5-6): with j* the first j >= 1 where c_j < 3 e_j (the paper's cut-off,
+ *   :116; all points if none), I_k = sum_{j < j*-1} (r_j^k c_j + r_{j+1}^k c_{j+1}) (r_{j+1} - r_j) / 2 (trapezoid),
+ *   out = { I_k, I_{k+1}, xi_k = I_{k+1} / I_k, r_{j*-1} }.  The paper adds the tail of its fitted form (4) beyond
+ *   the cut-off; fits are out of scope and no tail is added. */
+ea_status ea_c4_curve(const int64_t *S, const int64_t *mult, int n_bins, int n_samples, int64_t N, int r_lim,
+                      int *n_pts, double *r, double *c, double *e);
+ea_status ea_integral_estimator(int n, const double *r, const double *c, const double *e, int k, double out[4]);
 /* E[b] = -sum_<ij> J_ij S_i S_j over the 3N bonds (Eq. 1); host array of 64. */
 ea_status ea_energy(ea_sim *sim, int64_t *E);
 /* M[b] = sum_i S_i,b (C-S14); host array of 64. */

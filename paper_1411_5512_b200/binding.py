@@ -51,6 +51,10 @@ SIGNATURES = {
     "ea_snapshot": (_i, [_vp, _i]),
     "ea_autocorr": (_i, [_vp, _i, _vp, _vp]),
     "ea_c4": (_i, [_vp, _i, _vp, _vp, _vp]),
+    "ea_c4_vectors": (_i, [_vp, C.c_int64, _vp, _vp]),
+    "ea_c4_shells": (_i, [_vp, _i, _vp, _vp]),
+    "ea_c4_curve": (_i, [_vp, _vp, _i, _i, C.c_int64, _i, C.POINTER(_i), _vp, _vp, _vp]),
+    "ea_integral_estimator": (_i, [_i, _vp, _vp, _vp, _i, _vp]),
     "ea_energy": (_i, [_vp, _vp]),
     "ea_magnetisation": (_i, [_vp, _vp]),
     "ea_get_spins": (_i, [_vp, _vp]),
@@ -204,6 +208,21 @@ class Sim:
         out = (B,) + ((q,) if with_q else ()) + ((avg,) if with_avg else ())
         return out if len(out) > 1 else B
 
+    def c4_vectors(self, vectors):
+        """B[v, b] = sum_i q_i q_{i + r_v} for lattice vectors r_v = vectors[v] = (dx, dy, dz)."""
+        v = np.ascontiguousarray(vectors, dtype=np.int32).reshape(-1, 3)
+        B = np.zeros((v.shape[0], 32), dtype=np.int64)
+        self._ck(lib().ea_c4_vectors(self._h, v.shape[0], _ptr(v), _ptr(B)))
+        return B
+
+    def c4_shells(self, r_max):
+        """(S, mult): shell sums of B over the cube |component| <= r_max by squared length d2 = 0..3 r_max^2."""
+        n_bins = 3 * r_max * r_max + 1
+        S = np.zeros((n_bins, 32), dtype=np.int64)
+        mult = np.zeros(n_bins, dtype=np.int64)
+        self._ck(lib().ea_c4_shells(self._h, int(r_max), _ptr(S), _ptr(mult)))
+        return S, mult
+
     def energy(self):
         E = np.zeros(LANES, dtype=np.int64)
         self._ck(lib().ea_energy(self._h, _ptr(E)))
@@ -241,6 +260,29 @@ class Sim:
         w = np.zeros(self.N, dtype=np.uint64)
         self._ck(lib().ea_get_snapshot(self._h, int(slot), _ptr(w)))
         return w
+
+
+def c4_curve(S, mult, N, r_lim):
+    """Shell sums -> (r, c, e): radius, sample-mean C_4 and its standard error (host arithmetic in the library)."""
+    S = np.ascontiguousarray(S, dtype=np.int64)
+    mult = np.ascontiguousarray(mult, dtype=np.int64)
+    n_bins, n_samples = S.shape
+    r, c, e = (np.zeros(n_bins, dtype=np.float64) for _ in range(3))
+    n = C.c_int(0)
+    st = lib().ea_c4_curve(_ptr(S), _ptr(mult), n_bins, n_samples, int(N), int(r_lim), C.byref(n), _ptr(r), _ptr(c), _ptr(e))
+    if st != 0:
+        raise EAError(st, "ea_c4_curve: invalid argument")
+    return r[:n.value].copy(), c[:n.value].copy(), e[:n.value].copy()
+
+
+def integral_estimator(r, c, e, k):
+    """(I_k, I_{k+1}, xi_k, r_cut) of Eq. 5-6 with the 3-sigma cut-off of PAPER.md:116."""
+    r, c, e = (np.ascontiguousarray(a, dtype=np.float64) for a in (r, c, e))
+    out = np.zeros(4, dtype=np.float64)
+    st = lib().ea_integral_estimator(len(r), _ptr(r), _ptr(c), _ptr(e), int(k), _ptr(out))
+    if st != 0:
+        raise EAError(st, "ea_integral_estimator: invalid argument")
+    return tuple(float(x) for x in out)
 
 
 def philox_selftest(ctr, key):

@@ -503,6 +503,95 @@ ea_status ea_c4(ea_sim *sim, int r_max, int64_t *B, int64_t *q, double *c4_avg)
     return EA_OK;
 }
 
+ea_status ea_c4_vectors(ea_sim *sim, int64_t n_vec, const int32_t *dxyz, int64_t *B)
+{
+    if (!sim || n_vec < 0 || (n_vec && (!dxyz || !B))) return EA_ERR_INVALID;
+    if (sim->n_replicas != 2) EA_FAIL(sim, EA_ERR_STATE, "ea_c4_vectors needs a 2-replica sim");
+    if (!c4_vectors_supported(sim->lat.L)) EA_FAIL(sim, EA_ERR_INVALID, "ea_c4_vectors: L must be <= 32, 64 or 128");
+    DeviceGuard g(sim->device);
+    std::vector<unsigned long long> cnt((size_t)n_vec * 32);
+    EA_CUDA(sim, c4_vector_counts(sim, (size_t)n_vec, dxyz, cnt.data()));
+    EA_SYNC(sim);
+    for (size_t k = 0; k < cnt.size(); ++k) B[k] = sim->N - 2 * (int64_t)cnt[k];
+    return EA_OK;
+}
+
+ea_status ea_c4_shells(ea_sim *sim, int r_max, int64_t *S, int64_t *mult)
+{
+    if (!sim || !S || !mult) return EA_ERR_INVALID;
+    if (sim->n_replicas != 2) EA_FAIL(sim, EA_ERR_STATE, "ea_c4_shells needs a 2-replica sim");
+    if (r_max < 0 || r_max > sim->lat.L / 2) EA_FAIL(sim, EA_ERR_INVALID, "r_max %d outside [0, L/2]", r_max);
+    if (!c4_vectors_supported(sim->lat.L)) EA_FAIL(sim, EA_ERR_INVALID, "ea_c4_shells: L must be <= 32, 64 or 128");
+    // B(r) = B(-r): the device visits one vector of every +-r pair (the half space dz > 0, or dz = 0 and dy > 0,
+    // or dz = dy = 0 and dx > 0) and the shell receives it twice; r = 0 is B = N exactly
+    std::vector<int32_t> vec;
+    for (int dz = 0; dz <= r_max; ++dz)
+        for (int dy = (dz ? -r_max : 0); dy <= r_max; ++dy)
+            for (int dx = ((dz || dy) ? -r_max : 1); dx <= r_max; ++dx) {
+                vec.push_back(dx); vec.push_back(dy); vec.push_back(dz);
+            }
+    const size_t n = vec.size() / 3, n_bins = (size_t)3 * r_max * r_max + 1;
+    std::vector<unsigned long long> cnt(n * 32);
+    {
+        DeviceGuard g(sim->device);
+        EA_CUDA(sim, c4_vector_counts(sim, n, vec.data(), cnt.data()));
+        EA_SYNC(sim);
+    }
+    for (size_t k = 0; k < n_bins * 32; ++k) S[k] = 0;
+    for (size_t k = 0; k < n_bins; ++k) mult[k] = 0;
+    for (int b = 0; b < 32; ++b) S[b] = sim->N;
+    mult[0] = 1;
+    for (size_t v = 0; v < n; ++v) {
+        const int64_t d2 = (int64_t)vec[3 * v] * vec[3 * v] + (int64_t)vec[3 * v + 1] * vec[3 * v + 1] + (int64_t)vec[3 * v + 2] * vec[3 * v + 2];
+        for (int b = 0; b < 32; ++b) S[d2 * 32 + b] += 2 * (sim->N - 2 * (int64_t)cnt[v * 32 + b]);
+        mult[d2] += 2;
+    }
+    return EA_OK;
+}
+
+ea_status ea_c4_curve(const int64_t *S, const int64_t *mult, int n_bins, int n_samples, int64_t N, int r_lim,
+                      int *n_pts, double *r, double *c, double *e)
+{
+    if (!S || !mult || !n_pts || !r || !c || !e || n_bins < 1 || n_samples < 2 || N < 1 || r_lim < 0) return EA_ERR_INVALID;
+    int n = 0;
+    for (int d2 = 0; d2 < n_bins; ++d2) {
+        if (mult[d2] == 0 || (int64_t)d2 > (int64_t)r_lim * r_lim) continue;
+        const double denom = (double)mult[d2] * (double)N;
+        double sum = 0.0;
+        for (int b = 0; b < n_samples; ++b) sum += (double)S[(size_t)d2 * n_samples + b] / denom;
+        const double mean = sum / n_samples;
+        double ss = 0.0;
+        for (int b = 0; b < n_samples; ++b) {
+            const double d = (double)S[(size_t)d2 * n_samples + b] / denom - mean;
+            ss += d * d;
+        }
+        r[n] = sqrt((double)d2);
+        c[n] = mean;
+        e[n] = sqrt(ss / ((double)n_samples * (double)(n_samples - 1)));
+        ++n;
+    }
+    *n_pts = n;
+    return EA_OK;
+}
+
+ea_status ea_integral_estimator(int n, const double *r, const double *c, const double *e, int k, double out[4])
+{
+    if (n < 1 || !r || !c || !e || !out || k < 0) return EA_ERR_INVALID;
+    int n_use = n;
+    for (int j = 1; j < n; ++j)
+        if (c[j] < 3.0 * e[j]) { n_use = j; break; }
+    for (int m = 0; m < 2; ++m) {
+        const int kk = k + m;
+        double acc = 0.0;
+        for (int j = 0; j + 1 < n_use; ++j)
+            acc += 0.5 * (pow(r[j], kk) * c[j] + pow(r[j + 1], kk) * c[j + 1]) * (r[j + 1] - r[j]);
+        out[m] = acc;
+    }
+    out[2] = out[0] != 0.0 ? out[1] / out[0] : NAN;
+    out[3] = r[n_use - 1];
+    return EA_OK;
+}
+
 // ---- canonical packed I/O ---------------------------------------------------------------------------
 
 ea_status ea_get_spins(ea_sim *sim, uint64_t *host)

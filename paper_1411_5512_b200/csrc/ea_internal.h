@@ -89,6 +89,10 @@ cudaError_t launch_count_spins(ea_sim *s, const uint64_t *d_other /* nullable: X
 cudaError_t launch_count_energy(ea_sim *s);
 cudaError_t launch_count_c4(ea_sim *s, int r_max); // counters[(d*(r_max+1)+r)*32+b], then [3*(r_max+1)*32 + b] = overlap
 
+// full-vector C_4 (ea_c4_vectors.cu): per-sample counts of q_i != q_{i+r} for n lattice vectors; host result
+bool c4_vectors_supported(int L);
+cudaError_t c4_vector_counts(ea_sim *s, size_t n, const int32_t *vec, unsigned long long *counts);
+
 cudaError_t philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 
 } // namespace ea

@@ -82,3 +82,36 @@ def test_product_never_imports_the_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src, f
                 assert "ea_oracle" not in src, f
+
+
+def test_host_side_c4_curve_and_integral_estimator_match_the_oracle():
+    """ea_c4_curve / ea_integral_estimator do no device work (double arithmetic on the host, Eq. 5-6 and the
+    procedure of PAPER.md:116): compared here, without a GPU, with the oracle's fp64 restatement; 1e-12 relative."""
+    import numpy as np
+    import oracle
+    from paper_1411_5512_b200 import binding
+    rng = np.random.default_rng(11)
+    R, N = 6, 4096
+    n_bins = 3 * R * R + 1
+    mult = np.zeros(n_bins, dtype=np.int64)
+    for dz in range(-R, R + 1):
+        for dy in range(-R, R + 1):
+            for dx in range(-R, R + 1):
+                mult[dx * dx + dy * dy + dz * dz] += 1
+    r_all = np.sqrt(np.arange(n_bins))
+    base = N * np.exp(-r_all / 1.7)
+    S = np.rint((base[:, None] + rng.normal(0, 600.0, size=(n_bins, 32))) * mult[:, None]).astype(np.int64)
+    for r_lim in (R, 3):
+        got = binding.c4_curve(S, mult, N, r_lim)
+        want = oracle.c4_curve(S, mult, N, r_lim)
+        assert len(got[0]) == len(want[0]) > 3
+        for a, b in zip(got, want):
+            np.testing.assert_allclose(a, b, rtol=1e-12, atol=0)
+    r, c, e = oracle.c4_curve(S, mult, N, R)
+    for k in (0, 1, 2):
+        got = binding.integral_estimator(r, c, e, k)
+        want = oracle.integral_estimator(r, c, e, k)
+        np.testing.assert_allclose(got, want, rtol=1e-12, atol=0)
+    assert binding.integral_estimator(r, c, e, 1)[3] < R          # the noisy tail is cut off
+    got = binding.integral_estimator(r, np.abs(c) + 1e-9, np.zeros_like(e), 1)    # nothing below 3 e: no cut-off
+    assert got[3] == r[-1]

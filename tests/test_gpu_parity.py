@@ -399,3 +399,82 @@ def test_caller_stream_and_library_workspace():
     b = binding.Sim(8, 0.5, 0.8, n_replicas=2, seed=3, torch_workspace=False)
     a.sweep(70); b.sweep(70)
     assert np.array_equal(a.get_spins(), b.get_spins())
+
+
+# ----------------------------------------------------------------------------------------------------
+# NEXT-1: C_4 for arbitrary lattice vectors, shell sums, integral estimator
+# ----------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L,R,sweeps", [(2, 1, 3), (4, 2, 3), (6, 3, 5), (8, 4, 20), (12, 3, 5), (16, 5, 10), (32, 4, 6),
+                                        (64, 3, 2)])
+def test_c4_shells_match_the_oracle(L, R, sweeps):
+    """Every shell sum and multiplicity over the cube |component| <= R: the device visits one vector of each +-r
+    pair, the oracle all of them.  L = 2..32: one (masked) word per x-row; L = 64: two words."""
+    g, o = make_pair(L, 0.6, 1.0, 2, wl.seed_for(5, L), n_slots=0)
+    g.sweep(sweeps)
+    o.sweep(sweeps)
+    S, mult = g.c4_shells(R)
+    So, mo = o.c4_shells(R)
+    assert np.array_equal(mult, mo)
+    assert np.array_equal(S, So)
+    r, c, e = binding.c4_curve(S, mult, g.N, R)
+    ro, co, eo = oracle.c4_curve(So, mo, o.N, R)
+    for a, b in zip((r, c, e), (ro, co, eo)):
+        np.testing.assert_allclose(a, b, rtol=1e-12, atol=0)
+    np.testing.assert_allclose(binding.integral_estimator(r, c, e, 1), oracle.integral_estimator(ro, co, eo, 1), rtol=1e-12)
+
+
+@pytest.mark.parametrize("L", [8, 16, 32, 64, 128])
+def test_c4_vectors_sampled_against_the_oracle(L):
+    """Individual vectors, including negative, wrapping (|component| > L/2), repeated and word-crossing dx."""
+    g, o = make_pair(L, 0.5, 0.8, 2, wl.seed_for(5, L + 1), n_slots=0)
+    n = 3 if L == 128 else 6
+    g.sweep(n)
+    o.sweep(n)
+    rng = np.random.default_rng(L)
+    vecs = [(0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, 0, -1), (L // 2, L // 2, L // 2), (L - 1, 1 - L, L),
+            (31, 2, 1), (32, 0, 3), (33, -4, 0), (L + 5, 7, -9), (1, 0, 0)]
+    vecs += [tuple(int(x) for x in rng.integers(-L, L + 1, size=3)) for _ in range(6 if L == 128 else 20)]
+    B = g.c4_vectors(vecs)
+    for v, row in zip(vecs, B):
+        assert np.array_equal(row, o.c4_vector(*v)), v
+    for d, e in enumerate(((1, 0, 0), (0, 1, 0), (0, 0, 1))):           # the axis path (ea_c4) is the special case
+        axis = g.c4(min(4, L // 2))
+        assert np.array_equal(g.c4_vectors([tuple(3 * x for x in e)])[0], axis[d][3] if L >= 6 else axis[d][3 % L])
+
+
+def test_c4_shells_full_size_properties_and_sampled_shells():
+    """L = 128, bench configuration, R = 6 (1099 vectors visited): properties that hold at any size, plus the
+    shells the oracle can afford (d2 = 1, 2, 3: 26 vectors)."""
+    c = wl.CONFIGS["cfg4"]
+    g, o = make_pair(c.L, c.p, c.T, c.n_replicas, c.seed, n_slots=0)
+    g.sweep(4)
+    o.sweep(4)
+    R = 6
+    S, mult = g.c4_shells(R)
+    assert int(mult.sum()) == (2 * R + 1) ** 3 and (S[0] == g.N).all()
+    axis = g.c4(R)
+    for r in range(1, R + 1):                                             # pure-axis shells where no other vector has that length
+        if mult[r * r] == 6:
+            assert np.array_equal(S[r * r], 2 * axis[:, r, :].sum(axis=0))
+    assert (np.abs(S) <= mult[:, None] * g.N).all()
+    for d2 in (1, 2, 3):
+        want = np.zeros(32, dtype=np.int64)
+        for dz in (-1, 0, 1):
+            for dy in (-1, 0, 1):
+                for dx in (-1, 0, 1):
+                    if dx * dx + dy * dy + dz * dz == d2:
+                        want += o.c4_vector(dx, dy, dz)
+        assert np.array_equal(S[d2], want), d2
+
+
+def test_c4_vectors_argument_errors():
+    g = binding.Sim(8, 0.5, 0.8, n_replicas=1)
+    with pytest.raises(binding.EAError):
+        g.c4_vectors([(1, 0, 0)])
+    g2 = binding.Sim(8, 0.5, 0.8, n_replicas=2)
+    with pytest.raises(binding.EAError):
+        g2.c4_shells(5)
+    assert g2.c4_vectors(np.zeros((0, 3), dtype=np.int32)).shape == (0, 32)
+    g3 = binding.Sim(48, 0.5, 0.8, n_replicas=2, n_slots=0)
+    with pytest.raises(binding.EAError):
+        g3.c4_shells(2)
