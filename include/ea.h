@@ -85,8 +85,8 @@ ea_status ea_create_ex(const ea_params *prm, ea_sim **out);
 ea_status ea_destroy(ea_sim *sim);
 
 /* n full sweeps: each = all sites with (x+y+z)&1 == 0, then all with parity 1 (C-S2),
- * single-spin-flip Metropolis with Eq. 9 (C-A4), one Philox4x32-10 block per (site, sweep)
- * (C-A6, C-A7).  Asynchronous; t += n. */
+ * single-spin-flip Metropolis with Eq. 9 (C-A4), one Philox4x32-10 block per sweep and pair of
+ * x-adjacent same-colour sites, all four output words used (C-A6, C-A7).  Asynchronous; t += n. */
 ea_status ea_sweep(ea_sim *sim, uint64_t n);
 /* One colour only (parity 0 or 1) of sweep t; does not advance t.  For tests of the half-step. */
 ea_status ea_half_sweep(ea_sim *sim, int parity);

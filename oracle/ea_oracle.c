@@ -259,8 +259,12 @@ const int64_t *oracle_dE_accum(const oracle_sim *s) { return s->dE_accum; }
 
 /* ------------------------------------------------------------------------------------
  * One half-sweep: every site of one colour gets one Metropolis trial.
- * Random numbers (C-A6, C-A7): one Philox block per (site, sweep), counter
- * (site, t lo, t hi, tag = parity); out[0] drives samples 0..31, out[1] samples 32..63.
+ * Random numbers (C-A6, C-A7): the same-colour sites of one x-row are x = s, s+2, s+4, ...;
+ * number them j = x >> 1 = 0 .. L/2 - 1.  Sites j (even) and j + 1 form a pair and share ONE
+ * Philox block per sweep, counter (site index of the pair's first site, t lo, t hi,
+ * tag = parity): the first site takes out[0] (samples 0..31) and out[1] (samples 32..63),
+ * the second takes out[2] and out[3].  (L/2 odd: the last site of a row is a pair of its
+ * own; L = 2: every site is.)  All four words of a block are used, none twice.
  * "It is customary to save computational effort by using only one random number for
  * multiple samples"; the two replicas never share one.
  * Same-colour sites are never neighbours (L even), so the visiting order is immaterial;
@@ -296,10 +300,13 @@ void oracle_half_sweep(oracle_sim *s, int parity)
     for (int64_t site = 0; site < N; ++site) {
         int x = (int)(site % L), y = (int)((site / L) % L), z = (int)(site / ((int64_t)L * L));
         if (((x + y + z) & 1) != parity) continue;
+        int j = x >> 1;                /* position among the same-colour sites of this x-row */
+        int second = j & 1;            /* second site of its pair?                            */
+        int64_t first_site = site_of(L, x - 2 * second, y, z);
         uint32_t out[4];
-        stream_block(s, (uint32_t)site, (uint32_t)(s->t & 0xffffffffu), (uint32_t)(s->t >> 32), tag, out);
-        s->r_lo[site] = out[0];
-        s->r_hi[site] = out[1];
+        stream_block(s, (uint32_t)first_site, (uint32_t)(s->t & 0xffffffffu), (uint32_t)(s->t >> 32), tag, out);
+        s->r_lo[site] = out[2 * second];
+        s->r_hi[site] = out[2 * second + 1];
     }
 #pragma omp parallel for schedule(static) if (N >= 4096) /* tiny lattices: thread start-up costs more than the work */
     for (int lane = 0; lane < ORACLE_LANES; ++lane) {

@@ -61,18 +61,19 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// The update stream of one half-sweep: counter (site, t lo, t hi, parity), key = seed (C-A6).
-// Only c0 = site varies inside a launch, so everything that depends on (t, parity, seed) alone is
-// folded once per launch into SweepRng (rounds 1-2 collapse to two multiplies); and only out[0]
-// (samples 0..31) and out[1] (samples 32..63) are consumed (C-A7), so round 10 needs one multiply.
-// The result is bit-identical to philox4x32_10(site, t lo, t hi, parity; seed)[0..1].
+// The update stream of one half-sweep (C-A6, C-A7): the same-colour sites of an x-row, j = x >> 1 = compact index
+// xh, pair up (xh even, xh + 1) and share ONE block per sweep: counter (site index of the pair's first site,
+// t lo, t hi, parity), key = seed; the first site takes out[0] (samples 0..31) and out[1] (samples 32..63), the
+// second out[2] and out[3].  Only c0 varies inside a launch, so everything that depends on (t, parity, seed)
+// alone is folded once per launch into SweepRng (rounds 1-2 collapse to two multiplies).
+// The result is bit-identical to philox4x32_10(first site, t lo, t hi, parity; seed).
 struct SweepRng {
     uint32_t x2;     // tag ^ k1[0]
     uint32_t x0;     // lo(M1*t_hi) ^ k0[1]
     uint32_t y2;     // hi(M0*U0) ^ k1[1],  U0 = hi(M1*t_hi) ^ t_lo ^ k0[0]
     uint32_t z2;     // lo(M0*U0) ^ k1[2]
     uint32_t k0[10]; // round keys (only [2..9] used)
-    uint32_t k1[10]; // round keys (only [3..8] used)
+    uint32_t k1[10]; // round keys (only [3..9] used)
 };
 
 __host__ __device__ inline SweepRng make_sweep_rng(uint64_t seed, uint64_t t, uint32_t tag)
@@ -109,11 +110,11 @@ __host__ __device__ inline void sweep_rng_set_time(SweepRng &g, uint64_t t, uint
     g.z2 = (uint32_t)q0 ^ g.k1[2];
 }
 
-__device__ __forceinline__ void sweep_random(const SweepRng &g, uint32_t site, uint32_t &r_lo, uint32_t &r_hi)
+__device__ __forceinline__ uint4 sweep_random4(const SweepRng &g, uint32_t first_site)
 {
     uint32_t h, l, h0, l0, h1, l1;
     // round 1: (site, t_lo, t_hi, tag) -> (U0, U1, n2, n3)
-    mulhilo(PHILOX_M0, site, h, l);
+    mulhilo(PHILOX_M0, first_site, h, l);
     uint32_t n2 = h ^ g.x2, n3 = l;
     // round 2: (U0, U1, n2, n3) -> (m0, m1, m2, V3)
     mulhilo(PHILOX_M1, n2, h, l);
@@ -125,9 +126,9 @@ __device__ __forceinline__ void sweep_random(const SweepRng &g, uint32_t site, u
     c1 = l1;
     c2 = h0 ^ g.z2;
     uint32_t c3 = l0;
-    // rounds 4..9
+    // rounds 4..10
 #pragma unroll
-    for (int r = 3; r < 9; ++r) {
+    for (int r = 3; r < 10; ++r) {
         mulhilo(PHILOX_M0, c0, h0, l0);
         mulhilo(PHILOX_M1, c2, h1, l1);
         c0 = h1 ^ c1 ^ g.k0[r];
@@ -135,10 +136,16 @@ __device__ __forceinline__ void sweep_random(const SweepRng &g, uint32_t site, u
         c2 = h0 ^ c3 ^ g.k1[r];
         c3 = l0;
     }
-    // round 10: only out[0], out[1]
-    mulhilo(PHILOX_M1, c2, h1, l1);
-    r_lo = h1 ^ c1 ^ g.k0[9];
-    r_hi = l1;
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// the two numbers of ONE site: `second` = xh & 1 selects the half of its pair's block (scalar kernel, self-test)
+__device__ __forceinline__ void sweep_random(const SweepRng &g, uint32_t first_site, unsigned second, uint32_t &r_lo,
+                                             uint32_t &r_hi)
+{
+    const uint4 o = sweep_random4(g, first_site);
+    r_lo = second ? o.z : o.x;
+    r_hi = second ? o.w : o.y;
 }
 
 // Acceptance thresholds of Eq. 9 (C-A4) prepared for 32-bit compares:

@@ -101,9 +101,10 @@ __global__ void k_philox_selftest(uint32_t c0, uint32_t c1, uint32_t c2, uint32_
     uint32_t o[4];
     philox4x32_10(c0, c1, c2, c3, k0, k1, o);
     for (int e = 0; e < 4; ++e) out[e] = o[e];
-    // the folded update stream must agree with the block function: out[4..5] = sweep_random of the same counter
+    // the folded update stream must agree with the block function: out[4..7] = sweep_random4 of the same counter
     SweepRng g = make_sweep_rng((uint64_t)k0 | ((uint64_t)k1 << 32), (uint64_t)c1 | ((uint64_t)c2 << 32), c3);
-    sweep_random(g, c0, out[4], out[5]);
+    const uint4 f = sweep_random4(g, c0);
+    out[4] = f.x; out[5] = f.y; out[6] = f.z; out[7] = f.w;
 }
 
 static inline unsigned blocks_for(size_t n, unsigned block) { return (unsigned)((n + block - 1) / block); }
@@ -167,7 +168,7 @@ cudaError_t launch_unpack_bonds(ea_sim *s, int d, uint64_t *d_canon)
 
 cudaError_t philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
 {
-    uint32_t *d = nullptr, h[6];
+    uint32_t *d = nullptr, h[8];
     cudaError_t e = cudaMalloc(&d, sizeof(h));
     if (e != cudaSuccess) return e;
     k_philox_selftest<<<1, 1>>>(ctr[0], ctr[1], ctr[2], ctr[3], key[0], key[1], d);
@@ -176,7 +177,7 @@ cudaError_t philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32
     cudaFree(d);
     if (e != cudaSuccess) return e;
     // the folded stream is only defined for tags 0/1 but the algebra holds for any counter: require agreement
-    if (h[4] != h[0] || h[5] != h[1]) return cudaErrorUnknown;
+    if (h[4] != h[0] || h[5] != h[1] || h[6] != h[2] || h[7] != h[3]) return cudaErrorUnknown;
     for (int i = 0; i < 4; ++i) out[i] = h[i];
     return cudaSuccess;
 }

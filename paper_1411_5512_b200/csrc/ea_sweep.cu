@@ -80,9 +80,9 @@ __global__ void __launch_bounds__(256) k_sweep_scalar(const SweepArgs a)
     const BondT j_xm = __ldg(Jo + jm), j_ym = __ldg(Jo + Nh + iym), j_zm = __ldg(Jo + 2 * Nh + izm);
 
     const SweepRng g = make_sweep_rng(a.seed, sweep_time(a), (uint32_t)a.colour);
-    const uint32_t site = (2 * xh + s) + L * (y + L * z); // canonical site index = Philox counter word 0
-    uint32_t r_lo, r_hi;
-    sweep_random(g, site, r_lo, r_hi);
+    const uint32_t site = (2 * xh + s) + L * (y + L * z); // canonical site index
+    uint32_t r_lo, r_hi;                                   // counter word 0 = the first site of the pair (xh even)
+    sweep_random(g, site - 2 * (xh & 1u), xh & 1u, r_lo, r_hi);
     a.own[i] = metropolis_word<BondT, ALWAYS>(sg, n_xp, n_xm, n_yp, n_ym, n_zp, n_zm, j_xp, j_xm, j_yp, j_ym, j_zp, j_zm,
                                       r_lo, r_hi, a.th);
 }
@@ -142,12 +142,10 @@ __global__ void __launch_bounds__(256) k_sweep_vec2(const SweepArgs a)
 
     const SweepRng g = make_sweep_rng(a.seed, sweep_time(a), (uint32_t)a.colour);
     const uint32_t site0 = (4 * k + s) + L * (y + L * z);
-    uint32_t r0l, r0h, r1l, r1h;
-    sweep_random(g, site0, r0l, r0h);
-    sweep_random(g, site0 + 2, r1l, r1h);
+    const uint4 r = sweep_random4(g, site0); // the thread's two words are one pair (xh = 2k, 2k + 1): one block
     ulonglong2 out;
-    out.x = metropolis_word<BondT, ALWAYS>(sg0, np0, nm0, yp0, ym0, zp0, zm0, jx0, jm0, jy0, by0, jz0, bz0, r0l, r0h, a.th);
-    out.y = metropolis_word<BondT, ALWAYS>(sg1, np1, nm1, yp1, ym1, zp1, zm1, jx1, jm1, jy1, by1, jz1, bz1, r1l, r1h, a.th);
+    out.x = metropolis_word<BondT, ALWAYS>(sg0, np0, nm0, yp0, ym0, zp0, zm0, jx0, jm0, jy0, by0, jz0, bz0, r.x, r.y, a.th);
+    out.y = metropolis_word<BondT, ALWAYS>(sg1, np1, nm1, yp1, ym1, zp1, zm1, jx1, jm1, jy1, by1, jz1, bz1, r.z, r.w, a.th);
     *(ulonglong2 *)(a.own + i0) = out;
 }
 

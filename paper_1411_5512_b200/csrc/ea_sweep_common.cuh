@@ -74,9 +74,7 @@ __device__ __forceinline__ ulonglong2 update_pair(const ulonglong2 own, const ul
                                                   const SweepRng &g, const Thresholds &th, const int lane_m,
                                                   const int lane_p)
 {
-    uint4 r;
-    sweep_random(g, site0, r.x, r.y);
-    sweep_random(g, site0 + 2, r.z, r.w);
+    const uint4 r = sweep_random4(g, site0); // the lane's two words are one pair (xh = 2k, 2k + 1): one block
     return update_pair_r<S, BondT, ALWAYS, RARE>(own, P0, Pm, Pp, Zm, Zp, jx, jy, jz, bx, by, bz, r, th, lane_m, lane_p);
 }
 

@@ -173,16 +173,13 @@ struct ResidentStep {
     int lane_m, lane_p;
 };
 
-// the four random numbers of the lane's two words of a row (d.y = row offset, S = row phase): independent of the
+// the four random numbers of the lane's two words of a row (d.y = row offset, S = row phase; C-A7): independent of the
 // spins, so they are drawn one row ahead and their IMAD.WIDE chain (fma pipe) overlaps the LOP3 logic (alu pipe)
 // of the row before
 __device__ __forceinline__ uint4 row_random(const SweepRng &g, const unsigned k, const unsigned S, const uint4 d)
 {
-    const uint32_t site0 = 4 * k + S + 2 * d.y; // canonical site = x + L (y + L z), L = 2 Lh
-    uint4 r;
-    sweep_random(g, site0, r.x, r.y);
-    sweep_random(g, site0 + 2, r.z, r.w);
-    return r;
+    // canonical site = x + L (y + L z), L = 2 Lh; the lane's two words (xh = 2k, 2k + 1) are one pair: one block
+    return sweep_random4(g, 4 * k + S + 2 * d.y);
 }
 
 // one row of colour c with compile-time phase S; publishes it to global when `publish`

@@ -119,10 +119,13 @@ def test_P3_acceptance_frequency_with_frozen_neighbours():
 
 
 # ----------------------------------------------------------------------------------------
-# stream layout: counters (site, t lo, t hi, tag) and out[0] -> lanes 0..31, out[1] -> 32..63
+# stream layout (C-A6, C-A7): same-colour sites j = x >> 1 of an x-row pair up (j even, j + 1); the pair shares the
+# block at counter (first site, t lo, t hi, tag); first site: out[0] -> lanes 0..31, out[1] -> 32..63; second
+# site: out[2], out[3].  L = 6 has an unpaired last site per row (L/2 odd), L = 2 only single sites.
 # ----------------------------------------------------------------------------------------
-def test_stream_layout_of_update_numbers():
-    L, T, seed = 4, 6.0, 0xABCDEF0123456789
+@pytest.mark.parametrize("L", [2, 4, 6, 8])
+def test_stream_layout_of_update_numbers(L):
+    T, seed = 6.0, 0xABCDEF0123456789
     key = [seed & 0xFFFFFFFF, seed >> 32]
     thr0 = int(oracle.thresholds(T)[0])
     for t in (0, 5, (1 << 32) + 3):
@@ -137,9 +140,11 @@ def test_stream_layout_of_update_numbers():
                 if (x + y + z) & 1 != parity:
                     assert w[site] == 0
                     continue
-                out = oracle.philox4x32_10([site, t & 0xFFFFFFFF, t >> 32, parity], key)
-                lo = 0xFFFFFFFF if int(out[0]) < thr0 else 0
-                hi = 0xFFFFFFFF if int(out[1]) < thr0 else 0
+                second = (x >> 1) & 1
+                first_site = site - 2 * second
+                out = oracle.philox4x32_10([first_site, t & 0xFFFFFFFF, t >> 32, parity], key)
+                lo = 0xFFFFFFFF if int(out[2 * second]) < thr0 else 0
+                hi = 0xFFFFFFFF if int(out[2 * second + 1]) < thr0 else 0
                 assert int(w[site]) == lo | (hi << 32)
 
 
