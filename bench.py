@@ -327,7 +327,38 @@ def run_ours(args, cfg):
         roofline["alu"] = {"achieved": alu_rate / 1e9, "peak": ALU_PEAK_WARP_INST_PER_S / 1e9,
                            "unit": "G warp-inst/s (alu pipe)", "frac": alu_rate / ALU_PEAK_WARP_INST_PER_S,
                            "alu_warp_inst_per_half_sweep": ncu["alu_inst"]}
+    # ---- SURVEY 8(f) rows built so far, timed on the same state (not part of `value`) -----------------------
+    next_rows = None
+    if cfg.n_replicas == 2 and not args.no_next_rows:
+        R = 8
+        sim.c4_shells(2)  # warm-up (first-call allocations)
+        torch.cuda.synchronize()
+        w0 = time.perf_counter()
+        S_sh, mult = sim.c4_shells(R)
+        t_shells = time.perf_counter() - w0
+        r_c, c_c, e_c = binding.c4_curve(S_sh, mult, N, R)
+        xi = binding.integral_estimator(r_c, c_c, e_c, 1)
+        n_vec = ((2 * R + 1) ** 3 - 1) // 2
+        next_rows = {"c4_shells": {"r_max": R, "vectors_visited": n_vec, "ms": 1e3 * t_shells,
+                                   "popc_lane_ops_per_s": n_vec * float(N) / t_shells,
+                                   "popc_peak_per_s": 148 * 16 * 1.965e9,
+                                   "note": "NEXT-1: ea_c4_shells wall time incl. transposition, job upload and D2H; "
+                                           "bound = POPC rate (16 lanes/clk/SM); kernel alone: profiles/"},
+                     "xi_1": {"I_1": xi[0], "I_2": xi[1], "xi_1": xi[2], "r_cut": xi[3], "t_w": int(sim.time)}}
     sim.close()
+    if next_rows is not None and ws == 1:
+        from paper_1411_5512_b200.scan import Scan
+        Ls, Ks, n_sc = 64, 8, 2000
+        sc = Scan([{"L": Ls, "p": 0.6 + 0.01 * k, "T": cfg.T, "seed": seed + 1000 + k} for k in range(Ks)], device=local_rank)
+        sc.sweep(64)
+        sc.synchronize()
+        w0 = time.perf_counter()
+        sc.sweep(n_sc)
+        sc.synchronize()
+        t_sc = time.perf_counter() - w0
+        sc.close()
+        next_rows["scan"] = {"L": Ls, "sims": Ks, "sweeps": n_sc, "ps_per_attempt_aggregate": 1e12 * t_sc / (Ks * n_sc * Ls ** 3 * 64.0),
+                             "note": "NEXT-4 driver: K independent L=64 sims, one stream + CUDA graph each, issued back to back"}
 
     cpu_baseline = None
     if ws == 1 and not args.no_cpu_baseline:
@@ -345,6 +376,7 @@ def run_ours(args, cfg):
         "gpu_launches": int(launches),
         "roofline": roofline,
         "cpu_baseline": cpu_baseline,
+        "next_rows": next_rows,
         "wall_s_timed_loop": wall,
         "paper_context": "paper: ~8 ps per spin flip on a GeForce GTX 570 (PAPER.md:5, :92) -- other hardware, "
                          "context only",
@@ -366,6 +398,7 @@ def main():
     ap.add_argument("--config", default=wl.BENCH_CONFIG, choices=sorted(wl.CONFIGS))
     ap.add_argument("--sweeps-per-step", type=int, default=1000)
     ap.add_argument("--kernel", default="auto")
+    ap.add_argument("--no-next-rows", action="store_true", help="skip the timing of the SURVEY 8(f) rows (c4_shells, scan)")
     ap.add_argument("--flush-mib", type=int, default=256)
     ap.add_argument("--cpu-sweeps", type=int, default=12, help="oracle sweeps timed for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (profiler runs)")

@@ -26,6 +26,9 @@ def lib():
         sig = {
             "oracle_philox4x32_10": (None, [pu32, pu32, pu32]),
             "oracle_thresholds": (None, [dbl, pu64]),
+            "oracle_thresholds_heatbath": (None, [dbl, pu64]),
+            "oracle_accept_heatbath": (i32, [pu64, i32, C.c_uint32]),
+            "oracle_set_dynamics": (i32, [vp, i32]),
             "oracle_bond_threshold": (u64, [dbl]),
             "oracle_accept": (i32, [pu64, i32, C.c_uint32]),
             "oracle_shift": (i64, [i32, i64, i32, i32]),
@@ -85,6 +88,18 @@ def thresholds(T):
     return thr
 
 
+def thresholds_heatbath(T):
+    """thr[n_u] = floor(2^32 / (1 + exp((12 - 4 n_u) / T)) + 0.5), n_u = 0..6 (reading C-HB)."""
+    thr = np.zeros(7, dtype=np.uint64)
+    lib().oracle_thresholds_heatbath(float(T), _p(thr, C.c_uint64))
+    return thr
+
+
+def accept_heatbath(thr, local_sum, r):
+    t = np.ascontiguousarray(thr, dtype=np.uint64)
+    return bool(lib().oracle_accept_heatbath(_p(t, C.c_uint64), int(local_sum), int(r)))
+
+
 def bond_threshold(p):
     return int(lib().oracle_bond_threshold(float(p)))
 
@@ -131,6 +146,12 @@ class Oracle:
 
     def set_temperature(self, T):
         lib().oracle_set_temperature(self._h, float(T))
+
+    def set_dynamics(self, dynamics):
+        """"metropolis" (Eq. 9, the paper's) or "heatbath" (reading C-HB)."""
+        code = {"metropolis": 0, "heatbath": 1}[dynamics]
+        if lib().oracle_set_dynamics(self._h, code):
+            raise ValueError("bad dynamics")
 
     @property
     def thresholds(self):

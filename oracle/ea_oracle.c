@@ -40,6 +40,8 @@ typedef struct oracle_sim {
     uint64_t seed;
     uint64_t t;      /* completed sweeps since the random start           */
     uint64_t thr[3]; /* integer acceptance thresholds for n_u = 0,1,2 (C-A4)            */
+    int dynamics;       /* 0: Metropolis (Eq. 9, the paper's); 1: heat bath (C-HB)          */
+    uint64_t thr_hb[7]; /* heat-bath thresholds for n_u = 0..6 (C-HB)                       */
     int8_t *S;       /* S[lane*N + site]            = +-1                               */
     int8_t *J;       /* J[(lane*3 + d)*N + site]    = +-1, forward bond site->site+e_d  */
     int8_t *snap;    /* n_slots snapshots of S                                           */
@@ -102,6 +104,26 @@ void oracle_thresholds(double T, uint64_t thr[3])
         double prob = exp(-(4.0 * (double)(3 - n_u)) / T);
         thr[n_u] = (uint64_t)floor(4294967296.0 * prob + 0.5);
     }
+}
+
+/* Heat-bath variant (NOT the paper's dynamics, which is Metropolis) -- reading
+ * C-HB: a spin is flipped with probability 1 / (1 + exp(Delta E / T)), Delta E = 2 sum_j J_ij S_i S_j = 12 - 4 n_u,
+ * for every n_u = 0..6 (no "always flip" shortcut; Delta E = 0 gives exactly 1/2 at any T, T = 0 gives 0, 1/2, 1).
+ * thr_hb[n_u] = floor(2^32 P + 0.5), compared with the same 32-bit numbers by the same strict "<". */
+void oracle_thresholds_heatbath(double T, uint64_t thr[7])
+{
+    for (int n_u = 0; n_u < 7; ++n_u) {
+        double dE = 12.0 - 4.0 * (double)n_u;
+        double w = dE == 0.0 ? 1.0 : exp(dE / T); /* 0/0 at T = 0 is the Delta E = 0 case: weight 1 */
+        double prob = 1.0 / (1.0 + w);
+        thr[n_u] = (uint64_t)floor(4294967296.0 * prob + 0.5);
+    }
+}
+
+int oracle_accept_heatbath(const uint64_t thr[7], int local_sum, uint32_t r)
+{
+    int n_u = (6 - local_sum) / 2; /* 0..6 */
+    return (uint64_t)r < thr[n_u];
 }
 
 /* P(J = +1) = p as an integer threshold on a 32-bit uniform (C-A9). */
@@ -213,6 +235,8 @@ oracle_sim *oracle_create(int L, double p, double T, int n_replicas, uint64_t se
     s->L = L; s->N = (int64_t)L * L * L; s->n_replicas = n_replicas;
     s->p = p; s->T = T; s->seed = seed; s->t = 0; s->n_slots = n_slots;
     oracle_thresholds(T, s->thr);
+    s->dynamics = 0;
+    oracle_thresholds_heatbath(T, s->thr_hb);
     s->S = (int8_t *)malloc((size_t)ORACLE_LANES * s->N);
     s->J = (int8_t *)malloc((size_t)ORACLE_LANES * 3 * s->N);
     s->snap = n_slots ? (int8_t *)malloc((size_t)n_slots * ORACLE_LANES * s->N) : NULL;
@@ -232,7 +256,8 @@ void oracle_destroy(oracle_sim *s)
     free(s);
 }
 
-void oracle_set_temperature(oracle_sim *s, double T) { s->T = T; oracle_thresholds(T, s->thr); }
+void oracle_set_temperature(oracle_sim *s, double T) { s->T = T; oracle_thresholds(T, s->thr); oracle_thresholds_heatbath(T, s->thr_hb); }
+int oracle_set_dynamics(oracle_sim *s, int dynamics) { if (dynamics != 0 && dynamics != 1) return 1; s->dynamics = dynamics; return 0; }
 void oracle_get_thresholds(const oracle_sim *s, uint64_t thr[3]) { memcpy(thr, s->thr, sizeof(s->thr)); }
 uint64_t oracle_get_time(const oracle_sim *s) { return s->t; }
 void oracle_set_time(oracle_sim *s, uint64_t t) { s->t = t; }
@@ -287,7 +312,7 @@ static int metropolis_trial(oracle_sim *s, int lane, int x, int y, int z)
     int8_t *S = s->S + (int64_t)lane * s->N;
     int local_sum = local_sum_xyz(s, lane, x, y, z);
     uint32_t r = lane < 32 ? s->r_lo[site] : s->r_hi[site]; /* C-A7 */
-    if (!oracle_accept(s->thr, local_sum, r)) return 0;
+    if (!(s->dynamics == 0 ? oracle_accept(s->thr, local_sum, r) : oracle_accept_heatbath(s->thr_hb, local_sum, r))) return 0;
     S[site] = (int8_t)-S[site];
     return 2 * local_sum; /* Delta E of the flip = 2 sum_j J_ij S_i S_j (Eq. 1) */
 }

@@ -478,3 +478,27 @@ def test_c4_vectors_argument_errors():
     g3 = binding.Sim(48, 0.5, 0.8, n_replicas=2, n_slots=0)
     with pytest.raises(binding.EAError):
         g3.c4_shells(2)
+
+
+def test_scan_of_concurrent_sims_matches_the_oracle_point_by_point():
+    """NEXT-4 driver: a p-scan at L = 16 and 32 (each sim on its own stream, graphs replayed back to back) --
+    every point must be the trajectory the oracle computes for that point alone."""
+    from paper_1411_5512_b200.scan import Scan
+    points = [{"L": L, "p": p, "T": 0.8, "seed": wl.seed_for(4, k)} for k, (L, p) in
+              enumerate([(16, 0.5), (16, 0.77), (32, 0.6), (16, 1.0), (32, 0.9)])]
+    sc = Scan(points)
+    sc.sweep(3)
+    sc.snapshot(0)
+    sc.sweep(37)          # 32-sweep graph replay + direct launches, interleaved over the five streams
+    recs = sc.measure(slot=0, r_max=8)
+    for pt, sim, rec in zip(points, sc.sims, recs):
+        o = Oracle(pt["L"], pt["p"], pt["T"], n_replicas=2, seed=pt["seed"], n_slots=1)
+        o.sweep(3)
+        o.snapshot(0)
+        o.sweep(37)
+        assert rec["t"] == o.time == 40
+        assert_same_state(sim, o, "scan point %r" % (pt,))
+        assert np.array_equal(rec["E"], o.energy()) and np.array_equal(rec["M"], o.magnetisation())
+        assert np.array_equal(rec["A"], o.autocorr(0))
+        assert np.array_equal(rec["B"], o.c4(8)) and np.array_equal(rec["q"], o.overlap())
+    sc.close()

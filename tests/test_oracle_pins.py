@@ -230,16 +230,20 @@ def test_P2_metropolis_rule_with_integer_thresholds_leaves_boltzmann_stationary(
         assert np.abs(pi @ P - pi).max() < 1e-8
 
 
-def _l2_sweep_matrix(J, T):
-    """Exact 256x256 transition matrix of one sweep (parity 0 then 1) of checkerboard Metropolis on L = 2,
-    built ONLY from the brute-force energies: a(s -> s^i) = min(1, exp(-(E(s^i) - E(s)) / T)) (Eq. 9)."""
+def _l2_sweep_matrix(J, T, rule="metropolis"):
+    """Exact 256x256 transition matrix of one sweep (parity 0 then 1) of checkerboard dynamics on L = 2,
+    built ONLY from the brute-force energies: Metropolis a(s -> s^i) = min(1, exp(-(E(s^i) - E(s)) / T)) (Eq. 9),
+    heat bath a = 1 / (1 + exp((E(s^i) - E(s)) / T)) (C-HB)."""
     E = _l2_energies(J)
     P_full = np.eye(256)
     for parity in (0, 1):
         sites = [s for s in range(8) if ((s % 2) + ((s // 2) % 2) + (s // 4)) % 2 == parity]
         P = np.zeros((256, 256))
         for state in range(256):
-            acc = [min(1.0, math.exp(-(E[state ^ (1 << s)] - E[state]) / T)) for s in sites]
+            if rule == "metropolis":
+                acc = [min(1.0, math.exp(-(E[state ^ (1 << s)] - E[state]) / T)) for s in sites]
+            else:
+                acc = [1.0 / (1.0 + math.exp((E[state ^ (1 << s)] - E[state]) / T)) for s in sites]
             for flips in itertools.product((0, 1), repeat=4):
                 pr, new = 1.0, state
                 for s, f, q in zip(sites, flips, acc):
@@ -251,16 +255,18 @@ def _l2_sweep_matrix(J, T):
     return E, P_full
 
 
-def test_P2_oracle_one_sweep_transitions_match_the_exact_boltzmann_metropolis_matrix():
+@pytest.mark.parametrize("rule", ["metropolis", "heatbath"])
+def test_P2_oracle_one_sweep_transitions_match_the_exact_boltzmann_metropolis_matrix(rule):
     # For EVERY one of the 256 states, the oracle's empirical next-state distribution after one sweep
     # (over many sweep counters t = independent random numbers) must equal the exact row of the matrix
     # above, and that matrix must leave exp(-H/T)/Z stationary (detailed balance per half-sweep).
     T, K = 2.0, 1500
     o = Oracle(2, 0.5, T, 1, seed=77)
+    o.set_dynamics(rule)
     rng = np.random.default_rng(12)
     J = rng.choice([-1, 1], size=(3, 8))
     o.set_bonds(np.where(J.reshape(-1) < 0, ALL, np.uint64(0)))           # same disorder in all 64 lanes
-    E, P = _l2_sweep_matrix(J, T)
+    E, P = _l2_sweep_matrix(J, T, rule)
     pi = np.exp(-E / T)
     pi /= pi.sum()
     assert np.abs(pi @ P - pi).max() < 1e-12                              # Boltzmann is stationary
@@ -520,6 +526,57 @@ def test_P11_identical_replicas_give_full_correlation():
     assert (o.overlap() == o.N).all() and (o.c4(2) == o.N).all()
     with pytest.raises(ValueError):
         Oracle(4, 0.5, 0.8, 1, seed=1).c4(2)                              # needs two replicas
+
+
+# ----------------------------------------------------------------------------------------
+# P16  heat-bath variant (reading C-HB) -- not the paper's dynamics
+# ----------------------------------------------------------------------------------------
+def test_P16_heatbath_thresholds_closed_form_symmetry_and_limits():
+    for T in (0.5, 0.8, 2.0, 7.3):
+        thr = [int(x) for x in oracle.thresholds_heatbath(T)]
+        for n_u in range(7):
+            dE = 12 - 4 * n_u
+            assert abs(thr[n_u] / 2.0 ** 32 - 1.0 / (1.0 + math.exp(dE / T))) <= 2.0 ** -32   # closed form
+            assert abs(thr[n_u] + thr[6 - n_u] - 2 ** 32) <= 1                                 # P(dE) + P(-dE) = 1
+        assert thr[3] == 2 ** 31 and thr == sorted(thr)                                        # dE = 0: exactly 1/2
+        m = [int(x) for x in oracle.thresholds(T)]                                             # detailed balance ratio
+        for n_u in range(3):                                                                   # P(dE)/P(-dE) = e^{-dE/T} = Metropolis
+            assert abs(thr[n_u] / thr[6 - n_u] - m[n_u] / 2.0 ** 32) < 1e-6 * max(1.0, m[n_u] / 2.0 ** 32) + 2e-9
+    assert [int(x) for x in oracle.thresholds_heatbath(0.0)] == [0, 0, 0, 2 ** 31, 2 ** 32, 2 ** 32, 2 ** 32]
+    assert [int(x) for x in oracle.thresholds_heatbath(float("inf"))] == [2 ** 31] * 7
+    thr = oracle.thresholds_heatbath(0.8)
+    for n_u in range(7):                                                                       # strict "<" at the edge
+        t = int(thr[n_u])
+        if 0 < t < 2 ** 32:
+            assert oracle.accept_heatbath(thr, 6 - 2 * n_u, t - 1) and not oracle.accept_heatbath(thr, 6 - 2 * n_u, t)
+
+
+def test_P16_heatbath_single_spin_frequencies_and_energy_bookkeeping():
+    L, T = 4, 6.0
+    o = Oracle(L, 1.0, T, 1, seed=5)
+    o.set_dynamics("heatbath")
+    K, flips = 600, np.zeros(64)
+    for t in range(K):                                    # all-up ferromagnet: n_u = 0 at every site, P = 1/(1+e^{12/T})
+        o.set_spins(np.zeros(o.N, dtype=np.uint64))
+        o.time = t
+        o.half_sweep(0)
+        flips += (o.spin_bytes() < 0).sum(axis=1)
+    pf = 1.0 / (1.0 + math.exp(12.0 / T))
+    n = K * o.N // 2
+    assert abs(flips.sum() / 64 - n * pf) < 5 * math.sqrt(n * pf * (1 - pf) / 2)   # the 64 lanes share 2 numbers per site (C-A7)
+    o2 = Oracle(6, 0.5, 1.0, 2, seed=9)                   # energy from Eq. 1 = E(0) + accepted Delta E (as P4), under heat bath
+    o2.set_dynamics("heatbath")
+    E0 = o2.energy()
+    o2.sweep(5)
+    assert (o2.energy() == E0 + o2.dE_accum()).all()
+    o3 = Oracle(6, 0.5, 0.0, 1, seed=9)                   # T = 0: energy never rises; dE = 0 moves are coin flips
+    o3.set_dynamics("heatbath")
+    E = o3.energy()
+    for _ in range(6):
+        o3.sweep(1)
+        E2 = o3.energy()
+        assert (E2 <= E).all()
+        E = E2
 
 
 # ----------------------------------------------------------------------------------------
