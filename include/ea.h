@@ -55,6 +55,11 @@ typedef enum {
     EA_KERNEL_RESIDENT = 4 /* persistent cooperative kernel, many sweeps per launch       */
 } ea_kernel;
 
+/* Single-spin dynamics.  The paper uses Metropolis (Eq. 9); heat bath is the variant of SURVEY 8(f)
+ * item 4 -- reading C-HB: flip with probability 1 / (1 + exp(Delta E / T)), Delta E = 12 - 4 n_u, for every
+ * n_u = 0..6 (Delta E = 0: exactly 1/2), same random numbers, same strict "<" against 32-bit thresholds. */
+typedef enum { EA_DYN_METROPOLIS = 0, EA_DYN_HEATBATH = 1 } ea_dynamics;
+
 typedef struct ea_params {
     int32_t L;          /* lattice side; even, >= 2, L^3 < 2^31 (C-A1)                     */
     int32_t n_samples;  /* must be 64                                                      */
@@ -95,6 +100,9 @@ ea_status ea_get_time(const ea_sim *sim, uint64_t *t); /* completed sweeps since
 ea_status ea_set_time(ea_sim *sim, uint64_t t);
 ea_status ea_set_temperature(ea_sim *sim, double T);   /* recomputes the thresholds               */
 ea_status ea_get_thresholds(const ea_sim *sim, uint64_t thr[3]); /* thr[n_u], n_u = 0,1,2 (C-A4)  */
+ea_status ea_set_dynamics(ea_sim *sim, int dynamics);  /* ea_dynamics; heat bath runs the per-colour launches */
+ea_status ea_get_dynamics(const ea_sim *sim, int *dynamics);
+ea_status ea_get_thresholds_heatbath(const ea_sim *sim, uint64_t thr[7]); /* thr[n_u], n_u = 0..6 (C-HB)     */
 ea_status ea_set_kernel(ea_sim *sim, int kernel);      /* EA_ERR_INVALID if not valid for this L  */
 ea_status ea_get_kernel(const ea_sim *sim, int *kernel); /* the variant AUTO resolved to          */
 ea_status ea_synchronize(ea_sim *sim);                 /* wait for the sim's stream               */

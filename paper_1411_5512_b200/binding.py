@@ -44,6 +44,9 @@ SIGNATURES = {
     "ea_set_time": (_i, [_vp, _u64]),
     "ea_set_temperature": (_i, [_vp, _dbl]),
     "ea_get_thresholds": (_i, [_vp, C.POINTER(_u64)]),
+    "ea_set_dynamics": (_i, [_vp, _i]),
+    "ea_get_dynamics": (_i, [_vp, C.POINTER(_i)]),
+    "ea_get_thresholds_heatbath": (_i, [_vp, C.POINTER(_u64)]),
     "ea_set_kernel": (_i, [_vp, _i]),
     "ea_get_kernel": (_i, [_vp, C.POINTER(_i)]),
     "ea_synchronize": (_i, [_vp]),
@@ -178,6 +181,17 @@ class Sim:
     def thresholds(self):
         thr = (_u64 * 3)()
         self._ck(lib().ea_get_thresholds(self._h, thr))
+        return np.array(list(thr), dtype=np.uint64)
+
+    def set_dynamics(self, dynamics):
+        """"metropolis" (the paper's, Eq. 9) or "heatbath" (reading C-HB)."""
+        code = {"metropolis": 0, "heatbath": 1}[dynamics] if isinstance(dynamics, str) else int(dynamics)
+        self._ck(lib().ea_set_dynamics(self._h, code))
+
+    @property
+    def thresholds_heatbath(self):
+        thr = (C.c_uint64 * 7)()
+        self._ck(lib().ea_get_thresholds_heatbath(self._h, thr))
         return np.array(list(thr), dtype=np.uint64)
 
     @property

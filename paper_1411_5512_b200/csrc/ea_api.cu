@@ -49,6 +49,18 @@ static void compute_thresholds(double T, uint64_t thr[3], Thresholds &th)
     }
 }
 
+// Heat bath (C-HB): thr[n_u] = floor(2^32 / (1 + exp((12 - 4 n_u) / T)) + 0.5); Delta E = 0 is exactly 1/2 at any T.
+static void compute_thresholds_heatbath(double T, uint64_t thr[7], Thresholds &th)
+{
+    for (int k = 0; k < 7; ++k) {
+        const double dE = 12.0 - 4.0 * (double)k;
+        const double w = dE == 0.0 ? 1.0 : exp(dE / T);
+        thr[k] = (uint64_t)floor(4294967296.0 * (1.0 / (1.0 + w)) + 0.5);
+        th.hb[k] = thr[k] > 0xffffffffull ? 0xffffffffu : (uint32_t)thr[k];
+        th.hb_always[k] = thr[k] > 0xffffffffull ? 0xffffffffu : 0u;
+    }
+}
+
 struct DeviceGuard {
     int prev = -1;
     bool ok = true;
@@ -205,6 +217,7 @@ ea_status ea_create_ex(const ea_params *prm, ea_sim **out)
     s->device = device;
     s->kernel = kernel;
     compute_thresholds(s->T, s->thr, s->th);
+    compute_thresholds_heatbath(s->T, s->thr_hb, s->th);
     s->slot_set.assign(prm->n_slots, 0);
     s->slot_t.assign(prm->n_slots, 0);
 
@@ -309,7 +322,7 @@ ea_status ea_sweep(ea_sim *sim, uint64_t n)
     if (!sim) return EA_ERR_INVALID;
     DeviceGuard g(sim->device);
     uint64_t left = n;
-    if (sim->kernel == EA_KERNEL_RESIDENT && n >= sim->resident_min_sweeps) {
+    if (sim->kernel == EA_KERNEL_RESIDENT && sim->dynamics == EA_DYN_METROPOLIS && n >= sim->resident_min_sweeps) {
         while (left) {
             const uint32_t chunk = (uint32_t)(left < RESIDENT_MAX_SWEEPS ? left : RESIDENT_MAX_SWEEPS);
             EA_CUDA(sim, launch_sweeps_resident(sim, sim->t, chunk, sim->stream));
@@ -370,6 +383,7 @@ ea_status ea_set_temperature(ea_sim *sim, double T)
     if (!(T >= 0.0)) EA_FAIL(sim, EA_ERR_INVALID, "T must be >= 0");
     sim->T = T;
     compute_thresholds(T, sim->thr, sim->th);
+    compute_thresholds_heatbath(T, sim->thr_hb, sim->th);
     DeviceGuard g(sim->device);
     destroy_graph(sim); // thresholds are baked into the captured launches
     return EA_OK;
@@ -379,6 +393,32 @@ ea_status ea_get_thresholds(const ea_sim *sim, uint64_t thr[3])
 {
     if (!sim || !thr) return EA_ERR_INVALID;
     memcpy(thr, sim->thr, sizeof(sim->thr));
+    return EA_OK;
+}
+
+ea_status ea_set_dynamics(ea_sim *sim, int dynamics)
+{
+    if (!sim) return EA_ERR_INVALID;
+    if (dynamics != EA_DYN_METROPOLIS && dynamics != EA_DYN_HEATBATH) EA_FAIL(sim, EA_ERR_INVALID, "unknown dynamics %d", dynamics);
+    if (dynamics != sim->dynamics) {
+        DeviceGuard g(sim->device);
+        destroy_graph(sim); // the captured launches are of the other rule's kernels
+        sim->dynamics = dynamics;
+    }
+    return EA_OK;
+}
+
+ea_status ea_get_dynamics(const ea_sim *sim, int *dynamics)
+{
+    if (!sim || !dynamics) return EA_ERR_INVALID;
+    *dynamics = sim->dynamics;
+    return EA_OK;
+}
+
+ea_status ea_get_thresholds_heatbath(const ea_sim *sim, uint64_t thr[7])
+{
+    if (!sim || !thr) return EA_ERR_INVALID;
+    memcpy(thr, sim->thr_hb, sizeof(sim->thr_hb));
     return EA_OK;
 }
 

@@ -154,6 +154,10 @@ __device__ __forceinline__ void sweep_random(const SweepRng &g, uint32_t first_s
 struct Thresholds {
     uint32_t thr[3];    // min(thr[k], 2^32 - 1)
     uint32_t always[3]; // 0xffffffff if thr[k] == 2^32 else 0
+    // heat-bath variant (reading C-HB; not the paper's dynamics): P(flip | n_u) = 1 / (1 + exp((12 - 4 n_u) / T)),
+    // n_u = 0..6, increasing in n_u; same clamping
+    uint32_t hb[7];
+    uint32_t hb_always[7];
 };
 
 __device__ __forceinline__ uint32_t xor3(uint32_t a, uint32_t b, uint32_t c) { return a ^ b ^ c; }
@@ -198,6 +202,30 @@ __device__ __forceinline__ uint32_t flip_half(uint32_t u1, uint32_t u2, uint32_t
     return f;
 }
 
+// Heat bath (C-HB): flip iff r < hb[n_u].  hb is increasing in n_u, so with k* the smallest k with r < hb[k] the
+// decision is [n_u >= k*]: a chain of seven predicated assignments from k = 6 down to 0 (the last one taken is k*).
+// n_u = b0 + 2 b1 + 4 b2 from the two full adders; [n_u >= k] are LOP3s of (b2, b1, b0).
+__device__ __forceinline__ uint32_t flip_half_heatbath(uint32_t u1, uint32_t u2, uint32_t u3, uint32_t u4, uint32_t u5,
+                                                       uint32_t u6, uint32_t r, const Thresholds &th)
+{
+    const HalfCount h = count_half(u1, u2, u3, u4, u5, u6);
+    const uint32_t b0 = h.sa ^ h.sb, c1 = h.sa & h.sb;
+    const uint32_t b1 = xor3(h.ka, h.kb, c1), b2 = maj3(h.ka, h.kb, c1);
+    const uint32_t ge1 = b2 | b1 | b0, ge2 = b2 | b1, ge3 = b2 | (b1 & b0), ge4 = b2, ge5 = b2 & (b1 | b0), ge6 = b2 & b1;
+    uint32_t f = 0;
+    if (r < th.hb[6]) f = ge6;
+    if (r < th.hb[5]) f = ge5;
+    if (r < th.hb[4]) f = ge4;
+    if (r < th.hb[3]) f = ge3;
+    if (r < th.hb[2]) f = ge2;
+    if (r < th.hb[1]) f = ge1;
+    if (r < th.hb[0]) f = 0xffffffffu;
+    // hb[k] == 2^32 (T = 0, Delta E < 0): certain, whatever r
+    f |= (th.hb_always[6] & ge6) | (th.hb_always[5] & ge5) | (th.hb_always[4] & ge4) | (th.hb_always[3] & ge3) |
+         (th.hb_always[2] & ge2) | (th.hb_always[1] & ge1) | th.hb_always[0];
+    return f;
+}
+
 // 64-bit word <-> halves
 __device__ __forceinline__ uint32_t lo32(uint64_t w) { return (uint32_t)w; }
 __device__ __forceinline__ uint32_t hi32(uint64_t w) { return (uint32_t)(w >> 32); }
@@ -214,13 +242,22 @@ __device__ __forceinline__ uint32_t bond_hi(uint32_t j) { return j; } // replica
 // RARE (low temperature, thr[2] << 2^32): the three energy-raising levels sit behind ONE warp-level branch per
 // word, taken only if some lane drew r < thr[2] in either half (T = 0.8: 0.7 % per draw, 35 % per warp and word),
 // instead of six compares and eight predicated LOP3 on the alu pipe that binds these kernels.  Same result.
-template <typename BondT, bool ALWAYS, bool RARE = false>
+template <typename BondT, bool ALWAYS, bool RARE = false, bool HB = false>
 __device__ __forceinline__ uint64_t metropolis_word(uint64_t s, uint64_t n1, uint64_t n2, uint64_t n3, uint64_t n4,
                                                     uint64_t n5, uint64_t n6, BondT j1, BondT j2, BondT j3, BondT j4,
                                                     BondT j5, BondT j6, uint32_t r_lo, uint32_t r_hi,
                                                     const Thresholds &th)
 {
     const uint32_t sl = lo32(s), sh = hi32(s);
+    if (HB) {
+        const uint32_t fl = flip_half_heatbath(bond_lo(j1) ^ sl ^ lo32(n1), bond_lo(j2) ^ sl ^ lo32(n2),
+                                               bond_lo(j3) ^ sl ^ lo32(n3), bond_lo(j4) ^ sl ^ lo32(n4),
+                                               bond_lo(j5) ^ sl ^ lo32(n5), bond_lo(j6) ^ sl ^ lo32(n6), r_lo, th);
+        const uint32_t fh = flip_half_heatbath(bond_hi(j1) ^ sh ^ hi32(n1), bond_hi(j2) ^ sh ^ hi32(n2),
+                                               bond_hi(j3) ^ sh ^ hi32(n3), bond_hi(j4) ^ sh ^ hi32(n4),
+                                               bond_hi(j5) ^ sh ^ hi32(n5), bond_hi(j6) ^ sh ^ hi32(n6), r_hi, th);
+        return mk64(sl ^ fl, sh ^ fh);
+    }
     if (RARE && !ALWAYS) {
         const HalfCount hl = count_half(bond_lo(j1) ^ sl ^ lo32(n1), bond_lo(j2) ^ sl ^ lo32(n2), bond_lo(j3) ^ sl ^ lo32(n3),
                                         bond_lo(j4) ^ sl ^ lo32(n4), bond_lo(j5) ^ sl ^ lo32(n5), bond_lo(j6) ^ sl ^ lo32(n6));

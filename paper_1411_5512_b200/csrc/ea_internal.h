@@ -21,6 +21,8 @@ struct ea_sim {
     int n_sm = 148;
     cudaStream_t stream = nullptr;
     int kernel = EA_KERNEL_SCALAR; // resolved variant
+    int dynamics = EA_DYN_METROPOLIS;
+    uint64_t thr_hb[7] = {0, 0, 0, 0, 0, 0, 0};
 
     bool own_ws = false, own_stream = false;
     char *ws = nullptr;

@@ -49,7 +49,7 @@ __device__ __forceinline__ void decode_row(const Lattice &lat, unsigned tid, uns
 // SCALAR: one site per thread, any even L >= 2 (L = 2: +x and -x neighbours are the same site,
 // reached through two distinct bonds -- C-S15).
 // ---------------------------------------------------------------------------------------------
-template <typename BondT, bool POW2, bool ALWAYS>
+template <typename BondT, bool POW2, bool ALWAYS, bool HB>
 __global__ void __launch_bounds__(256) k_sweep_scalar(const SweepArgs a)
 {
     const Lattice lat = a.lat;
@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(256) k_sweep_scalar(const SweepArgs a)
     const uint32_t site = (2 * xh + s) + L * (y + L * z); // canonical site index
     uint32_t r_lo, r_hi;                                   // counter word 0 = the first site of the pair (xh even)
     sweep_random(g, site - 2 * (xh & 1u), xh & 1u, r_lo, r_hi);
-    a.own[i] = metropolis_word<BondT, ALWAYS>(sg, n_xp, n_xm, n_yp, n_ym, n_zp, n_zm, j_xp, j_xm, j_yp, j_ym, j_zp, j_zm,
+    a.own[i] = metropolis_word<BondT, ALWAYS, false, HB>(sg, n_xp, n_xm, n_yp, n_ym, n_zp, n_zm, j_xp, j_xm, j_yp, j_ym, j_zp, j_zm,
                                       r_lo, r_hi, a.th);
 }
 
@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(256) k_sweep_scalar(const SweepArgs a)
 // bond word per thread is a 128-bit (uint64 pairs) or 64-bit (uint32 bond pairs) vector.  L % 4 == 0.
 // ---------------------------------------------------------------------------------------------
 
-template <typename BondT, bool POW2, bool ALWAYS>
+template <typename BondT, bool POW2, bool ALWAYS, bool HB>
 __global__ void __launch_bounds__(256) k_sweep_vec2(const SweepArgs a)
 {
     const Lattice lat = a.lat;
@@ -144,8 +144,8 @@ __global__ void __launch_bounds__(256) k_sweep_vec2(const SweepArgs a)
     const uint32_t site0 = (4 * k + s) + L * (y + L * z);
     const uint4 r = sweep_random4(g, site0); // the thread's two words are one pair (xh = 2k, 2k + 1): one block
     ulonglong2 out;
-    out.x = metropolis_word<BondT, ALWAYS>(sg0, np0, nm0, yp0, ym0, zp0, zm0, jx0, jm0, jy0, by0, jz0, bz0, r.x, r.y, a.th);
-    out.y = metropolis_word<BondT, ALWAYS>(sg1, np1, nm1, yp1, ym1, zp1, zm1, jx1, jm1, jy1, by1, jz1, bz1, r.z, r.w, a.th);
+    out.x = metropolis_word<BondT, ALWAYS, false, HB>(sg0, np0, nm0, yp0, ym0, zp0, zm0, jx0, jm0, jy0, by0, jz0, bz0, r.x, r.y, a.th);
+    out.y = metropolis_word<BondT, ALWAYS, false, HB>(sg1, np1, nm1, yp1, ym1, zp1, zm1, jx1, jm1, jy1, by1, jz1, bz1, r.z, r.w, a.th);
     *(ulonglong2 *)(a.own + i0) = out;
 }
 
@@ -162,7 +162,7 @@ __global__ void k_bump_time(uint64_t *d_time, uint32_t n) { *d_time += n; }
 // warp-uniform.
 // ---------------------------------------------------------------------------------------------
 
-template <int L, int M, int S0, typename BondT, bool ALWAYS>
+template <int L, int M, int S0, typename BondT, bool ALWAYS, bool HB>
 __device__ __forceinline__ void march_rows(const SweepArgs &a, const SweepRng &g, const unsigned y0, const unsigned z,
                                            const unsigned k, const int lane_m, const int lane_p)
 {
@@ -186,16 +186,16 @@ __device__ __forceinline__ void march_rows(const SweepArgs &a, const SweepRng &g
         const uint32_t site0 = 4 * k + L * (y + L * z);
         ulonglong2 out;
         if (((m & 1) ^ S0) == 0)
-            out = update_pair<0, BondT, ALWAYS>(own, P0, Pm, Pp, Zm, Zp, jx, jy, jz, bx, by, bz, site0, g, a.th, lane_m, lane_p);
+            out = update_pair<0, BondT, ALWAYS, false, HB>(own, P0, Pm, Pp, Zm, Zp, jx, jy, jz, bx, by, bz, site0, g, a.th, lane_m, lane_p);
         else
-            out = update_pair<1, BondT, ALWAYS>(own, P0, Pm, Pp, Zm, Zp, jx, jy, jz, bx, by, bz, site0 + 1, g, a.th, lane_m, lane_p);
+            out = update_pair<1, BondT, ALWAYS, false, HB>(own, P0, Pm, Pp, Zm, Zp, jx, jy, jz, bx, by, bz, site0 + 1, g, a.th, lane_m, lane_p);
         *(ulonglong2 *)(a.own + row) = out;
         Pm = P0;
         P0 = Pp;
     }
 }
 
-template <int L, int M, typename BondT, bool ALWAYS>
+template <int L, int M, typename BondT, bool ALWAYS, bool HB>
 __global__ void __launch_bounds__(128) k_sweep_rows(const SweepArgs a)
 {
     constexpr unsigned RL = L / 4, G = 32 / RL; // lanes per row, rows per warp
@@ -208,41 +208,41 @@ __global__ void __launch_bounds__(128) k_sweep_rows(const SweepArgs a)
     const int lane_m = (int)((lane & ~(RL - 1)) | ((k - 1) & (RL - 1))), lane_p = (int)((lane & ~(RL - 1)) | ((k + 1) & (RL - 1)));
     const SweepRng g = make_sweep_rng(a.seed, sweep_time(a), (uint32_t)a.colour);
     if ((a.colour ^ zpar) == 0) // phase of row y0 (even): warp-uniform
-        march_rows<L, M, 0, BondT, ALWAYS>(a, g, y0, z, k, lane_m, lane_p);
+        march_rows<L, M, 0, BondT, ALWAYS, HB>(a, g, y0, z, k, lane_m, lane_p);
     else
-        march_rows<L, M, 1, BondT, ALWAYS>(a, g, y0, z, k, lane_m, lane_p);
+        march_rows<L, M, 1, BondT, ALWAYS, HB>(a, g, y0, z, k, lane_m, lane_p);
 }
 
-template <int L, typename BondT, bool ALWAYS>
+template <int L, typename BondT, bool ALWAYS, bool HB>
 static void launch_rows(const SweepArgs &a, cudaStream_t st)
 {
     constexpr int M = (L >= 128) ? 4 : 2, G = 32 / (L / 4);
     constexpr unsigned warps = (L / M) * (L / G), block = 128, grid = (warps * 32 + block - 1) / block;
-    k_sweep_rows<L, M, BondT, ALWAYS><<<grid, block, 0, st>>>(a);
+    k_sweep_rows<L, M, BondT, ALWAYS, HB><<<grid, block, 0, st>>>(a);
 }
 
 // ---------------------------------------------------------------------------------------------
-template <typename BondT, bool ALWAYS>
+template <typename BondT, bool ALWAYS, bool HB>
 static cudaError_t launch_typed(ea_sim *s, const SweepArgs &a, cudaStream_t st)
 {
     const Lattice &lat = s->lat;
     const bool pow2 = lat.log2L >= 0;
     if (s->kernel == EA_KERNEL_ROWS || s->kernel == EA_KERNEL_RESIDENT) { // RESIDENT: single half-sweeps go as ROWS
         switch (lat.L) {
-        case 16: launch_rows<16, BondT, ALWAYS>(a, st); break;
-        case 32: launch_rows<32, BondT, ALWAYS>(a, st); break;
-        case 64: launch_rows<64, BondT, ALWAYS>(a, st); break;
-        case 128: launch_rows<128, BondT, ALWAYS>(a, st); break;
+        case 16: launch_rows<16, BondT, ALWAYS, HB>(a, st); break;
+        case 32: launch_rows<32, BondT, ALWAYS, HB>(a, st); break;
+        case 64: launch_rows<64, BondT, ALWAYS, HB>(a, st); break;
+        case 128: launch_rows<128, BondT, ALWAYS, HB>(a, st); break;
         default: return cudaErrorInvalidValue;
         }
     } else if (s->kernel == EA_KERNEL_VEC2) {
         unsigned n = lat.Nh / 2, block = 256, grid = (n + block - 1) / block;
-        if (pow2) k_sweep_vec2<BondT, true, ALWAYS><<<grid, block, 0, st>>>(a);
-        else k_sweep_vec2<BondT, false, ALWAYS><<<grid, block, 0, st>>>(a);
+        if (pow2) k_sweep_vec2<BondT, true, ALWAYS, HB><<<grid, block, 0, st>>>(a);
+        else k_sweep_vec2<BondT, false, ALWAYS, HB><<<grid, block, 0, st>>>(a);
     } else {
         unsigned n = lat.Nh, block = 256, grid = (n + block - 1) / block;
-        if (pow2) k_sweep_scalar<BondT, true, ALWAYS><<<grid, block, 0, st>>>(a);
-        else k_sweep_scalar<BondT, false, ALWAYS><<<grid, block, 0, st>>>(a);
+        if (pow2) k_sweep_scalar<BondT, true, ALWAYS, HB><<<grid, block, 0, st>>>(a);
+        else k_sweep_scalar<BondT, false, ALWAYS, HB><<<grid, block, 0, st>>>(a);
     }
     s->count_launch();
     return cudaGetLastError();
@@ -251,8 +251,9 @@ static cudaError_t launch_typed(ea_sim *s, const SweepArgs &a, cudaStream_t st)
 template <typename BondT>
 static cudaError_t launch_typed(ea_sim *s, const SweepArgs &a, cudaStream_t st)
 {
+    if (s->dynamics == EA_DYN_HEATBATH) return launch_typed<BondT, false, true>(s, a, st); // carries its own always-masks
     const bool always = a.th.always[0] | a.th.always[1] | a.th.always[2]; // T = inf: some thr == 2^32
-    return always ? launch_typed<BondT, true>(s, a, st) : launch_typed<BondT, false>(s, a, st);
+    return always ? launch_typed<BondT, true, false>(s, a, st) : launch_typed<BondT, false, false>(s, a, st);
 }
 
 cudaError_t launch_half_sweep(ea_sim *s, int parity, uint64_t t, const uint64_t *d_time, uint32_t t_offset,

@@ -502,3 +502,46 @@ def test_scan_of_concurrent_sims_matches_the_oracle_point_by_point():
         assert np.array_equal(rec["A"], o.autocorr(0))
         assert np.array_equal(rec["B"], o.c4(8)) and np.array_equal(rec["q"], o.overlap())
     sc.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# NEXT-4: heat-bath dynamics (reading C-HB)
+# ----------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("T", [0.0, 0.8, 2.0, float("inf")])
+def test_heatbath_thresholds_match(T):
+    g = binding.Sim(4, 0.5, T)
+    assert [int(x) for x in g.thresholds_heatbath] == [int(x) for x in oracle.thresholds_heatbath(T)]
+
+
+@pytest.mark.parametrize("L,n_rep,T,sweeps", [(2, 1, 2.0, 100), (4, 2, 0.8, 100), (6, 1, 1.5, 60), (8, 2, 2.0, 60),
+                                               (12, 2, 0.0, 40), (16, 1, 0.8, 40), (16, 2, float("inf"), 10),
+                                               (32, 2, 2.0, 40), (64, 2, 0.8, 6), (128, 2, 0.8, 3)])
+def test_heatbath_sweeps_bit_exact_every_kernel(L, n_rep, T, sweeps):
+    for kern in kernels_for(L):
+        g, o = make_pair(L, 0.6, T, n_rep, wl.seed_for(3, L), kernel=kern)
+        g.set_dynamics("heatbath")
+        o.set_dynamics("heatbath")
+        done = 0
+        for chunk in (1, 2, sweeps):      # the last chunk goes through the CUDA graph when >= 32
+            n = min(chunk, sweeps - done)
+            if n <= 0:
+                break
+            g.sweep(n)
+            o.sweep(n)
+            done += n
+            assert_same_state(g, o, "heat bath L=%d %s after %d sweeps" % (L, kern, done))
+        assert np.array_equal(g.energy(), o.energy())
+
+
+def test_switching_dynamics_mid_run_and_auto_kernel_at_L128():
+    """Metropolis (RESIDENT at L = 128) -> heat bath (per-colour launches) -> Metropolis, same sim, same clock."""
+    c = wl.CONFIGS["cfg4"]
+    g, o = make_pair(c.L, c.p, c.T, c.n_replicas, c.seed, n_slots=0)
+    for dyn, n in (("metropolis", 8), ("heatbath", 2), ("metropolis", 8)):
+        g.set_dynamics(dyn)
+        o.set_dynamics(dyn)
+        g.sweep(n)
+        o.sweep(n)
+        assert_same_state(g, o, "after %s x %d" % (dyn, n))
+    with pytest.raises(binding.EAError):
+        g.set_dynamics(7)
