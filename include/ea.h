@@ -147,7 +147,8 @@ ea_status ea_energy(ea_sim *sim, int64_t *E);
 ea_status ea_magnetisation(ea_sim *sim, int64_t *M);
 
 /* Canonical packed I/O (host arrays: spins N words, bonds 3N words).
- * ea_set_bonds on a 2-replica sim: EA_ERR_INVALID unless hi half == lo half in every word. */
+ * ea_set_bonds on a 2-replica sim: EA_ERR_INVALID unless hi half == lo half in every word (checked on the device
+ * while packing: after this error the sim's bonds are undefined and must be set again). */
 ea_status ea_get_spins(ea_sim *sim, uint64_t *host);
 ea_status ea_set_spins(ea_sim *sim, const uint64_t *host);
 ea_status ea_get_bonds(ea_sim *sim, uint64_t *host);

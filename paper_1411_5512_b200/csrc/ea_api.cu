@@ -682,17 +682,20 @@ ea_status ea_get_bonds(ea_sim *sim, uint64_t *host)
 ea_status ea_set_bonds(ea_sim *sim, const uint64_t *host)
 {
     if (!sim || !host) return EA_ERR_INVALID;
-    if (sim->n_replicas == 2) // both replicas have "the same bond configuration"
-        for (int64_t k = 0; k < 3 * sim->N; ++k)
-            if ((uint32_t)host[k] != (uint32_t)(host[k] >> 32))
-                EA_FAIL(sim, EA_ERR_INVALID, "2-replica sim: bond word %lld has hi half != lo half", (long long)k);
     DeviceGuard g(sim->device);
-    for (int d = 0; d < 3; ++d) {
+    // both replicas have "the same bond configuration": the pack kernel raises a flag on hi != lo
+    unsigned *d_bad = sim->resident_flags + (resident_flag_bytes() / sizeof(unsigned) - 31);
+    EA_CUDA(sim, cudaMemsetAsync(d_bad, 0, sizeof(unsigned), sim->stream));
+    for (int d = 0; d < 3; ++d) { // the staging buffer holds one direction; stream order keeps copy d+1 behind pack d
         EA_CUDA(sim, cudaMemcpyAsync(sim->stage, host + (size_t)d * sim->N, (size_t)sim->N * 8, cudaMemcpyHostToDevice,
                                      sim->stream));
-        EA_CUDA(sim, launch_pack_bonds(sim, d, sim->stage));
-        EA_SYNC(sim);
+        EA_CUDA(sim, launch_pack_bonds(sim, d, sim->stage, d_bad));
     }
+    unsigned bad = 0;
+    EA_CUDA(sim, cudaMemcpyAsync(&bad, d_bad, sizeof(bad), cudaMemcpyDeviceToHost, sim->stream));
+    EA_SYNC(sim);
+    if (bad)
+        EA_FAIL(sim, EA_ERR_INVALID, "2-replica sim: a bond word has hi half != lo half; the sim's bonds are now undefined, set them again");
     return EA_OK;
 }
 

@@ -83,7 +83,7 @@ cudaError_t launch_sweeps_resident(ea_sim *s, uint64_t t0, uint32_t n, cudaStrea
 // canonical <-> internal
 cudaError_t launch_pack_spins(ea_sim *s, const uint64_t *d_canon, uint64_t *d_internal);   // canonical -> internal
 cudaError_t launch_unpack_spins(ea_sim *s, const uint64_t *d_internal, uint64_t *d_canon); // internal -> canonical
-cudaError_t launch_pack_bonds(ea_sim *s, int d, const uint64_t *d_canon);                  // one direction, N words
+cudaError_t launch_pack_bonds(ea_sim *s, int d, const uint64_t *d_canon, unsigned *d_bad); // one direction, N words; *d_bad |= 1 if hi != lo (2 replicas)
 cudaError_t launch_unpack_bonds(ea_sim *s, int d, uint64_t *d_canon);
 
 // observables: per-sample bit counts into s->counters (zeroed by the wrapper)

@@ -74,14 +74,18 @@ __global__ void k_unpack_spins(Lattice lat, const uint64_t *internal, uint64_t *
     canon[site] = internal[(size_t)c * lat.Nh + i];
 }
 
+// bad != nullptr (32-bit bond words): raise *bad if a word's hi half differs from its lo half -- both replicas must
+// have "the same bond configuration"; checked here instead of in a host loop over 3 N words
 template <typename BondT>
-__global__ void k_pack_bonds(Lattice lat, unsigned d, const uint64_t *canon, BondT *bonds)
+__global__ void k_pack_bonds(Lattice lat, unsigned d, const uint64_t *canon, BondT *bonds, unsigned *bad)
 {
     unsigned site = blockIdx.x * blockDim.x + threadIdx.x;
     if (site >= 2 * lat.Nh) return;
     unsigned c, i;
     compact_of(lat, site, c, i);
-    bonds[((size_t)c * 3 + d) * lat.Nh + i] = (BondT)canon[site];
+    const uint64_t w = canon[site];
+    if (sizeof(BondT) == 4 && bad && lo32(w) != hi32(w)) atomicOr(bad, 1u);
+    bonds[((size_t)c * 3 + d) * lat.Nh + i] = (BondT)w;
 }
 
 template <typename BondT>
@@ -146,12 +150,12 @@ cudaError_t launch_unpack_spins(ea_sim *s, const uint64_t *d_internal, uint64_t 
     return cudaGetLastError();
 }
 
-cudaError_t launch_pack_bonds(ea_sim *s, int d, const uint64_t *d_canon)
+cudaError_t launch_pack_bonds(ea_sim *s, int d, const uint64_t *d_canon, unsigned *d_bad)
 {
     if (s->n_replicas == 2)
-        k_pack_bonds<uint32_t><<<blocks_for(s->N, 256), 256, 0, s->stream>>>(s->lat, d, d_canon, (uint32_t *)s->bonds);
+        k_pack_bonds<uint32_t><<<blocks_for(s->N, 256), 256, 0, s->stream>>>(s->lat, d, d_canon, (uint32_t *)s->bonds, d_bad);
     else
-        k_pack_bonds<uint64_t><<<blocks_for(s->N, 256), 256, 0, s->stream>>>(s->lat, d, d_canon, (uint64_t *)s->bonds);
+        k_pack_bonds<uint64_t><<<blocks_for(s->N, 256), 256, 0, s->stream>>>(s->lat, d, d_canon, (uint64_t *)s->bonds, nullptr);
     s->count_launch();
     return cudaGetLastError();
 }
