@@ -52,7 +52,8 @@ typedef enum {
     EA_KERNEL_SCALAR = 1, /* one site per thread, 64-bit loads; any even L >= 2           */
     EA_KERNEL_VEC2 = 2,   /* two sites per thread, 128-bit loads; L % 4 == 0              */
     EA_KERNEL_ROWS = 3,   /* warp marches along y with a register window; L % 4 == 0      */
-    EA_KERNEL_RESIDENT = 4 /* persistent cooperative kernel, many sweeps per launch       */
+    EA_KERNEL_RESIDENT = 4, /* persistent cooperative kernel, many sweeps per launch (L = 128) */
+    EA_KERNEL_FOLD = 5     /* what a sim with n_samples < 64 runs (not selectable)        */
 } ea_kernel;
 
 /* Single-spin dynamics.  The paper uses Metropolis (Eq. 9); heat bath is the variant of SURVEY 8(f)
@@ -62,7 +63,11 @@ typedef enum { EA_DYN_METROPOLIS = 0, EA_DYN_HEATBATH = 1 } ea_dynamics;
 
 typedef struct ea_params {
     int32_t L;          /* lattice side; even, >= 2, L^3 < 2^31 (C-A1)                     */
-    int32_t n_samples;  /* must be 64                                                      */
+    int32_t n_samples;  /* M = samples per word: 64, or 32, 16, ... (mixed multispin coding, PAPER.md:94:
+                           64/M z-slabs of the lattice share a word; needs L % 4 == 0 and L*M/64 even;
+                           the M samples are lanes 0..M/2-1 and 32..32+M/2-1 of the 64-sample sim of
+                           the same seed (2 replicas) or lanes 0..M-1 (1 replica), bit for bit: C-M.
+                           Host arrays keep their 64- / 32-entry shape; unused entries are unspecified) */
     int32_t n_replicas; /* 1: 64 independent samples; 2: 32 disorders x 2 replicas (C-A2r) */
     int32_t n_slots;    /* snapshot slots for ea_snapshot / ea_autocorr (>= 0)             */
     double p;           /* P(J = +1), in [0,1]                              */
@@ -78,12 +83,13 @@ typedef struct ea_params {
 } ea_params;
 
 /* Bytes of device memory one sim needs (0 if the arguments are invalid). */
-size_t ea_workspace_bytes(int L, int n_replicas, int n_slots);
+size_t ea_workspace_bytes(int L, int n_replicas, int n_slots);                 /* n_samples = 64 */
+size_t ea_workspace_bytes_ex(int L, int n_samples, int n_replicas, int n_slots);
 
 /* Create a sim: bonds iid with P(J=+1) = p per disorder sample (C-A9), spins
  * uniform +-1 (random start = quench from T = inf, C-A8), t = 0.
  * ea_create: 64 independent samples (n_samples must be 64), 2 slots, current device, own stream.
- * EA_ERR_INVALID: L odd / < 2 / too large, p outside [0,1] or NaN, T < 0 or NaN, n_samples != 64,
+ * EA_ERR_INVALID: L odd / < 2 / too large, p outside [0,1] or NaN, T < 0 or NaN, n_samples not valid for L,
  * n_replicas not 1|2, n_slots < 0, out == NULL.  The caller owns *out until ea_destroy. */
 ea_status ea_create(int L, double p, double T, int n_samples, uint64_t seed, ea_sim **out);
 ea_status ea_create_ex(const ea_params *prm, ea_sim **out);

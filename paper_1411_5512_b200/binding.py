@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libea_b200.so")
 
 EA_OK, EA_ERR_INVALID, EA_ERR_CUDA, EA_ERR_NOMEM, EA_ERR_STATE = range(5)
-EA_KERNEL_AUTO, EA_KERNEL_SCALAR, EA_KERNEL_VEC2, EA_KERNEL_ROWS, EA_KERNEL_RESIDENT = range(5)
+EA_KERNEL_AUTO, EA_KERNEL_SCALAR, EA_KERNEL_VEC2, EA_KERNEL_ROWS, EA_KERNEL_RESIDENT, EA_KERNEL_FOLD = range(6)
 KERNEL_NAMES = {"auto": 0, "scalar": 1, "vec2": 2, "rows": 3, "resident": 4}
 LANES = 64
 
@@ -37,6 +37,7 @@ SIGNATURES = {
     "ea_workspace_bytes": (C.c_size_t, [_i, _i, _i]),
     "ea_create": (_i, [_i, _dbl, _dbl, _i, _u64, C.POINTER(_vp)]),
     "ea_create_ex": (_i, [C.POINTER(ea_params), C.POINTER(_vp)]),
+    "ea_workspace_bytes_ex": (C.c_size_t, [_i, _i, _i, _i]),
     "ea_destroy": (_i, [_vp]),
     "ea_sweep": (_i, [_vp, _u64]),
     "ea_half_sweep": (_i, [_vp, _i]),
@@ -104,11 +105,12 @@ class Sim:
     """One batch of 64 samples on an L^3 lattice on the GPU.  Methods mirror the C entry points."""
 
     def __init__(self, L, p, T, n_replicas=1, seed=0, n_slots=2, kernel="auto", device=None, stream=None,
-                 torch_workspace=True):
+                 torch_workspace=True, n_samples=LANES):
         self._h = _vp()
         self.L, self.N, self.n_replicas, self.n_slots = int(L), int(L) ** 3, int(n_replicas), int(n_slots)
+        self.n_samples = int(n_samples)
         prm = ea_params()
-        prm.L, prm.n_samples, prm.n_replicas, prm.n_slots = int(L), LANES, int(n_replicas), int(n_slots)
+        prm.L, prm.n_samples, prm.n_replicas, prm.n_slots = int(L), int(n_samples), int(n_replicas), int(n_slots)
         prm.p, prm.T, prm.seed = float(p), float(T), int(seed)
         prm.kernel = KERNEL_NAMES[kernel] if isinstance(kernel, str) else int(kernel)
         prm.device = -1 if device is None else int(device)
@@ -116,7 +118,7 @@ class Sim:
         self._stream = stream
         if stream is not None:  # a torch.cuda.Stream: the library launches on it
             prm.stream = stream.cuda_stream
-        nbytes = lib().ea_workspace_bytes(int(L), int(n_replicas), int(n_slots))
+        nbytes = lib().ea_workspace_bytes_ex(int(L), int(n_samples), int(n_replicas), int(n_slots))
         if torch_workspace and nbytes:
             import torch  # device memory only
             if not torch.cuda.is_available():
@@ -130,6 +132,17 @@ class Sim:
         if st != EA_OK:
             self._h = _vp()
             raise EAError(st, lib().ea_strerror(st).decode() + " (ea_create_ex)")
+
+    @property
+    def lane_mask(self):
+        """64-lane mask of the samples this sim carries (n_samples < 64: reading C-M)."""
+        M = self.n_samples
+        if M == LANES:
+            return 0xFFFFFFFFFFFFFFFF
+        if self.n_replicas == 2:
+            h = (1 << (M // 2)) - 1
+            return h | (h << 32)
+        return (1 << M) - 1
 
     # -- plumbing -----------------------------------------------------------------------------------
     def _ck(self, st):
@@ -150,6 +163,8 @@ class Sim:
 
     # -- dynamics -------------------------------------------------------------------------------------
     def sweep(self, n=1):
+        if int(n) < 0:
+            raise ValueError("sweep count must be >= 0 (got %d)" % int(n))  # would wrap to 2^64 - |n| in the C ABI
         self._ck(lib().ea_sweep(self._h, int(n)))
 
     def half_sweep(self, parity):

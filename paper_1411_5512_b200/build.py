@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libea_b200.so")
 SOURCES = ["ea_api.cu", "ea_sweep.cu", "ea_sweep_resident.cu", "ea_setup.cu", "ea_observables.cu",
-           "ea_c4_vectors.cu"]
+           "ea_c4_vectors.cu", "ea_fold.cu"]
 HEADERS = ["ea_device.cuh", "ea_sweep_common.cuh", "ea_internal.h", os.path.join("..", "..", "include", "ea.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]

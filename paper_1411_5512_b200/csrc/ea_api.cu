@@ -12,7 +12,7 @@ namespace ea {
 
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
-WorkspaceLayout workspace_layout(int L, int n_replicas, int n_slots)
+WorkspaceLayout workspace_layout(int L, int n_samples, int n_replicas, int n_slots)
 {
     WorkspaceLayout w;
     size_t N = (size_t)L * L * L, bond_bytes = n_replicas == 2 ? 4 : 8;
@@ -25,6 +25,7 @@ WorkspaceLayout workspace_layout(int L, int n_replicas, int n_slots)
     w.off_counters = off; off = align_up(off + w.n_counters * 8);
     w.off_time = off;     off = align_up(off + 8);
     w.off_flags = off;    off = align_up(off + resident_flag_bytes());
+    w.off_fold = off;     off = align_up(off + fold_bytes(L, n_samples));
     w.total = off;
     return w;
 }
@@ -128,6 +129,7 @@ static bool kernel_valid_for(int kernel, int L)
     case EA_KERNEL_VEC2: return L % 4 == 0;
     case EA_KERNEL_ROWS: return L == 16 || L == 32 || L == 64 || L == 128;
     case EA_KERNEL_RESIDENT: return L == 128; // plus a device check (resident_supported) once the sim exists
+    case EA_KERNEL_FOLD: return false;        // not selectable: it is what a sim with n_samples < 64 runs
     default: return false;
     }
 }
@@ -157,10 +159,12 @@ const char *ea_strerror(ea_status s)
 
 const char *ea_last_error(const ea_sim *sim) { return sim ? sim->err.c_str() : "null handle"; }
 
-size_t ea_workspace_bytes(int L, int n_replicas, int n_slots)
+size_t ea_workspace_bytes(int L, int n_replicas, int n_slots) { return ea_workspace_bytes_ex(L, EA_LANES, n_replicas, n_slots); }
+
+size_t ea_workspace_bytes_ex(int L, int n_samples, int n_replicas, int n_slots)
 {
-    if (!valid_L(L) || (n_replicas != 1 && n_replicas != 2) || n_slots < 0) return 0;
-    return workspace_layout(L, n_replicas, n_slots).total;
+    if (!valid_L(L) || (n_replicas != 1 && n_replicas != 2) || n_slots < 0 || !fold_valid(L, n_samples, n_replicas)) return 0;
+    return workspace_layout(L, n_samples, n_replicas, n_slots).total;
 }
 
 static void destroy_graph(ea_sim *s)
@@ -187,7 +191,8 @@ ea_status ea_destroy(ea_sim *sim)
 ea_status ea_create_ex(const ea_params *prm, ea_sim **out)
 {
     if (!prm || !out) return EA_ERR_INVALID;
-    if (!valid_L(prm->L) || prm->n_samples != EA_LANES || (prm->n_replicas != 1 && prm->n_replicas != 2) ||
+    if (!valid_L(prm->L) || (prm->n_replicas != 1 && prm->n_replicas != 2) ||
+        !fold_valid(prm->L, prm->n_samples, prm->n_replicas) ||
         prm->n_slots < 0 || !(prm->p >= 0.0 && prm->p <= 1.0) || !(prm->T >= 0.0))
         return EA_ERR_INVALID;
     int kernel = resolve_kernel(prm->kernel, prm->L);
@@ -209,6 +214,7 @@ ea_status ea_create_ex(const ea_params *prm, ea_sim **out)
     s->N = (int64_t)L * L * L;
     s->lat.Nh = (unsigned)(s->N / 2);
     s->n_replicas = prm->n_replicas;
+    s->n_samples = prm->n_samples;
     s->n_slots = prm->n_slots;
     s->p = prm->p;
     s->T = prm->T;
@@ -224,7 +230,7 @@ ea_status ea_create_ex(const ea_params *prm, ea_sim **out)
     DeviceGuard g(device);
     ea_status rc = EA_OK;
     cudaError_t e = cudaSuccess;
-    WorkspaceLayout w = workspace_layout(L, s->n_replicas, s->n_slots);
+    WorkspaceLayout w = workspace_layout(L, s->n_samples, s->n_replicas, s->n_slots);
     do {
         if (!g.ok) { rc = EA_ERR_CUDA; break; }
         cudaDeviceGetAttribute(&s->n_sm, cudaDevAttrMultiProcessorCount, device);
@@ -261,6 +267,12 @@ ea_status ea_create_ex(const ea_params *prm, ea_sim **out)
         s->h_counters.resize(w.n_counters);
         if ((e = launch_init_bonds(s)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
         if ((e = launch_init_spins(s)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
+        if (s->n_samples < EA_LANES) { // mixed multispin coding: the sweeps run on folded words (ea_fold.cu)
+            s->f_spins = (uint64_t *)(s->ws + w.off_fold);
+            s->f_bonds = s->f_spins + (size_t)2 * (s->lat.Nh / (EA_LANES / s->n_samples));
+            s->kernel = EA_KERNEL_FOLD;
+            if ((e = fold_from_standard(s, true, true)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
+        }
         if ((e = cudaMemsetAsync(s->d_time, 0, 8, s->stream)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
         if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
     } while (0);
@@ -322,6 +334,7 @@ ea_status ea_sweep(ea_sim *sim, uint64_t n)
     if (!sim) return EA_ERR_INVALID;
     DeviceGuard g(sim->device);
     uint64_t left = n;
+    if (n && sim->n_samples < EA_LANES) sim->unfolded_valid = false; // the standard-layout mirror goes stale
     if (sim->kernel == EA_KERNEL_RESIDENT && sim->dynamics == EA_DYN_METROPOLIS && n >= sim->resident_min_sweeps) {
         while (left) {
             const uint32_t chunk = (uint32_t)(left < RESIDENT_MAX_SWEEPS ? left : RESIDENT_MAX_SWEEPS);
@@ -360,6 +373,7 @@ ea_status ea_half_sweep(ea_sim *sim, int parity)
     if (parity != 0 && parity != 1) EA_FAIL(sim, EA_ERR_INVALID, "parity must be 0 or 1");
     DeviceGuard g(sim->device);
     EA_CUDA(sim, launch_half_sweep(sim, parity, sim->t, nullptr, 0, sim->stream));
+    if (sim->n_samples < EA_LANES) sim->unfolded_valid = false;
     return EA_OK;
 }
 
@@ -400,6 +414,8 @@ ea_status ea_set_dynamics(ea_sim *sim, int dynamics)
 {
     if (!sim) return EA_ERR_INVALID;
     if (dynamics != EA_DYN_METROPOLIS && dynamics != EA_DYN_HEATBATH) EA_FAIL(sim, EA_ERR_INVALID, "unknown dynamics %d", dynamics);
+    if (dynamics == EA_DYN_HEATBATH && sim->n_samples < EA_LANES)
+        EA_FAIL(sim, EA_ERR_STATE, "heat bath is not available with n_samples < 64");
     if (dynamics != sim->dynamics) {
         DeviceGuard g(sim->device);
         destroy_graph(sim); // the captured launches are of the other rule's kernels
@@ -425,6 +441,10 @@ ea_status ea_get_thresholds_heatbath(const ea_sim *sim, uint64_t thr[7])
 ea_status ea_set_kernel(ea_sim *sim, int kernel)
 {
     if (!sim) return EA_ERR_INVALID;
+    if (sim->n_samples < EA_LANES) {
+        if (kernel == EA_KERNEL_AUTO || kernel == EA_KERNEL_FOLD) return EA_OK;
+        EA_FAIL(sim, EA_ERR_STATE, "a sim with n_samples < 64 runs the folded kernel only");
+    }
     int k = resolve_kernel(kernel, sim->lat.L);
     if (!kernel_valid_for(k, sim->lat.L)) EA_FAIL(sim, EA_ERR_INVALID, "kernel %d not valid for L=%d", kernel, sim->lat.L);
     sim->resident_min_sweeps = 1;
@@ -475,6 +495,7 @@ ea_status ea_snapshot(ea_sim *sim, int slot)
     if (!sim) return EA_ERR_INVALID;
     if (slot < 0 || slot >= sim->n_slots) EA_FAIL(sim, EA_ERR_INVALID, "slot %d out of range [0,%d)", slot, sim->n_slots);
     DeviceGuard g(sim->device);
+    EA_CUDA(sim, fold_ensure_unfolded(sim));
     EA_CUDA(sim, cudaMemcpyAsync(sim->snaps + (size_t)slot * sim->N, sim->spins, (size_t)sim->N * 8,
                                  cudaMemcpyDeviceToDevice, sim->stream));
     sim->slot_set[slot] = 1;
@@ -488,6 +509,7 @@ ea_status ea_autocorr(ea_sim *sim, int slot, int64_t *A, double *C)
     if (slot < 0 || slot >= sim->n_slots) EA_FAIL(sim, EA_ERR_INVALID, "slot %d out of range [0,%d)", slot, sim->n_slots);
     if (!sim->slot_set[slot]) EA_FAIL(sim, EA_ERR_STATE, "slot %d holds no snapshot", slot);
     DeviceGuard g(sim->device);
+    EA_CUDA(sim, fold_ensure_unfolded(sim));
     EA_CUDA(sim, launch_count_spins(sim, sim->snaps + (size_t)slot * sim->N));
     ea_status rc = fetch_counters(sim, 64);
     if (rc != EA_OK) return rc;
@@ -502,6 +524,7 @@ ea_status ea_magnetisation(ea_sim *sim, int64_t *M)
 {
     if (!sim || !M) return EA_ERR_INVALID;
     DeviceGuard g(sim->device);
+    EA_CUDA(sim, fold_ensure_unfolded(sim));
     EA_CUDA(sim, launch_count_spins(sim, nullptr));
     ea_status rc = fetch_counters(sim, 64);
     if (rc != EA_OK) return rc;
@@ -513,6 +536,7 @@ ea_status ea_energy(ea_sim *sim, int64_t *E)
 {
     if (!sim || !E) return EA_ERR_INVALID;
     DeviceGuard g(sim->device);
+    EA_CUDA(sim, fold_ensure_unfolded(sim));
     EA_CUDA(sim, launch_count_energy(sim));
     ea_status rc = fetch_counters(sim, 64);
     if (rc != EA_OK) return rc;
@@ -526,6 +550,7 @@ ea_status ea_c4(ea_sim *sim, int r_max, int64_t *B, int64_t *q, double *c4_avg)
     if (sim->n_replicas != 2) EA_FAIL(sim, EA_ERR_STATE, "ea_c4 needs a 2-replica sim");
     if (r_max < 0 || r_max > sim->lat.L / 2) EA_FAIL(sim, EA_ERR_INVALID, "r_max %d outside [0, L/2]", r_max);
     DeviceGuard g(sim->device);
+    EA_CUDA(sim, fold_ensure_unfolded(sim));
     EA_CUDA(sim, launch_count_c4(sim, r_max));
     const size_t n_r = (size_t)r_max + 1, jobs = 3 * n_r + 1;
     ea_status rc = fetch_counters(sim, jobs * 32);
@@ -550,6 +575,7 @@ ea_status ea_c4_vectors(ea_sim *sim, int64_t n_vec, const int32_t *dxyz, int64_t
     if (!c4_vectors_supported(sim->lat.L)) EA_FAIL(sim, EA_ERR_INVALID, "ea_c4_vectors: L must be <= 32, 64 or 128");
     DeviceGuard g(sim->device);
     std::vector<unsigned long long> cnt((size_t)n_vec * 32);
+    EA_CUDA(sim, fold_ensure_unfolded(sim));
     EA_CUDA(sim, c4_vector_counts(sim, (size_t)n_vec, dxyz, cnt.data()));
     EA_SYNC(sim);
     for (size_t k = 0; k < cnt.size(); ++k) B[k] = sim->N - 2 * (int64_t)cnt[k];
@@ -574,6 +600,7 @@ ea_status ea_c4_shells(ea_sim *sim, int r_max, int64_t *S, int64_t *mult)
     std::vector<unsigned long long> cnt(n * 32);
     {
         DeviceGuard g(sim->device);
+        EA_CUDA(sim, fold_ensure_unfolded(sim));
         EA_CUDA(sim, c4_vector_counts(sim, n, vec.data(), cnt.data()));
         EA_SYNC(sim);
     }
@@ -638,6 +665,7 @@ ea_status ea_get_spins(ea_sim *sim, uint64_t *host)
 {
     if (!sim || !host) return EA_ERR_INVALID;
     DeviceGuard g(sim->device);
+    EA_CUDA(sim, fold_ensure_unfolded(sim));
     EA_CUDA(sim, launch_unpack_spins(sim, sim->spins, sim->stage));
     EA_CUDA(sim, cudaMemcpyAsync(host, sim->stage, (size_t)sim->N * 8, cudaMemcpyDeviceToHost, sim->stream));
     EA_SYNC(sim);
@@ -662,6 +690,7 @@ ea_status ea_set_spins(ea_sim *sim, const uint64_t *host)
     DeviceGuard g(sim->device);
     EA_CUDA(sim, cudaMemcpyAsync(sim->stage, host, (size_t)sim->N * 8, cudaMemcpyHostToDevice, sim->stream));
     EA_CUDA(sim, launch_pack_spins(sim, sim->stage, sim->spins));
+    if (sim->n_samples < EA_LANES) EA_CUDA(sim, fold_from_standard(sim, true, false)); // unused lanes are dropped
     EA_SYNC(sim);
     return EA_OK;
 }
@@ -691,6 +720,7 @@ ea_status ea_set_bonds(ea_sim *sim, const uint64_t *host)
                                      sim->stream));
         EA_CUDA(sim, launch_pack_bonds(sim, d, sim->stage, d_bad));
     }
+    if (sim->n_samples < EA_LANES) EA_CUDA(sim, fold_from_standard(sim, false, true));
     unsigned bad = 0;
     EA_CUDA(sim, cudaMemcpyAsync(&bad, d_bad, sizeof(bad), cudaMemcpyDeviceToHost, sim->stream));
     EA_SYNC(sim);

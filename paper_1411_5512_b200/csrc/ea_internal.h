@@ -13,6 +13,10 @@ struct ea_sim {
     ea::Lattice lat;
     int64_t N = 0;
     int n_replicas = 1, n_slots = 0;
+    int n_samples = 64;           // M: samples per word; < 64 = mixed multispin coding (ea_fold.cu), K = 64 / M slabs
+    uint64_t *f_spins = nullptr;  // folded spins [2][Nh/K]: the state the sweeps run on when M < 64
+    uint64_t *f_bonds = nullptr;  // folded bonds [2][3][Nh/K], 64-bit words
+    bool unfolded_valid = true;   // M < 64: does `spins` (standard layout, unused lanes zero) mirror f_spins?
     double p = 0, T = 0;
     uint64_t seed = 0, t = 0;
     uint64_t thr[3] = {0, 0, 0};
@@ -63,10 +67,10 @@ struct ea_sim {
 namespace ea {
 
 struct WorkspaceLayout {
-    size_t off_spins, off_bonds, off_snaps, off_stage, off_counters, off_time, off_flags, total;
+    size_t off_spins, off_bonds, off_snaps, off_stage, off_counters, off_time, off_flags, off_fold, total;
     size_t n_counters;
 };
-WorkspaceLayout workspace_layout(int L, int n_replicas, int n_slots);
+WorkspaceLayout workspace_layout(int L, int n_samples, int n_replicas, int n_slots);
 
 // ---- launch wrappers (each returns the cudaError_t of the launch) -------------------------------
 cudaError_t launch_init_spins(ea_sim *s);
@@ -75,6 +79,14 @@ cudaError_t launch_init_bonds(ea_sim *s);
 cudaError_t launch_half_sweep(ea_sim *s, int parity, uint64_t t, const uint64_t *d_time, uint32_t t_offset,
                               cudaStream_t st);
 cudaError_t launch_bump_time(ea_sim *s, uint32_t n, cudaStream_t st);
+// mixed multispin coding, M < 64 samples per word (ea_fold.cu)
+bool fold_valid(int L, int n_samples, int n_replicas);
+size_t fold_bytes(int L, int n_samples);
+uint64_t expand_lanes_host(const ea_sim *s);                     // the 64-lane mask of the samples carried
+cudaError_t fold_from_standard(ea_sim *s, bool spins, bool bonds); // mask unused lanes, (re)build the folded copies
+cudaError_t fold_ensure_unfolded(ea_sim *s);                     // refresh `spins` from f_spins if stale
+cudaError_t launch_half_sweep_fold(ea_sim *s, int parity, uint64_t t, const uint64_t *d_time, uint32_t t_offset,
+                                   cudaStream_t st);
 // RESIDENT (ea_sweep_resident.cu): n sweeps from sweep index t0 in one cooperative launch
 bool resident_supported(const ea_sim *s);
 size_t resident_flag_bytes();

@@ -259,6 +259,7 @@ static cudaError_t launch_typed(ea_sim *s, const SweepArgs &a, cudaStream_t st)
 cudaError_t launch_half_sweep(ea_sim *s, int parity, uint64_t t, const uint64_t *d_time, uint32_t t_offset,
                               cudaStream_t st)
 {
+    if (s->n_samples < EA_LANES) return launch_half_sweep_fold(s, parity, t, d_time, t_offset, st); // M < 64 (ea_fold.cu)
     SweepArgs a;
     a.lat = s->lat;
     a.colour = parity;

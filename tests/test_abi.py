@@ -57,7 +57,8 @@ def test_workspace_bytes_and_argument_validation(lib):
     assert n1 >= N * 8 * (1 + 3 + 2 + 1) and n1 < N * 8 * 7 + (1 << 20)
     assert n1 - n2 == 3 * N * 4                          # 32-bit bond words in replica mode
     h = C.c_void_p()
-    bad = [(7, 0.5, 0.8, 64), (8, 1.5, 0.8, 64), (8, 0.5, -1.0, 64), (8, 0.5, 0.8, 32), (8, float("nan"), 0.8, 64)]
+    bad = [(7, 0.5, 0.8, 64), (8, 1.5, 0.8, 64), (8, 0.5, -1.0, 64), (8, 0.5, 0.8, 48), (8, 0.5, 0.8, 8),
+           (8, float("nan"), 0.8, 64)]  # n_samples 48: not 2^m; 8 at L = 8: one plane per slab (needs an even number)
     for L, p, T, ns in bad:
         assert lib.ea_create(L, p, T, ns, 1, C.byref(h)) == binding.EA_ERR_INVALID
     assert lib.ea_strerror(binding.EA_ERR_STATE) == b"invalid state"
@@ -115,3 +116,16 @@ def test_host_side_c4_curve_and_integral_estimator_match_the_oracle():
     assert binding.integral_estimator(r, c, e, 1)[3] < R          # the noisy tail is cut off
     got = binding.integral_estimator(r, np.abs(c) + 1e-9, np.zeros_like(e), 1)    # nothing below 3 e: no cut-off
     assert got[3] == r[-1]
+
+
+def test_workspace_bytes_ex_validates_the_mixed_coding_parameters():
+    """No device needed: sizes and the validity rule of n_samples = M < 64 (DESIGN.md C-M)."""
+    from paper_1411_5512_b200 import binding
+    f = binding.lib().ea_workspace_bytes_ex
+    base = binding.lib().ea_workspace_bytes(16, 2, 1)
+    assert f(16, 64, 2, 1) == base > 0
+    assert f(16, 32, 2, 1) >= base + (16 ** 3 // 2) * 4 * 8        # folded spins + 3 folded bond planes, K = 2
+    assert f(16, 8, 2, 1) > base
+    for L, M, n_rep in ((10, 32, 2), (16, 3, 2), (16, 1, 2), (8, 8, 2), (16, 128, 2), (16, 0, 1)):
+        assert f(L, M, n_rep, 1) == 0
+    assert f(128, 1, 1, 0) > 0                                     # one sample, 64 slabs of two planes

@@ -545,3 +545,68 @@ def test_switching_dynamics_mid_run_and_auto_kernel_at_L128():
         assert_same_state(g, o, "after %s x %d" % (dyn, n))
     with pytest.raises(binding.EAError):
         g.set_dynamics(7)
+
+
+# ----------------------------------------------------------------------------------------------------
+# NEXT-3: mixed multispin coding, M < 64 samples per word (reading C-M)
+# ----------------------------------------------------------------------------------------------------
+def _used(mask64, n):
+    return [b for b in range(n) if (mask64 >> b) & 1]
+
+
+@pytest.mark.parametrize("L,M,n_rep,T,sweeps", [(8, 32, 2, 0.8, 40), (8, 16, 2, 2.0, 40), (16, 8, 2, 0.8, 40), (16, 32, 1, 0.8, 20),
+                                                 (16, 16, 1, float("inf"), 6), (32, 4, 2, 0.8, 36), (64, 2, 2, 2.0, 6),
+                                                 (12, 32, 2, 0.0, 20), (128, 32, 2, 0.8, 4), (128, 1, 1, 0.8, 4)])
+def test_folded_sim_is_the_used_lanes_of_the_64_sample_trajectory(L, M, n_rep, T, sweeps):
+    """A sim with n_samples = M < 64 stores 64/M z-slabs per word and rotates by M at the seam; by C-M its samples
+    are lanes of the 64-sample definition, so the ORACLE AS IT STANDS (64 lanes, same seed) is the reference:
+    spin words and bond words masked to the used lanes, and every observable on the used lanes."""
+    g = binding.Sim(L, 0.6, T, n_replicas=n_rep, seed=wl.seed_for(2, L + M), n_slots=1, n_samples=M)
+    o = Oracle(L, 0.6, T, n_replicas=n_rep, seed=wl.seed_for(2, L + M), n_slots=1)
+    assert g.kernel == binding.EA_KERNEL_FOLD
+    mask = np.uint64(g.lane_mask)
+    assert np.array_equal(g.get_bonds(), o.get_bonds() & mask)
+    assert np.array_equal(g.get_spins(), o.get_spins() & mask)
+    done = 0
+    for n in (1, 2, sweeps - 3):
+        g.sweep(n)
+        o.sweep(n)
+        done += n
+        if done == 3:
+            g.snapshot(0)
+            o.snapshot(0)
+        a, b = g.get_spins(), o.get_spins() & mask
+        assert np.array_equal(a, b), "L=%d M=%d after %d sweeps: %d words differ" % (L, M, done, int((a != b).sum()))
+    lanes = _used(int(mask), 64)
+    assert np.array_equal(g.energy()[lanes], o.energy()[lanes])
+    assert np.array_equal(g.magnetisation()[lanes], o.magnetisation()[lanes])
+    assert np.array_equal(g.autocorr(0)[lanes], o.autocorr(0)[lanes])
+    if n_rep == 2:
+        dis = _used(int(mask) & 0xFFFFFFFF, 32)
+        r_max = min(3, L // 2)
+        B, q = g.c4(r_max, with_q=True)
+        assert np.array_equal(B[:, :, dis], o.c4(r_max)[:, :, dis]) and np.array_equal(q[dis], o.overlap()[dis])
+        if L <= 32 or L in (64, 128):
+            assert np.array_equal(g.c4_vectors([(1, -2, 3)])[0][dis], o.c4_vector(1, -2, 3)[dis])
+
+
+def test_folded_sim_set_state_and_argument_errors():
+    L, M = 16, 16
+    g = binding.Sim(L, 0.5, 0.8, n_replicas=2, seed=1, n_slots=0, n_samples=M)
+    o = Oracle(L, 0.5, 0.8, n_replicas=2, seed=1, n_slots=0)
+    mask = np.uint64(g.lane_mask)
+    spins = wl.random_words(L ** 3, 5)
+    lo = wl.random_words(3 * L ** 3, 6) & np.uint64(0xFFFFFFFF)
+    bonds = lo | (lo << np.uint64(32))
+    g.set_spins(spins); g.set_bonds(bonds)          # unused lanes are dropped
+    o.set_spins(spins); o.set_bonds(bonds)
+    assert np.array_equal(g.get_spins(), spins & mask) and np.array_equal(g.get_bonds(), bonds & mask)
+    g.sweep(5); o.sweep(5)
+    assert np.array_equal(g.get_spins(), o.get_spins() & mask)
+    with pytest.raises(binding.EAError):
+        g.set_dynamics("heatbath")
+    with pytest.raises(binding.EAError):
+        g.kernel = "rows"
+    for bad in ((10, 32, 2), (16, 3, 2), (16, 1, 2), (8, 8, 2), (16, 128, 2)):   # L % 4, M not 2^m, M < 2 replicas, L M / 64 odd, M > 64
+        with pytest.raises(binding.EAError):
+            binding.Sim(bad[0], 0.5, 0.8, n_replicas=bad[2], n_samples=bad[1])
