@@ -119,7 +119,7 @@ struct FoldSweepArgs {
     uint64_t seed, t;
     const uint64_t *d_time;
     uint32_t t_offset;
-    uint64_t thr[3];      // full-width thresholds (2^32 = always)
+    Thresholds th;        // 32-bit thresholds + "always" flags (thr == 2^32, T = inf)
 };
 
 // flip word of one 64-bit multispin given the level masks m_k (bit set <=> that sample's number is below thr[k])
@@ -136,6 +136,7 @@ __device__ __forceinline__ uint64_t flip_word_masks(uint64_t s, uint64_t n1, uin
 }
 
 // one thread = two x-adjacent folded words of one colour (L % 4 == 0)
+template <bool ALWAYS>
 __global__ void __launch_bounds__(256) k_sweep_fold(const FoldSweepArgs a)
 {
     const FoldGeom f = a.f;
@@ -181,16 +182,32 @@ __global__ void __launch_bounds__(256) k_sweep_fold(const FoldSweepArgs a)
     const uint64_t time = (a.d_time ? *a.d_time : a.t) + a.t_offset;
     const SweepRng g = make_sweep_rng(a.seed, time, (uint32_t)a.colour);
     uint64_t m0a = 0, m1a = 0, m2a = 0, m0b = 0, m1b = 0, m2b = 0; // word 0 (a), word 1 (b)
+    uint64_t glo = f.g_lo, ghi = f.g_hi;                           // the slab's group bits, shifted by M per slab
     for (int kk = 0; kk < f.K; ++kk) {
         const uint32_t site0 = (4 * k + s) + L * (y + L * (z + kk * Lz));
         const uint4 r = sweep_random4(g, site0);
-        const int sh = f.M * kk;
-        m0a |= (((uint64_t)r.x < a.thr[0] ? f.g_lo : 0) | ((uint64_t)r.y < a.thr[0] ? f.g_hi : 0)) << sh;
-        m1a |= (((uint64_t)r.x < a.thr[1] ? f.g_lo : 0) | ((uint64_t)r.y < a.thr[1] ? f.g_hi : 0)) << sh;
-        m2a |= (((uint64_t)r.x < a.thr[2] ? f.g_lo : 0) | ((uint64_t)r.y < a.thr[2] ? f.g_hi : 0)) << sh;
-        m0b |= (((uint64_t)r.z < a.thr[0] ? f.g_lo : 0) | ((uint64_t)r.w < a.thr[0] ? f.g_hi : 0)) << sh;
-        m1b |= (((uint64_t)r.z < a.thr[1] ? f.g_lo : 0) | ((uint64_t)r.w < a.thr[1] ? f.g_hi : 0)) << sh;
-        m2b |= (((uint64_t)r.z < a.thr[2] ? f.g_lo : 0) | ((uint64_t)r.w < a.thr[2] ? f.g_hi : 0)) << sh;
+        // energy-raising moves are rare at low T: one branch per slab skips all the mask work when none of the four
+        // numbers is below thr[2] (thr[0] <= thr[1] <= thr[2])
+        if (ALWAYS || min(min(r.x, r.y), min(r.z, r.w)) < a.th.thr[2]) {
+            if (r.x < a.th.thr[2]) m2a |= glo;
+            if (r.y < a.th.thr[2]) m2a |= ghi;
+            if (r.z < a.th.thr[2]) m2b |= glo;
+            if (r.w < a.th.thr[2]) m2b |= ghi;
+            if (r.x < a.th.thr[1]) m1a |= glo;
+            if (r.y < a.th.thr[1]) m1a |= ghi;
+            if (r.z < a.th.thr[1]) m1b |= glo;
+            if (r.w < a.th.thr[1]) m1b |= ghi;
+            if (r.x < a.th.thr[0]) m0a |= glo;
+            if (r.y < a.th.thr[0]) m0a |= ghi;
+            if (r.z < a.th.thr[0]) m0b |= glo;
+            if (r.w < a.th.thr[0]) m0b |= ghi;
+        }
+        glo <<= f.M;
+        ghi <<= f.M;
+    }
+    if (ALWAYS) { // thr[k] == 2^32 (T = inf): certain, whatever the number
+        const uint64_t al0 = a.th.always[0] ? ~(uint64_t)0 : 0, al1 = a.th.always[1] ? ~(uint64_t)0 : 0, al2 = a.th.always[2] ? ~(uint64_t)0 : 0;
+        m0a |= al0; m0b |= al0; m1a |= al1; m1b |= al1; m2a |= al2; m2b |= al2;
     }
     ulonglong2 out;
     out.x = own.x ^ flip_word_masks(own.x, np0, nm0, Yp.x, Ym.x, Zp.x, Zm.x, jx.x, jm0, jy.x, by.x, jz.x, bz.x, m0a, m1a, m2a);
@@ -281,8 +298,9 @@ cudaError_t launch_half_sweep_fold(ea_sim *s, int parity, uint64_t t, const uint
     a.t = t;
     a.d_time = d_time;
     a.t_offset = t_offset;
-    for (int k = 0; k < 3; ++k) a.thr[k] = s->thr[k];
-    k_sweep_fold<<<blocks_for(a.f.Nhf / 2, 256), 256, 0, st>>>(a);
+    a.th = s->th;
+    if (a.th.always[0] | a.th.always[1] | a.th.always[2]) k_sweep_fold<true><<<blocks_for(a.f.Nhf / 2, 256), 256, 0, st>>>(a);
+    else k_sweep_fold<false><<<blocks_for(a.f.Nhf / 2, 256), 256, 0, st>>>(a);
     s->count_launch();
     s->unfolded_valid = false;
     return cudaGetLastError();
