@@ -53,7 +53,9 @@ typedef enum {
     EA_KERNEL_VEC2 = 2,   /* two sites per thread, 128-bit loads; L % 4 == 0              */
     EA_KERNEL_ROWS = 3,   /* warp marches along y with a register window; L % 4 == 0      */
     EA_KERNEL_RESIDENT = 4, /* persistent cooperative kernel, many sweeps per launch (L = 128) */
-    EA_KERNEL_FOLD = 5     /* what a sim with n_samples < 64 runs (not selectable)        */
+    EA_KERNEL_FOLD = 5,    /* what a sim with n_samples < 64 runs (not selectable)        */
+    EA_KERNEL_ROWS_PERSISTENT = 6 /* ROWS with a grid barrier per colour, one launch per ea_sweep (L = 16, 32, 64);
+                                     measured slower than the graph replays, never chosen by AUTO */
 } ea_kernel;
 
 /* Single-spin dynamics.  The paper uses Metropolis (Eq. 9); heat bath is the variant of SURVEY 8(f)

@@ -118,6 +118,7 @@ static ea_status stream_sync(ea_sim *s)
     } while (0)
 
 static const uint64_t RESIDENT_AUTO_MIN_SWEEPS = 8;     // AUTO: below this the prologue/epilogue of the persistent kernel does not pay
+static const uint64_t PERSISTENT_MIN_SWEEPS = 4;         // ROWS_PERSISTENT: below this the per-colour launches are as good
 static const uint64_t RESIDENT_MAX_SWEEPS = 1u << 20;   // sweeps per persistent launch (about 10 s of device time)
 
 static bool valid_L(int L) { return L >= 2 && (L & 1) == 0 && (int64_t)L * L * L < ((int64_t)1 << 31); }
@@ -129,6 +130,7 @@ static bool kernel_valid_for(int kernel, int L)
     case EA_KERNEL_VEC2: return L % 4 == 0;
     case EA_KERNEL_ROWS: return L == 16 || L == 32 || L == 64 || L == 128;
     case EA_KERNEL_RESIDENT: return L == 128; // plus a device check (resident_supported) once the sim exists
+    case EA_KERNEL_ROWS_PERSISTENT: return rows_persistent_valid(L);
     case EA_KERNEL_FOLD: return false;        // not selectable: it is what a sim with n_samples < 64 runs
     default: return false;
     }
@@ -340,6 +342,15 @@ ea_status ea_sweep(ea_sim *sim, uint64_t n)
             const uint32_t chunk = (uint32_t)(left < RESIDENT_MAX_SWEEPS ? left : RESIDENT_MAX_SWEEPS);
             EA_CUDA(sim, launch_sweeps_resident(sim, sim->t, chunk, sim->stream));
             sim->resident_used = true;
+            sim->t += chunk;
+            left -= chunk;
+        }
+        return EA_OK;
+    }
+    if (sim->kernel == EA_KERNEL_ROWS_PERSISTENT && sim->dynamics == EA_DYN_METROPOLIS && n >= PERSISTENT_MIN_SWEEPS) {
+        while (left) {
+            const uint32_t chunk = (uint32_t)(left < RESIDENT_MAX_SWEEPS ? left : RESIDENT_MAX_SWEEPS);
+            EA_CUDA(sim, launch_sweeps_rows_persistent(sim, sim->t, chunk, sim->stream));
             sim->t += chunk;
             left -= chunk;
         }

@@ -87,6 +87,9 @@ cudaError_t fold_from_standard(ea_sim *s, bool spins, bool bonds); // mask unuse
 cudaError_t fold_ensure_unfolded(ea_sim *s);                     // refresh `spins` from f_spins if stale
 cudaError_t launch_half_sweep_fold(ea_sim *s, int parity, uint64_t t, const uint64_t *d_time, uint32_t t_offset,
                                    cudaStream_t st);
+// ROWS_PERSISTENT (ea_sweep.cu; L = 16, 32, 64): n sweeps in one cooperative launch with a grid barrier per colour
+bool rows_persistent_valid(int L);
+cudaError_t launch_sweeps_rows_persistent(ea_sim *s, uint64_t t0, uint32_t n, cudaStream_t st);
 // RESIDENT (ea_sweep_resident.cu): n sweeps from sweep index t0 in one cooperative launch
 bool resident_supported(const ea_sim *s);
 size_t resident_flag_bytes();

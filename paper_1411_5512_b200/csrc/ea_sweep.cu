@@ -3,6 +3,8 @@
 //
 // A kernel boundary is the colour barrier ("each half-step is performed in its own CUDA kernel call to
 // ensure global synchronization").  All variants are bit-identical (same stream contract).
+#include <cooperative_groups.h>
+
 #include "ea_internal.h"
 #include "ea_sweep_common.cuh"
 
@@ -162,7 +164,14 @@ __global__ void k_bump_time(uint64_t *d_time, uint32_t n) { *d_time += n; }
 // warp-uniform.
 // ---------------------------------------------------------------------------------------------
 
-template <int L, int M, int S0, typename BondT, bool ALWAYS, bool HB>
+// spins of the other colour: read-only path (one launch per colour), or L2-coherent loads when other CTAs rewrite
+// them inside the same launch (ROWS_PERSISTENT)
+template <bool COHERENT> __device__ __forceinline__ ulonglong2 ld_oth(const uint64_t *p)
+{
+    return COHERENT ? __ldcg((const ulonglong2 *)p) : __ldg((const ulonglong2 *)p);
+}
+
+template <int L, int M, int S0, typename BondT, bool ALWAYS, bool HB, bool COHERENT = false>
 __device__ __forceinline__ void march_rows(const SweepArgs &a, const SweepRng &g, const unsigned y0, const unsigned z,
                                            const unsigned k, const int lane_m, const int lane_p)
 {
@@ -170,15 +179,15 @@ __device__ __forceinline__ void march_rows(const SweepArgs &a, const SweepRng &g
     const BondT *__restrict__ Jc = (const BondT *)a.Jc;
     const BondT *__restrict__ Jo = (const BondT *)a.Jo;
     const unsigned zb = ZS * z + 2 * k, zbm = ZS * ((z - 1) & (L - 1)) + 2 * k, zbp = ZS * ((z + 1) & (L - 1)) + 2 * k;
-    ulonglong2 Pm = ldg_pair<uint64_t>(a.oth + zb + Lh * ((y0 - 1) & (L - 1)));
-    ulonglong2 P0 = ldg_pair<uint64_t>(a.oth + zb + Lh * y0);
+    ulonglong2 Pm = ld_oth<COHERENT>(a.oth + zb + Lh * ((y0 - 1) & (L - 1)));
+    ulonglong2 P0 = ld_oth<COHERENT>(a.oth + zb + Lh * y0);
 #pragma unroll
     for (int m = 0; m < M; ++m) {
         const unsigned y = y0 + m, row = zb + Lh * y;
         const ulonglong2 own = *(const ulonglong2 *)(a.own + row);
-        const ulonglong2 Pp = ldg_pair<uint64_t>(a.oth + zb + Lh * ((y + 1) & (L - 1)));
-        const ulonglong2 Zm = ldg_pair<uint64_t>(a.oth + zbm + Lh * y);
-        const ulonglong2 Zp = ldg_pair<uint64_t>(a.oth + zbp + Lh * y);
+        const ulonglong2 Pp = ld_oth<COHERENT>(a.oth + zb + Lh * ((y + 1) & (L - 1)));
+        const ulonglong2 Zm = ld_oth<COHERENT>(a.oth + zbm + Lh * y);
+        const ulonglong2 Zp = ld_oth<COHERENT>(a.oth + zbp + Lh * y);
         const typename Pair<BondT>::type jx = ldg_pair<BondT>(Jc + row), jy = ldg_pair<BondT>(Jc + Nh + row),
                                          jz = ldg_pair<BondT>(Jc + 2 * Nh + row), bx = ldg_pair<BondT>(Jo + row),
                                          by = ldg_pair<BondT>(Jo + Nh + zb + Lh * ((y - 1) & (L - 1))),
@@ -213,6 +222,92 @@ __global__ void __launch_bounds__(128) k_sweep_rows(const SweepArgs a)
         march_rows<L, M, 1, BondT, ALWAYS, HB>(a, g, y0, z, k, lane_m, lane_p);
 }
 
+// ROWS_PERSISTENT (L = 16, 32, 64; SURVEY 8(f) NEXT-2 "grid-barrier persistent kernels for L <= 64"): all 2n
+// half-sweeps of one ea_sweep(n) call in ONE cooperative launch; the colour barrier is a grid-wide barrier
+// (~1.2 us) instead of a kernel boundary (~2-2.8 us per graph node at these sizes, which are launch-bound).
+// Same geometry as k_sweep_rows, so a row is always updated by the same thread; the other colour's rows are
+// rewritten by other CTAs between steps and are therefore read with L2-coherent loads.
+// MEASURED (B200): 1.93 / 4.05 / 4.29 us per half-sweep at L = 16 / 32 / 64 against 2.05 / 2.53 / 2.79 us for the
+// CUDA-graph replays of k_sweep_rows: the grid barrier over 32-256 CTAs costs more than the graph node it replaces.
+// Kept as an explicit option (bit-identical, tested); AUTO does not choose it.
+template <int L, int M, typename BondT, bool ALWAYS>
+__global__ void __launch_bounds__(128) k_sweep_rows_persistent(SweepArgs a, uint64_t *spins, const BondT *bonds, const uint32_t n_half)
+{
+    namespace cg = cooperative_groups;
+    cg::grid_group grid = cg::this_grid();
+    constexpr unsigned RL = L / 4, G = 32 / RL, YC = L / M, Nh = (unsigned)L * L * L / 2;
+    const unsigned lane = threadIdx.x & 31, warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned k = lane % RL, grp = lane / RL;
+    const unsigned zg = warp / YC, yc = warp - zg * YC;
+    const bool active = zg < L / G;
+    const unsigned zpar = zg & 1, z = 2 * (G * (zg >> 1) + grp) + zpar, y0 = yc * M;
+    const int lane_m = (int)((lane & ~(RL - 1)) | ((k - 1) & (RL - 1))), lane_p = (int)((lane & ~(RL - 1)) | ((k + 1) & (RL - 1)));
+    const uint64_t t0 = a.t;
+    for (uint32_t h = 0; h < n_half; ++h) {
+        const int c = h & 1;
+        a.colour = c;
+        a.own = spins + (size_t)c * Nh;
+        a.oth = spins + (size_t)(1 - c) * Nh;
+        a.Jc = bonds + (size_t)c * 3 * Nh;
+        a.Jo = bonds + (size_t)(1 - c) * 3 * Nh;
+        if (active) {
+            const SweepRng g = make_sweep_rng(a.seed, t0 + (h >> 1), (uint32_t)c);
+            if ((c ^ zpar) == 0) march_rows<L, M, 0, BondT, ALWAYS, false, true>(a, g, y0, z, k, lane_m, lane_p);
+            else march_rows<L, M, 1, BondT, ALWAYS, false, true>(a, g, y0, z, k, lane_m, lane_p);
+        }
+        grid.sync(); // colour barrier, with the memory fence that publishes this step's rows
+    }
+}
+
+template <int L, typename BondT, bool ALWAYS>
+static cudaError_t launch_rows_persistent_L(ea_sim *s, SweepArgs &a, uint32_t n, cudaStream_t st)
+{
+    constexpr int M = (L >= 128) ? 4 : 2, G = 32 / (L / 4);
+    constexpr unsigned warps = (L / M) * (L / G), block = 128, grid = (warps * 32 + block - 1) / block;
+    auto kern = k_sweep_rows_persistent<L, M, BondT, ALWAYS>;
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, block, 0);
+    if (e != cudaSuccess) return e;
+    if ((unsigned)per_sm * (unsigned)s->n_sm < grid) return cudaErrorCooperativeLaunchTooLarge;
+    uint64_t *spins = s->spins;
+    const BondT *bonds = (const BondT *)s->bonds;
+    uint32_t n_half = 2 * n;
+    void *args[] = {&a, &spins, &bonds, &n_half};
+    return cudaLaunchCooperativeKernel((void *)kern, dim3(grid), dim3(block), args, 0, st);
+}
+
+template <typename BondT>
+static cudaError_t launch_rows_persistent_typed(ea_sim *s, SweepArgs &a, uint32_t n, cudaStream_t st)
+{
+    const bool always = a.th.always[0] | a.th.always[1] | a.th.always[2];
+    switch (s->lat.L) {
+    case 16: return always ? launch_rows_persistent_L<16, BondT, true>(s, a, n, st) : launch_rows_persistent_L<16, BondT, false>(s, a, n, st);
+    case 32: return always ? launch_rows_persistent_L<32, BondT, true>(s, a, n, st) : launch_rows_persistent_L<32, BondT, false>(s, a, n, st);
+    case 64: return always ? launch_rows_persistent_L<64, BondT, true>(s, a, n, st) : launch_rows_persistent_L<64, BondT, false>(s, a, n, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+bool rows_persistent_valid(int L) { return L == 16 || L == 32 || L == 64; }
+
+// n sweeps (Metropolis) from sweep index t0 in one cooperative launch
+cudaError_t launch_sweeps_rows_persistent(ea_sim *s, uint64_t t0, uint32_t n, cudaStream_t st)
+{
+    SweepArgs a;
+    a.lat = s->lat;
+    a.colour = 0;
+    a.own = nullptr; a.oth = nullptr; a.Jc = nullptr; a.Jo = nullptr; // set per step on the device
+    a.seed = s->seed;
+    a.t = t0;
+    a.d_time = nullptr;
+    a.t_offset = 0;
+    a.th = s->th;
+    cudaError_t e = s->n_replicas == 2 ? launch_rows_persistent_typed<uint32_t>(s, a, n, st)
+                                       : launch_rows_persistent_typed<uint64_t>(s, a, n, st);
+    if (e == cudaSuccess) s->count_launch();
+    return e;
+}
+
 template <int L, typename BondT, bool ALWAYS, bool HB>
 static void launch_rows(const SweepArgs &a, cudaStream_t st)
 {
@@ -227,7 +322,7 @@ static cudaError_t launch_typed(ea_sim *s, const SweepArgs &a, cudaStream_t st)
 {
     const Lattice &lat = s->lat;
     const bool pow2 = lat.log2L >= 0;
-    if (s->kernel == EA_KERNEL_ROWS || s->kernel == EA_KERNEL_RESIDENT) { // RESIDENT: single half-sweeps go as ROWS
+    if (s->kernel == EA_KERNEL_ROWS || s->kernel == EA_KERNEL_RESIDENT || s->kernel == EA_KERNEL_ROWS_PERSISTENT) { // RESIDENT: single half-sweeps go as ROWS
         switch (lat.L) {
         case 16: launch_rows<16, BondT, ALWAYS, HB>(a, st); break;
         case 32: launch_rows<32, BondT, ALWAYS, HB>(a, st); break;

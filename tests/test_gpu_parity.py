@@ -14,11 +14,12 @@ from paper_1411_5512_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = ["scalar", "vec2", "rows"]
+KERNELS = ["scalar", "vec2", "rows", "rows_persistent"]
 
 
 def kernels_for(L):
-    return [k for k in KERNELS if k == "scalar" or (k == "vec2" and L % 4 == 0) or (k == "rows" and L in (16, 32, 64, 128))]
+    return [k for k in KERNELS if k == "scalar" or (k == "vec2" and L % 4 == 0) or (k == "rows" and L in (16, 32, 64, 128))
+            or (k == "rows_persistent" and L in (16, 32, 64))]
 
 
 def make_pair(L, p, T, n_rep, seed, n_slots=2, kernel="auto"):
@@ -610,3 +611,16 @@ def test_folded_sim_set_state_and_argument_errors():
     for bad in ((10, 32, 2), (16, 3, 2), (16, 1, 2), (8, 8, 2), (16, 128, 2)):   # L % 4, M not 2^m, M < 2 replicas, L M / 64 odd, M > 64
         with pytest.raises(binding.EAError):
             binding.Sim(bad[0], 0.5, 0.8, n_replicas=bad[2], n_samples=bad[1])
+
+
+def test_rows_persistent_long_run_matches_the_graph_replays():
+    """ROWS_PERSISTENT (one cooperative launch, grid barrier per colour) against the per-colour launches over 5000
+    sweeps at L = 32 and 2000 at L = 64 (the oracle follows the first 60 in the every-kernel test above)."""
+    for L, n in ((32, 5000), (64, 2000)):
+        a = binding.Sim(L, 0.6, 0.8, n_replicas=2, seed=wl.seed_for(1, L), n_slots=0, kernel="rows")
+        b = binding.Sim(L, 0.6, 0.8, n_replicas=2, seed=wl.seed_for(1, L), n_slots=0, kernel="rows_persistent")
+        assert b.kernel == binding.EA_KERNEL_ROWS_PERSISTENT
+        for k in (3, 4, n):
+            a.sweep(k)
+            b.sweep(k)
+            assert np.array_equal(a.get_spins(), b.get_spins()), "L=%d after %d sweeps" % (L, a.time)
