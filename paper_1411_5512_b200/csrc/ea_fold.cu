@@ -131,19 +131,37 @@ __device__ __forceinline__ uint64_t flip_word_masks(uint64_t s, uint64_t n1, uin
     const uint64_t sa = u1 ^ u2 ^ u3, ka = (u1 & u2) | (u3 & (u1 | u2));
     const uint64_t sb = u4 ^ u5 ^ u6, kb = (u4 & u5) | (u6 & (u4 | u5));
     const uint64_t t = sa | sb;
-    const uint64_t ge3 = (ka & kb) | (t & (ka | kb)), ge2 = ka | kb | (sa & sb), ge1 = ka | kb | t;
-    return ge3 | (m2 & ge2) | (m1 & ge1) | m0; // Eq. 9 with nested thresholds (see flip_half)
+    uint64_t f = (ka & kb) | (t & (ka | kb)); // [n_u >= 3]: Delta E <= 0, always flipped
+    if (m2) {                                 // some sample of this word drew a number below thr[2] (rare at low T)
+        const uint64_t ge2 = ka | kb | (sa & sb), ge1 = ka | kb | t;
+        f |= (m2 & ge2) | (m1 & ge1) | m0;    // Eq. 9 with nested thresholds (see flip_half): m0 <= m1 <= m2 bitwise
+    }
+    return f;
 }
 
 // one thread = two x-adjacent folded words of one colour (L % 4 == 0)
-template <bool ALWAYS>
+// MT = M as a compile-time constant (shifts and the slab loop unroll), or 0: taken from the arguments.
+// POW2: L is a power of two (index arithmetic by shifts).
+template <int MT, bool POW2, bool ALWAYS>
 __global__ void __launch_bounds__(256) k_sweep_fold(const FoldSweepArgs a)
 {
     const FoldGeom f = a.f;
+    const int M = MT ? MT : f.M, K = MT ? 64 / MT : f.K;
     const unsigned L = a.lat.L, Lh = a.lat.Lh, W = Lh >> 1, Lz = f.Lz;
     const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= f.Nhf / 2) return;
-    const unsigned k = tid % W, row = tid / W, y = row % L, z = row / L; // z = folded plane
+    unsigned k, y, z; // z = folded plane
+    if (POW2) {
+        k = tid & (W - 1);
+        const unsigned row = tid >> (a.lat.log2Lh - 1);
+        y = row & (L - 1);
+        z = row >> a.lat.log2L;
+    } else {
+        k = tid % W;
+        const unsigned row = tid / W;
+        y = row % L;
+        z = row / L;
+    }
     const unsigned s = (a.colour ^ (y + z)) & 1u;
     const unsigned yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
     const bool top = z + 1 == Lz, bottom = z == 0;
@@ -167,11 +185,11 @@ __global__ void __launch_bounds__(256) k_sweep_fold(const FoldSweepArgs a)
     const ulonglong2 by = *(const ulonglong2 *)(a.Jo + Nhf + iym);
     ulonglong2 bz = *(const ulonglong2 *)(a.Jo + 2 * Nhf + izm);
     if (top) { // slab k couples to slab k + 1 across the seam ("rotate the bits ... by M positions")
-        Zp.x = rotr64(Zp.x, f.M); Zp.y = rotr64(Zp.y, f.M);
+        Zp.x = rotr64(Zp.x, M); Zp.y = rotr64(Zp.y, M);
     }
     if (bottom) {
-        Zm.x = rotl64(Zm.x, f.M); Zm.y = rotl64(Zm.y, f.M);
-        bz.x = rotl64(bz.x, f.M); bz.y = rotl64(bz.y, f.M);
+        Zm.x = rotl64(Zm.x, M); Zm.y = rotl64(Zm.y, M);
+        bz.x = rotl64(bz.x, M); bz.y = rotl64(bz.y, M);
     }
     const uint64_t np0 = s ? A.y : A.x, nm0 = s ? A.x : ex;
     const uint64_t np1 = s ? ex : A.y, nm1 = s ? A.y : A.x;
@@ -183,7 +201,8 @@ __global__ void __launch_bounds__(256) k_sweep_fold(const FoldSweepArgs a)
     const SweepRng g = make_sweep_rng(a.seed, time, (uint32_t)a.colour);
     uint64_t m0a = 0, m1a = 0, m2a = 0, m0b = 0, m1b = 0, m2b = 0; // word 0 (a), word 1 (b)
     uint64_t glo = f.g_lo, ghi = f.g_hi;                           // the slab's group bits, shifted by M per slab
-    for (int kk = 0; kk < f.K; ++kk) {
+#pragma unroll(MT ? (64 / (MT ? MT : 1) <= 8 ? 64 / (MT ? MT : 1) : 4) : 1)
+    for (int kk = 0; kk < K; ++kk) {
         const uint32_t site0 = (4 * k + s) + L * (y + L * (z + kk * Lz));
         const uint4 r = sweep_random4(g, site0);
         // energy-raising moves are rare at low T: one branch per slab skips all the mask work when none of the four
@@ -202,8 +221,8 @@ __global__ void __launch_bounds__(256) k_sweep_fold(const FoldSweepArgs a)
             if (r.z < a.th.thr[0]) m0b |= glo;
             if (r.w < a.th.thr[0]) m0b |= ghi;
         }
-        glo <<= f.M;
-        ghi <<= f.M;
+        glo <<= M;
+        ghi <<= M;
     }
     if (ALWAYS) { // thr[k] == 2^32 (T = inf): certain, whatever the number
         const uint64_t al0 = a.th.always[0] ? ~(uint64_t)0 : 0, al1 = a.th.always[1] ? ~(uint64_t)0 : 0, al2 = a.th.always[2] ? ~(uint64_t)0 : 0;
@@ -299,8 +318,20 @@ cudaError_t launch_half_sweep_fold(ea_sim *s, int parity, uint64_t t, const uint
     a.d_time = d_time;
     a.t_offset = t_offset;
     a.th = s->th;
-    if (a.th.always[0] | a.th.always[1] | a.th.always[2]) k_sweep_fold<true><<<blocks_for(a.f.Nhf / 2, 256), 256, 0, st>>>(a);
-    else k_sweep_fold<false><<<blocks_for(a.f.Nhf / 2, 256), 256, 0, st>>>(a);
+    const bool always = a.th.always[0] | a.th.always[1] | a.th.always[2];
+    const unsigned grid = blocks_for(a.f.Nhf / 2, 256);
+    if (always || s->lat.log2L < 0) { // T = inf or L not a power of two: the generic kernel
+        if (always) k_sweep_fold<0, false, true><<<grid, 256, 0, st>>>(a);
+        else k_sweep_fold<0, false, false><<<grid, 256, 0, st>>>(a);
+    } else {
+        switch (a.f.M) {
+        case 32: k_sweep_fold<32, true, false><<<grid, 256, 0, st>>>(a); break;
+        case 16: k_sweep_fold<16, true, false><<<grid, 256, 0, st>>>(a); break;
+        case 8: k_sweep_fold<8, true, false><<<grid, 256, 0, st>>>(a); break;
+        case 4: k_sweep_fold<4, true, false><<<grid, 256, 0, st>>>(a); break;
+        default: k_sweep_fold<0, true, false><<<grid, 256, 0, st>>>(a); break;
+        }
+    }
     s->count_launch();
     s->unfolded_valid = false;
     return cudaGetLastError();
