@@ -624,3 +624,29 @@ def test_rows_persistent_long_run_matches_the_graph_replays():
             a.sweep(k)
             b.sweep(k)
             assert np.array_equal(a.get_spins(), b.get_spins()), "L=%d after %d sweeps" % (L, a.time)
+
+
+def test_ageing_protocol_driver_matches_the_oracle_step_by_step():
+    """The paper's protocol (t_w = 1, 10, 100; t on the {1, 2, 5} x 10^m grid) through paper_1411_5512_b200.ageing,
+    against the oracle driven by hand through the same schedule: cfg2's lattice (L = 32, 32 x 2)."""
+    from paper_1411_5512_b200 import ageing
+    c = wl.CONFIGS["cfg2"]
+    t_w, t_grid = [1, 10, 100], ageing.decade_grid(200)
+    assert t_grid == [1, 2, 5, 10, 20, 50, 100, 200]
+    g = binding.Sim(c.L, c.p, c.T, n_replicas=2, seed=c.seed, n_slots=3)
+    res = ageing.run(g, t_w, t_grid, r_max=8, shells_r_max=2)
+    o = Oracle(c.L, c.p, c.T, n_replicas=2, seed=c.seed, n_slots=3)
+    times = sorted(set(t_w) | {a + b for a in t_w for b in t_grid})
+    for when in times:
+        o.sweep(when - o.time)
+        if when in t_w:
+            i = t_w.index(when)
+            o.snapshot(i)
+            assert np.array_equal(res["E"][i], o.energy()) and np.array_equal(res["M"][i], o.magnetisation())
+            assert np.array_equal(res["B"][i], o.c4(8)) and np.array_equal(res["q"][i], o.overlap())
+            So, mo = o.c4_shells(2)
+            assert np.array_equal(res["S"][i], So) and np.array_equal(res["mult"][i], mo)
+        for i, tw in enumerate(t_w):
+            if when - tw in t_grid:
+                assert np.array_equal(res["A"][i][t_grid.index(when - tw)], o.autocorr(i)), (tw, when)
+    assert g.time == o.time == 300
