@@ -163,6 +163,10 @@ ea_status ea_get_bonds(ea_sim *sim, uint64_t *host);
 ea_status ea_set_bonds(ea_sim *sim, const uint64_t *host);
 ea_status ea_get_snapshot(ea_sim *sim, int slot, uint64_t *host);
 
+/* Host-only self-test (no device needed): the row schedules of the RESIDENT kernel -- every row of a tile exactly
+ * once, boundary rows first, consecutive rows of a warp alternating in parity.  EA_OK or EA_ERR_STATE. */
+ea_status ea_selftest_host(void);
+
 /* Philox4x32-10 block on the device (one thread), for the known-answer test of the GPU side (C-A6). */
 ea_status ea_philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 

@@ -66,6 +66,7 @@ SIGNATURES = {
     "ea_get_bonds": (_i, [_vp, _vp]),
     "ea_set_bonds": (_i, [_vp, _vp]),
     "ea_get_snapshot": (_i, [_vp, _i, _vp]),
+    "ea_selftest_host": (_i, []),
     "ea_philox_selftest": (_i, [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]),
     "ea_strerror": (C.c_char_p, [_i]),
     "ea_last_error": (C.c_char_p, [_vp]),

@@ -740,6 +740,9 @@ ea_status ea_set_bonds(ea_sim *sim, const uint64_t *host)
     return EA_OK;
 }
 
+/* Host-only consistency checks (no device): the RESIDENT row schedules. */
+ea_status ea_selftest_host(void) { return resident_tables_ok() ? EA_OK : EA_ERR_STATE; }
+
 ea_status ea_philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
 {
     if (!ctr || !key || !out) return EA_ERR_INVALID;

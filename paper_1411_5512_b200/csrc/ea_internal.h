@@ -93,6 +93,7 @@ cudaError_t launch_sweeps_rows_persistent(ea_sim *s, uint64_t t0, uint32_t n, cu
 // RESIDENT (ea_sweep_resident.cu): n sweeps from sweep index t0 in one cooperative launch
 bool resident_supported(const ea_sim *s);
 size_t resident_flag_bytes();
+bool resident_tables_ok();
 cudaError_t launch_sweeps_resident(ea_sim *s, uint64_t t0, uint32_t n, cudaStream_t st);
 
 // canonical <-> internal

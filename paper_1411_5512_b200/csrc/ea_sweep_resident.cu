@@ -461,6 +461,14 @@ bool resident_supported(const ea_sim *s)
            prop.sharedMemPerBlockOptin >= Geom128::SMEM_BYTES;
 }
 
+// host-only check of the row schedules of both geometries (every row once, boundary rows first, alternating parity)
+bool resident_tables_ok()
+{
+    RowTable<Geom128Of<uint32_t>::type> t32;
+    RowTable<Geom128Of<uint64_t>::type> t64;
+    return build_row_table<Geom128Of<uint32_t>::type>(t32) && build_row_table<Geom128Of<uint64_t>::type>(t64);
+}
+
 size_t resident_flag_bytes() { return (size_t)(Geom128::G * 32 + 32) * sizeof(unsigned); }
 
 // n sweeps starting at sweep index t0, one launch.  Asynchronous; ea_sim::resident_epoch advances by 2n.

@@ -129,3 +129,9 @@ def test_workspace_bytes_ex_validates_the_mixed_coding_parameters():
     for L, M, n_rep in ((10, 32, 2), (16, 3, 2), (16, 1, 2), (8, 8, 2), (16, 128, 2), (16, 0, 1)):
         assert f(L, M, n_rep, 1) == 0
     assert f(128, 1, 1, 0) > 0                                     # one sample, 64 slabs of two planes
+
+
+def test_resident_row_schedules_are_consistent_on_the_host():
+    """The RESIDENT kernel's host-built row tables satisfy their invariants; no device needed."""
+    from paper_1411_5512_b200 import binding
+    assert binding.lib().ea_selftest_host() == binding.EA_OK
