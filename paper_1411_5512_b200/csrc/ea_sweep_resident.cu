@@ -212,6 +212,9 @@ __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4
     constexpr int RPW = G::ROWS / G::CW;
     constexpr unsigned Nh = (unsigned)G::L * G::L * G::L / 2;
     static_assert(RPW % 2 == 0, "rows are taken two at a time (phases S0, 1 - S0)");
+    // a warp has NB_LO or NB_HI boundary rows: with the loop unrolled only those positions carry the publish store and
+    // the barrier arrive (an asm statement is a scheduling fence, so the other rows are free to interleave)
+    constexpr int NB_LO = G::NB / G::CW, NB_HI = (G::NB + G::CW - 1) / G::CW;
 #pragma unroll(G::UNROLL ? RPW / 2 : 1)
     for (int i = 0; i < RPW; i += 2) {
         const bool last = i + 2 >= RPW;
@@ -220,8 +223,8 @@ __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4
         const uint4 r0 = rnx;
         const RowBonds<BondT> b1 = load_row_bonds<BondT>(Jc_l, Jo_l, d1, Nh);
         const uint4 r1 = row_random(g, x.k, 1 - S0, d1);
-        resident_row<S0, G, BondT, ALWAYS, RARE>(x, d0, b0, r0, th, i < n_bnd);
-        if (i + 1 == n_bnd) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
+        resident_row<S0, G, BondT, ALWAYS, RARE>(x, d0, b0, r0, th, (!G::UNROLL || i < NB_HI) && i < n_bnd);
+        if ((!G::UNROLL || i + 1 == NB_LO || i + 1 == NB_HI) && i + 1 == n_bnd) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
         // the row after next; for the last pair that is the first row of the next half-step: the colours swap
         // roles, the stream moves on, and the phase of row 0 flips with the colour
         if (!last) {
@@ -231,8 +234,8 @@ __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4
             nxt = load_row_bonds<BondT>(Jo_l, Jc_l, d2, Nh);
             rnx = row_random(gn, x.k, 1 - S0, d2);
         }
-        resident_row<1 - S0, G, BondT, ALWAYS, RARE>(x, d1, b1, r1, th, i + 1 < n_bnd);
-        if (i + 2 == n_bnd) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
+        resident_row<1 - S0, G, BondT, ALWAYS, RARE>(x, d1, b1, r1, th, (!G::UNROLL || i + 1 < NB_HI) && i + 1 < n_bnd);
+        if ((!G::UNROLL || i + 2 == NB_LO || i + 2 == NB_HI) && i + 2 == n_bnd) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
     }
 }
 
