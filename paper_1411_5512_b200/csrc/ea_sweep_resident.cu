@@ -212,9 +212,11 @@ __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4
     constexpr int RPW = G::ROWS / G::CW;
     constexpr unsigned Nh = (unsigned)G::L * G::L * G::L / 2;
     static_assert(RPW % 2 == 0, "rows are taken two at a time (phases S0, 1 - S0)");
-    // a warp has NB_LO or NB_HI boundary rows: with the loop unrolled only those positions carry the publish store and
-    // the barrier arrive (an asm statement is a scheduling fence, so the other rows are free to interleave)
-    constexpr int NB_LO = G::NB / G::CW, NB_HI = (G::NB + G::CW - 1) / G::CW;
+    // a warp has at most NB_HI boundary rows (the slowest warps of the boundary phase have exactly NB_HI, and the
+    // producer waits for all of them): ONE arrive after row NB_HI - 1, and only the first NB_HI rows carry the publish
+    // store.  (An asm statement is a scheduling fence: every other row is free to interleave with its neighbours.)
+    constexpr int NB_HI = (G::NB + G::CW - 1) / G::CW;
+    static_assert(NB_HI >= 1 && NB_HI <= RPW, "the arrive must sit inside the row loop");
 #pragma unroll(G::UNROLL ? RPW / 2 : 1)
     for (int i = 0; i < RPW; i += 2) {
         const bool last = i + 2 >= RPW;
@@ -224,7 +226,7 @@ __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4
         const RowBonds<BondT> b1 = load_row_bonds<BondT>(Jc_l, Jo_l, d1, Nh);
         const uint4 r1 = row_random(g, x.k, 1 - S0, d1);
         resident_row<S0, G, BondT, ALWAYS, RARE>(x, d0, b0, r0, th, (!G::UNROLL || i < NB_HI) && i < n_bnd);
-        if ((!G::UNROLL || i + 1 == NB_LO || i + 1 == NB_HI) && i + 1 == n_bnd) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
+        if (i + 1 == NB_HI) named_bar_arrive(BAR_BOUNDARY, G::THREADS); // every warp's boundary rows are done by now
         // the row after next; for the last pair that is the first row of the next half-step: the colours swap
         // roles, the stream moves on, and the phase of row 0 flips with the colour
         if (!last) {
@@ -235,7 +237,7 @@ __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4
             rnx = row_random(gn, x.k, 1 - S0, d2);
         }
         resident_row<1 - S0, G, BondT, ALWAYS, RARE>(x, d1, b1, r1, th, (!G::UNROLL || i + 1 < NB_HI) && i + 1 < n_bnd);
-        if ((!G::UNROLL || i + 2 == NB_LO || i + 2 == NB_HI) && i + 2 == n_bnd) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
+        if (i + 2 == NB_HI) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
     }
 }
 
@@ -356,7 +358,6 @@ __global__ void __launch_bounds__(G::THREADS, 1) k_sweep_resident(const Resident
                 const unsigned parity = (h - 1) & 1;
                 while (!mbar_try_wait(halo_bar, parity)) { } // always completes: the producer arms it even on abort
             }
-            if (n_bnd == 0) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
             // y0, z0 are even, so the phase of row i is (c ^ phi ^ i) & 1
             if (((unsigned)c ^ phi) & 1u) resident_step<1, G, BondT, ALWAYS, RARE>(x, desc, n_bnd, nxt, rnx, Jc_l, Jo_l, g, gn, a.th);
             else resident_step<0, G, BondT, ALWAYS, RARE>(x, desc, n_bnd, nxt, rnx, Jc_l, Jo_l, g, gn, a.th);
