@@ -38,7 +38,7 @@ struct ResidentArgs {
     Thresholds th;
 };
 
-template <int L_, int TY_, int TZ_, int CW_, bool UNROLL_> struct ResidentGeom {
+template <int L_, int TY_, int TZ_, int CW_, int UNROLL_> struct ResidentGeom {
     static constexpr int L = L_, TY = TY_, TZ = TZ_;
     static constexpr int Lh = L / 2;                 // words per colour row
     static constexpr int NTY = L / TY, NTZ = L / TZ; // tiles along y, z
@@ -46,7 +46,7 @@ template <int L_, int TY_, int TZ_, int CW_, bool UNROLL_> struct ResidentGeom {
     static constexpr int ROWS = TY * TZ;             // rows updated per CTA per half-step
     static constexpr int HY = TY + 2, HZ = TZ + 2;   // with halo ring
     static constexpr int CW = CW_;                   // compute warps
-    static constexpr bool UNROLL = UNROLL_;          // unroll the row loop of a half-step (code size vs. selects)
+    static constexpr int UNROLL = UNROLL_;           // row pairs unrolled per loop iteration of a half-step (code size vs. scheduling freedom)
     static constexpr int THREADS = (CW + 1) * 32;    // + one producer warp
     static constexpr int NB = ROWS - (TY - 2) * (TZ - 2); // boundary rows
     static constexpr unsigned HALO_BYTES = (2 * TY + 2 * TZ) * Lh * 8;
@@ -217,7 +217,7 @@ __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4
     // store.  (An asm statement is a scheduling fence: every other row is free to interleave with its neighbours.)
     constexpr int NB_HI = (G::NB + G::CW - 1) / G::CW;
     static_assert(NB_HI >= 1 && NB_HI <= RPW, "the arrive must sit inside the row loop");
-#pragma unroll(G::UNROLL ? RPW / 2 : 1)
+#pragma unroll(G::UNROLL)
     for (int i = 0; i < RPW; i += 2) {
         const bool last = i + 2 >= RPW;
         const uint4 d0 = desc[i], d1 = desc[i + 1], d2 = desc[last ? 0 : i + 2];
@@ -225,7 +225,7 @@ __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4
         const uint4 r0 = rnx;
         const RowBonds<BondT> b1 = load_row_bonds<BondT>(Jc_l, Jo_l, d1, Nh);
         const uint4 r1 = row_random(g, x.k, 1 - S0, d1);
-        resident_row<S0, G, BondT, ALWAYS, RARE>(x, d0, b0, r0, th, (!G::UNROLL || i < NB_HI) && i < n_bnd);
+        resident_row<S0, G, BondT, ALWAYS, RARE>(x, d0, b0, r0, th, (G::UNROLL * 2 < RPW || i < NB_HI) && i < n_bnd);
         if (i + 1 == NB_HI) named_bar_arrive(BAR_BOUNDARY, G::THREADS); // every warp's boundary rows are done by now
         // the row after next; for the last pair that is the first row of the next half-step: the colours swap
         // roles, the stream moves on, and the phase of row 0 flips with the colour
@@ -236,7 +236,7 @@ __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4
             nxt = load_row_bonds<BondT>(Jo_l, Jc_l, d2, Nh);
             rnx = row_random(gn, x.k, 1 - S0, d2);
         }
-        resident_row<1 - S0, G, BondT, ALWAYS, RARE>(x, d1, b1, r1, th, (!G::UNROLL || i + 1 < NB_HI) && i + 1 < n_bnd);
+        resident_row<1 - S0, G, BondT, ALWAYS, RARE>(x, d1, b1, r1, th, (G::UNROLL * 2 < RPW || i + 1 < NB_HI) && i + 1 < n_bnd);
         if (i + 2 == NB_HI) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
     }
 }
@@ -431,10 +431,11 @@ template <typename G> static bool build_row_table(RowTable<G> &t)
 }
 
 // ---------------------------------------------------------------------------------------------
-// 32-bit bond words (2 replicas): 16 compute warps, row loop unrolled (89 -> 96 registers, no spills).
-// 64-bit bond words: twice the bond registers in flight, so 8 compute warps with up to 168 registers each.
-template <typename BondT> struct Geom128Of { typedef ResidentGeom<128, 16, 8, 16, true> type; };
-template <> struct Geom128Of<uint64_t> { typedef ResidentGeom<128, 16, 8, 8, false> type; };
+// 32-bit bond words (2 replicas): 16 compute warps of 96 registers.  64-bit bond words: twice the bond registers in
+// flight, so 8 compute warps with up to 168 registers each.  Both unroll two row pairs per loop iteration: measured
+// best (4.83 / 6.14 us per half-sweep; no unrolling 5.3 / 6.4, full unrolling 4.91 / 9.2 -- instruction cache).
+template <typename BondT> struct Geom128Of { typedef ResidentGeom<128, 16, 8, 16, 2> type; };
+template <> struct Geom128Of<uint64_t> { typedef ResidentGeom<128, 16, 8, 8, 2> type; };
 typedef Geom128Of<uint32_t>::type Geom128; // tile shape, grid and flag layout are the same for both
 
 template <typename BondT, bool ALWAYS, bool RARE>
