@@ -52,7 +52,7 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only if 
 #   alu_inst = sm__inst_executed_pipe_alu.sum per half-sweep (warp instructions on the LOP3/ISETP pipe).
 NCU = {
     "rows": {"traffic": 41996032, "alu_inst": None, "profile": "profiles/r01_ncu_full_k_sweep_rows.md"},
-    "resident": {"traffic": 42020000 + 169200, "alu_inst": 649821868 / 400.0,  # profiles/r01_launches_resident.md
+    "resident": {"traffic": 42000000 + 255000, "alu_inst": 631011472 / 400.0,  # profiles/r01_launches_resident.md
                  "profile": "profiles/r01_ncu_full_k_sweep_resident.md"},
 }
 # alu pipe: one warp instruction per 2 clocks per SM sub-partition (B300_MICROARCH "Pipe rates": rt_SMSP = 2),
