@@ -650,3 +650,17 @@ def test_ageing_protocol_driver_matches_the_oracle_step_by_step():
             if when - tw in t_grid:
                 assert np.array_equal(res["A"][i][t_grid.index(when - tw)], o.autocorr(i)), (tw, when)
     assert g.time == o.time == 300
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("EA_LONG_PARITY"), reason="long horizons: set EA_LONG_PARITY=1 (minutes of oracle time)")
+@pytest.mark.parametrize("name,sweeps", [("cfg2", 10 ** 5), ("cfg3a", 3000), ("cfg4", 300)])
+def test_long_horizon_parity(name, sweeps):
+    """cfg2 over its full 10^5 sweeps, cfg3 over 3000, cfg4 over 300 -- every spin word at the end and at
+    log-spaced times on the way, AUTO kernels (ROWS graph replays / RESIDENT)."""
+    c = wl.CONFIGS[name]
+    g, o = make_pair(c.L, c.p, c.T, c.n_replicas, c.seed, n_slots=1)
+    for t in [t for t in wl.log_spaced_times(sweeps) if t >= 10]:
+        g.sweep(t - g.time)
+        o.sweep(t - o.time)
+        assert_same_state(g, o, "%s t=%d" % (name, t))
+    assert_same_observables(g, o)
