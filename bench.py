@@ -142,6 +142,14 @@ def time_oracle(cfg, S, steps, warmup):
         o.sweep(1)
         per.append(time.perf_counter() - t0)
     t_sweep = float(np.mean(per))
+    # also one thread (the lanes are run one after the other), two sweeps
+    t_one = None
+    if hasattr(oracle, "set_threads"):
+        oracle.set_threads(1)
+        t0 = time.perf_counter()
+        o.sweep(2)
+        t_one = (time.perf_counter() - t0) / 2
+        oracle.set_threads(cores)
     # one measure point; C_4 on bytes is the slow part (3 (L/2+1) passes over 32 N bytes), so it is timed on a
     # bounded sample -- r = 1 on each of the 3 axes -- and scaled by (L/2 + 1) (every r costs the same loop)
     t0 = time.perf_counter()
@@ -166,8 +174,11 @@ def time_oracle(cfg, S, steps, warmup):
               "%d timed single sweeps of %s (L=%d) after %d warm-up sweeps, mean %.3f s/sweep; one measure point "
               "(snapshot, C, E, M; %s) %.3f s; value = (S*t_sweep + t_obs)/(S*N*64) at S=%d"
               % (steps, cfg.name, cfg.L, warmup, t_sweep, c4_note, t_obs, S))
-    return {"value": ps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
-            "s_per_sweep": t_sweep, "s_per_measure_point": t_obs}, step_s
+    out = {"value": ps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+           "s_per_sweep": t_sweep, "s_per_measure_point": t_obs}
+    if t_one is not None:
+        out["one_thread"] = {"s_per_sweep": t_one, "ps_per_attempt_sweeps_only": 1e12 * t_one / (cfg.N * LANES)}
+    return out, step_s
 
 
 def run_reference(args, cfg):
@@ -366,7 +377,7 @@ def run_ours(args, cfg):
     cpu_baseline = None
     if ws == 1 and not args.no_cpu_baseline:
         base, _ = time_oracle(cfg, S, steps=args.cpu_sweeps, warmup=1)
-        cpu_baseline = {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        cpu_baseline = {k: base[k] for k in ("value", "unit", "cores", "kind", "sample", "one_thread") if k in base}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": W,
