@@ -337,7 +337,7 @@ ea_status ea_sweep(ea_sim *sim, uint64_t n)
     DeviceGuard g(sim->device);
     uint64_t left = n;
     if (n && sim->n_samples < EA_LANES) sim->unfolded_valid = false; // the standard-layout mirror goes stale
-    if (sim->kernel == EA_KERNEL_RESIDENT && sim->dynamics == EA_DYN_METROPOLIS && n >= sim->resident_min_sweeps) {
+    if (sim->kernel == EA_KERNEL_RESIDENT && n >= sim->resident_min_sweeps) {
         while (left) {
             const uint32_t chunk = (uint32_t)(left < RESIDENT_MAX_SWEEPS ? left : RESIDENT_MAX_SWEEPS);
             EA_CUDA(sim, launch_sweeps_resident(sim, sim->t, chunk, sim->stream));

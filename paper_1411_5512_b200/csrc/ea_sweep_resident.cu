@@ -183,7 +183,7 @@ __device__ __forceinline__ uint4 row_random(const SweepRng &g, const unsigned k,
 }
 
 // one row of colour c with compile-time phase S; publishes it to global when `publish`
-template <int S, typename G, typename BondT, bool ALWAYS, bool RARE>
+template <int S, typename G, typename BondT, bool ALWAYS, bool RARE, bool HB>
 __device__ __forceinline__ void resident_row(const ResidentStep &x, const uint4 d, const RowBonds<BondT> &bd,
                                              const uint4 r, const Thresholds &th, const bool publish)
 {
@@ -196,7 +196,7 @@ __device__ __forceinline__ void resident_row(const ResidentStep &x, const uint4 
     const ulonglong2 Pp = *(const ulonglong2 *)(o + ROWB);
     const ulonglong2 Zm = *(const ulonglong2 *)(o - PLANEB);
     const ulonglong2 Zp = *(const ulonglong2 *)(o + PLANEB);
-    const ulonglong2 out = update_pair_r<S, BondT, ALWAYS, RARE>(own, P0, Pm, Pp, Zm, Zp, bd.jx, bd.jy, bd.jz, bd.bx, bd.by,
+    const ulonglong2 out = update_pair_r<S, BondT, ALWAYS, RARE, HB>(own, P0, Pm, Pp, Zm, Zp, bd.jx, bd.jy, bd.jz, bd.bx, bd.by,
                                                                  bd.bz, r, th, x.lane_m, x.lane_p);
     *(ulonglong2 *)own_row = out;
     if (publish) *x.g_own.at<ulonglong2>(d.y / 2) = out;
@@ -204,7 +204,7 @@ __device__ __forceinline__ void resident_row(const ResidentStep &x, const uint4 
 
 // all rows of one compute warp for one half-step; S0 = phase of the warp's first row.  Carried across rows and
 // steps: nxt = bond words of the next row, rnx = random numbers of the next row (gn = stream of the next step).
-template <int S0, typename G, typename BondT, bool ALWAYS, bool RARE>
+template <int S0, typename G, typename BondT, bool ALWAYS, bool RARE, bool HB>
 __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4 *__restrict__ desc, const int n_bnd,
                                               RowBonds<BondT> &nxt, uint4 &rnx, const Ptr32 Jc_l, const Ptr32 Jo_l,
                                               const SweepRng &g, const SweepRng &gn, const Thresholds &th)
@@ -225,7 +225,7 @@ __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4
         const uint4 r0 = rnx;
         const RowBonds<BondT> b1 = load_row_bonds<BondT>(Jc_l, Jo_l, d1, Nh);
         const uint4 r1 = row_random(g, x.k, 1 - S0, d1);
-        resident_row<S0, G, BondT, ALWAYS, RARE>(x, d0, b0, r0, th, (G::UNROLL * 2 < RPW || i < NB_HI) && i < n_bnd);
+        resident_row<S0, G, BondT, ALWAYS, RARE, HB>(x, d0, b0, r0, th, (G::UNROLL * 2 < RPW || i < NB_HI) && i < n_bnd);
         if (i + 1 == NB_HI) named_bar_arrive(BAR_BOUNDARY, G::THREADS); // every warp's boundary rows are done by now
         // the row after next; for the last pair that is the first row of the next half-step: the colours swap
         // roles, the stream moves on, and the phase of row 0 flips with the colour
@@ -236,12 +236,12 @@ __device__ __forceinline__ void resident_step(const ResidentStep &x, const uint4
             nxt = load_row_bonds<BondT>(Jo_l, Jc_l, d2, Nh);
             rnx = row_random(gn, x.k, 1 - S0, d2);
         }
-        resident_row<1 - S0, G, BondT, ALWAYS, RARE>(x, d1, b1, r1, th, (G::UNROLL * 2 < RPW || i + 1 < NB_HI) && i + 1 < n_bnd);
+        resident_row<1 - S0, G, BondT, ALWAYS, RARE, HB>(x, d1, b1, r1, th, (G::UNROLL * 2 < RPW || i + 1 < NB_HI) && i + 1 < n_bnd);
         if (i + 2 == NB_HI) named_bar_arrive(BAR_BOUNDARY, G::THREADS);
     }
 }
 
-template <typename G, typename BondT, bool ALWAYS, bool RARE>
+template <typename G, typename BondT, bool ALWAYS, bool RARE, bool HB>
 __global__ void __launch_bounds__(G::THREADS, 1) k_sweep_resident(const ResidentArgs a, const RowTable<G> tab)
 {
     constexpr int L = G::L, Lh = G::Lh, TY = G::TY, TZ = G::TZ, HY = G::HY, HZ = G::HZ, CW = G::CW, ROWS = G::ROWS;
@@ -359,8 +359,8 @@ __global__ void __launch_bounds__(G::THREADS, 1) k_sweep_resident(const Resident
                 while (!mbar_try_wait(halo_bar, parity)) { } // always completes: the producer arms it even on abort
             }
             // y0, z0 are even, so the phase of row i is (c ^ phi ^ i) & 1
-            if (((unsigned)c ^ phi) & 1u) resident_step<1, G, BondT, ALWAYS, RARE>(x, desc, n_bnd, nxt, rnx, Jc_l, Jo_l, g, gn, a.th);
-            else resident_step<0, G, BondT, ALWAYS, RARE>(x, desc, n_bnd, nxt, rnx, Jc_l, Jo_l, g, gn, a.th);
+            if (((unsigned)c ^ phi) & 1u) resident_step<1, G, BondT, ALWAYS, RARE, HB>(x, desc, n_bnd, nxt, rnx, Jc_l, Jo_l, g, gn, a.th);
+            else resident_step<0, G, BondT, ALWAYS, RARE, HB>(x, desc, n_bnd, nxt, rnx, Jc_l, Jo_l, g, gn, a.th);
             named_bar_sync(BAR_STEP, CW * 32); // colour c of the tile is complete before anyone reads it
         }
         // ---- epilogue: interior rows were never stored; write them back (boundary rows are current) ----
@@ -438,7 +438,7 @@ template <typename BondT> struct Geom128Of { typedef ResidentGeom<128, 16, 8, 16
 template <> struct Geom128Of<uint64_t> { typedef ResidentGeom<128, 16, 8, 8, 2> type; };
 typedef Geom128Of<uint32_t>::type Geom128; // tile shape, grid and flag layout are the same for both
 
-template <typename BondT, bool ALWAYS, bool RARE>
+template <typename BondT, bool ALWAYS, bool RARE, bool HB = false>
 static cudaError_t launch_resident_typed(ea_sim *s, ResidentArgs &a, cudaStream_t st)
 {
     typedef typename Geom128Of<BondT>::type G;
@@ -446,7 +446,7 @@ static cudaError_t launch_resident_typed(ea_sim *s, ResidentArgs &a, cudaStream_
     static RowTable<G> tab;
     static const bool tab_ok = build_row_table<G>(tab);
     if (!tab_ok) return cudaErrorInvalidConfiguration;
-    auto kern = k_sweep_resident<G, BondT, ALWAYS, RARE>;
+    auto kern = k_sweep_resident<G, BondT, ALWAYS, RARE, HB>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     void *args[] = {&a, &tab};
@@ -494,7 +494,10 @@ cudaError_t launch_sweeps_resident(ea_sim *s, uint64_t t0, uint32_t n, cudaStrea
     // low temperature: energy-raising moves are rare enough for a warp-level branch (see metropolis_word)
     const bool rare = !always && a.th.thr[2] < RARE_THR2_MAX;
     cudaError_t e;
-    if (s->n_replicas == 2)
+    if (s->dynamics == EA_DYN_HEATBATH) // heat bath (C-HB) carries its own always-masks; no rare branch
+        e = s->n_replicas == 2 ? launch_resident_typed<uint32_t, false, false, true>(s, a, st)
+                               : launch_resident_typed<uint64_t, false, false, true>(s, a, st);
+    else if (s->n_replicas == 2)
         e = always ? launch_resident_typed<uint32_t, true, false>(s, a, st)
             : rare ? launch_resident_typed<uint32_t, false, true>(s, a, st)
                    : launch_resident_typed<uint32_t, false, false>(s, a, st);

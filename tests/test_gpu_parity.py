@@ -535,10 +535,11 @@ def test_heatbath_sweeps_bit_exact_every_kernel(L, n_rep, T, sweeps):
 
 
 def test_switching_dynamics_mid_run_and_auto_kernel_at_L128():
-    """Metropolis (RESIDENT at L = 128) -> heat bath (per-colour launches) -> Metropolis, same sim, same clock."""
+    """Metropolis -> heat bath -> Metropolis on one sim at L = 128 (RESIDENT for the 8-sweep calls of either rule, ROWS for
+    the 2-sweep call), same clock."""
     c = wl.CONFIGS["cfg4"]
     g, o = make_pair(c.L, c.p, c.T, c.n_replicas, c.seed, n_slots=0)
-    for dyn, n in (("metropolis", 8), ("heatbath", 2), ("metropolis", 8)):
+    for dyn, n in (("metropolis", 8), ("heatbath", 2), ("heatbath", 9), ("metropolis", 8)):
         g.set_dynamics(dyn)
         o.set_dynamics(dyn)
         g.sweep(n)
