@@ -163,6 +163,16 @@ ea_status ea_get_bonds(ea_sim *sim, uint64_t *host);
 ea_status ea_set_bonds(ea_sim *sim, const uint64_t *host);
 ea_status ea_get_snapshot(ea_sim *sim, int slot, uint64_t *host);
 
+/* Batches: K independent small sims -- one L in {16, 32, 64}, one replica mode, 64 samples, one
+ * device, one dynamics; each with its own p, T, seed and clock -- advanced by ONE kernel launch per colour for all of
+ * them (such lattices are launch-bound alone).  ea_batch_sweep(b, n) is exactly ea_sweep(sim, n) on every member;
+ * the members stay ordinary sims (observables, get/set, ea_sweep still work, correctly ordered across streams).
+ * The batch runs on the first member's stream.  Destroy the batch before its members. */
+typedef struct ea_batch ea_batch;
+ea_status ea_batch_create(ea_sim *const *sims, int n_sims, ea_batch **out);
+ea_status ea_batch_sweep(ea_batch *batch, uint64_t n);
+ea_status ea_batch_destroy(ea_batch *batch);
+
 /* Host-only self-test (no device needed): the row schedules of the RESIDENT kernel -- every row of a tile exactly
  * once, boundary rows first, consecutive rows of a warp alternating in parity.  EA_OK or EA_ERR_STATE. */
 ea_status ea_selftest_host(void);

@@ -66,6 +66,9 @@ SIGNATURES = {
     "ea_get_bonds": (_i, [_vp, _vp]),
     "ea_set_bonds": (_i, [_vp, _vp]),
     "ea_get_snapshot": (_i, [_vp, _i, _vp]),
+    "ea_batch_create": (_i, [_vp, _i, C.POINTER(_vp)]),
+    "ea_batch_sweep": (_i, [_vp, _u64]),
+    "ea_batch_destroy": (_i, [_vp]),
     "ea_selftest_host": (_i, []),
     "ea_philox_selftest": (_i, [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]),
     "ea_strerror": (C.c_char_p, [_i]),
@@ -290,6 +293,37 @@ class Sim:
         w = np.zeros(self.N, dtype=np.uint64)
         self._ck(lib().ea_get_snapshot(self._h, int(slot), _ptr(w)))
         return w
+
+
+class Batch:
+    """K small sims (L = 16, 32, 64) advanced by one launch per colour (ea_batch_*).  The members stay usable."""
+
+    def __init__(self, sims):
+        self.sims = list(sims)
+        arr = (_vp * len(self.sims))(*[s._h for s in self.sims])
+        self._h = _vp()
+        st = lib().ea_batch_create(arr, len(self.sims), C.byref(self._h))
+        if st != EA_OK:
+            self._h = _vp()
+            raise EAError(st, lib().ea_strerror(st).decode() + " (ea_batch_create)")
+
+    def sweep(self, n=1):
+        if int(n) < 0:
+            raise ValueError("sweep count must be >= 0")
+        st = lib().ea_batch_sweep(self._h, int(n))
+        if st != EA_OK:
+            raise EAError(st, lib().ea_last_error(self.sims[0]._h).decode())
+
+    def close(self):
+        if self._h:
+            lib().ea_batch_destroy(self._h)
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def c4_curve(S, mult, N, r_lim):

@@ -743,6 +743,144 @@ ea_status ea_set_bonds(ea_sim *sim, const uint64_t *host)
 /* Host-only consistency checks (no device): the RESIDENT row schedules. */
 ea_status ea_selftest_host(void) { return resident_tables_ok() ? EA_OK : EA_ERR_STATE; }
 
+// ---- batches of small sims (one launch per colour for all of them) ---------------------------------
+
+struct ea_batch {
+    std::vector<ea_sim *> sims;
+    int L = 0, n_replicas = 0, device = 0;
+    cudaStream_t stream = nullptr; // the first sim's stream
+    char *d_args = nullptr;        // [2][K] launch arguments (parity-major)
+    uint64_t **d_times = nullptr;  // [K] the sims' device clocks
+    cudaEvent_t ev = nullptr;
+    cudaGraphExec_t graph_exec = nullptr;
+    bool graph_always = false, graph_hb = false;
+    std::vector<char> h_args;
+};
+
+static void batch_free(ea_batch *b)
+{
+    if (b->graph_exec) cudaGraphExecDestroy(b->graph_exec);
+    if (b->d_args) cudaFree(b->d_args);
+    if (b->d_times) cudaFree(b->d_times);
+    if (b->ev) cudaEventDestroy(b->ev);
+    delete b;
+}
+
+ea_status ea_batch_create(ea_sim *const *sims, int n_sims, ea_batch **out)
+{
+    if (!sims || !out || n_sims < 1 || n_sims > 65535) return EA_ERR_INVALID;
+    for (int i = 0; i < n_sims; ++i) {
+        if (!sims[i]) return EA_ERR_INVALID;
+        for (int j = 0; j < i; ++j)
+            if (sims[j] == sims[i]) return EA_ERR_INVALID;
+        if (sims[i]->lat.L != sims[0]->lat.L || sims[i]->n_replicas != sims[0]->n_replicas || sims[i]->device != sims[0]->device ||
+            sims[i]->n_samples != EA_LANES)
+            EA_FAIL(sims[i], EA_ERR_INVALID, "a batch needs sims of one L, one replica mode, 64 samples, one device");
+    }
+    if (!rows_persistent_valid(sims[0]->lat.L)) EA_FAIL(sims[0], EA_ERR_INVALID, "batches are for L = 16, 32, 64 (larger lattices fill the device alone)");
+    ea_batch *b = new (std::nothrow) ea_batch();
+    if (!b) return EA_ERR_NOMEM;
+    b->sims.assign(sims, sims + n_sims);
+    b->L = sims[0]->lat.L;
+    b->n_replicas = sims[0]->n_replicas;
+    b->device = sims[0]->device;
+    b->stream = sims[0]->stream;
+    DeviceGuard g(b->device);
+    const size_t K = (size_t)n_sims;
+    std::vector<uint64_t *> h_times(K);
+    for (size_t i = 0; i < K; ++i) h_times[i] = sims[i]->d_time;
+    b->h_args.resize(2 * K * batch_args_bytes());
+    if (cudaMalloc((void **)&b->d_args, b->h_args.size()) != cudaSuccess || cudaMalloc((void **)&b->d_times, K * sizeof(uint64_t *)) != cudaSuccess ||
+        cudaEventCreateWithFlags(&b->ev, cudaEventDisableTiming) != cudaSuccess ||
+        cudaMemcpy(b->d_times, h_times.data(), K * sizeof(uint64_t *), cudaMemcpyHostToDevice) != cudaSuccess) {
+        batch_free(b);
+        return EA_ERR_NOMEM;
+    }
+    *out = b;
+    return EA_OK;
+}
+
+ea_status ea_batch_destroy(ea_batch *b)
+{
+    if (!b) return EA_OK;
+    DeviceGuard g(b->device);
+    cudaStreamSynchronize(b->stream);
+    batch_free(b);
+    return EA_OK;
+}
+
+static cudaError_t batch_half_sweeps(ea_batch *b, bool always, bool hb, uint32_t k)
+{
+    const unsigned K = (unsigned)b->sims.size();
+    const char *a0 = b->d_args, *a1 = b->d_args + (size_t)K * batch_args_bytes();
+    cudaError_t e = launch_half_sweep_batch(b->L, b->n_replicas, always, hb, a0, K, k, b->stream);
+    if (e == cudaSuccess) e = launch_half_sweep_batch(b->L, b->n_replicas, always, hb, a1, K, k, b->stream);
+    return e;
+}
+
+ea_status ea_batch_sweep(ea_batch *b, uint64_t n)
+{
+    if (!b) return EA_ERR_INVALID;
+    ea_sim *s0 = b->sims[0];
+    const size_t K = b->sims.size(), az = batch_args_bytes();
+    bool always = false;
+    const bool hb = s0->dynamics == EA_DYN_HEATBATH;
+    for (ea_sim *s : b->sims) {
+        if (s->dynamics != s0->dynamics) EA_FAIL(s0, EA_ERR_STATE, "the sims of a batch must share the dynamics");
+        always |= (s->th.always[0] | s->th.always[1] | s->th.always[2]) != 0;
+    }
+    if (!n) return EA_OK;
+    DeviceGuard g(b->device);
+    for (size_t i = 0; i < K; ++i) { // temperatures may have changed: the arguments are rebuilt every call
+        fill_batch_args(b->sims[i], 0, b->h_args.data() + i * az);
+        fill_batch_args(b->sims[i], 1, b->h_args.data() + (K + i) * az);
+    }
+    for (size_t i = 1; i < K; ++i) // the batch runs on the first sim's stream, behind whatever the others have queued
+        if (b->sims[i]->stream != b->stream) {
+            EA_CUDA(s0, cudaEventRecord(b->ev, b->sims[i]->stream));
+            EA_CUDA(s0, cudaStreamWaitEvent(b->stream, b->ev, 0));
+        }
+    EA_CUDA(s0, cudaMemcpyAsync(b->d_args, b->h_args.data(), b->h_args.size(), cudaMemcpyHostToDevice, b->stream));
+    for (ea_sim *s : b->sims) EA_CUDA(s0, cudaMemcpyAsync(s->d_time, &s->t, 8, cudaMemcpyHostToDevice, b->stream));
+    uint64_t left = n;
+    if (left >= (uint64_t)GRAPH_SWEEPS) {
+        if (!b->graph_exec || b->graph_always != always || b->graph_hb != hb) {
+            if (b->graph_exec) cudaGraphExecDestroy(b->graph_exec);
+            b->graph_exec = nullptr;
+            cudaGraph_t graph = nullptr;
+            EA_CUDA(s0, cudaStreamBeginCapture(b->stream, cudaStreamCaptureModeThreadLocal));
+            cudaError_t e = cudaSuccess;
+            for (int k = 0; k < GRAPH_SWEEPS && e == cudaSuccess; ++k) e = batch_half_sweeps(b, always, hb, (uint32_t)k);
+            if (e == cudaSuccess) e = launch_bump_time_batch(b->d_times, (unsigned)K, GRAPH_SWEEPS, b->stream);
+            cudaError_t e2 = cudaStreamEndCapture(b->stream, &graph);
+            if (e != cudaSuccess || e2 != cudaSuccess) {
+                if (graph) cudaGraphDestroy(graph);
+                EA_FAIL(s0, EA_ERR_CUDA, "batch graph capture: %s", cudaGetErrorString(e != cudaSuccess ? e : e2));
+            }
+            e = cudaGraphInstantiate(&b->graph_exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) { b->graph_exec = nullptr; EA_FAIL(s0, EA_ERR_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e)); }
+            b->graph_always = always;
+            b->graph_hb = hb;
+        }
+        while (left >= (uint64_t)GRAPH_SWEEPS) {
+            EA_CUDA(s0, cudaGraphLaunch(b->graph_exec, b->stream));
+            s0->count_launch(2 * GRAPH_SWEEPS + 1);
+            left -= GRAPH_SWEEPS;
+        }
+    }
+    if (left) {
+        for (uint32_t k = 0; k < (uint32_t)left; ++k) EA_CUDA(s0, batch_half_sweeps(b, always, hb, k));
+        EA_CUDA(s0, launch_bump_time_batch(b->d_times, (unsigned)K, (uint32_t)left, b->stream));
+        s0->count_launch(2 * (unsigned)left + 1);
+    }
+    for (ea_sim *s : b->sims) s->t += n;
+    EA_CUDA(s0, cudaEventRecord(b->ev, b->stream)); // later calls on the other sims' streams see the batch's work
+    for (size_t i = 1; i < K; ++i)
+        if (b->sims[i]->stream != b->stream) EA_CUDA(s0, cudaStreamWaitEvent(b->sims[i]->stream, b->ev, 0));
+    return EA_OK;
+}
+
 ea_status ea_philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
 {
     if (!ctr || !key || !out) return EA_ERR_INVALID;

@@ -87,6 +87,12 @@ cudaError_t fold_from_standard(ea_sim *s, bool spins, bool bonds); // mask unuse
 cudaError_t fold_ensure_unfolded(ea_sim *s);                     // refresh `spins` from f_spins if stale
 cudaError_t launch_half_sweep_fold(ea_sim *s, int parity, uint64_t t, const uint64_t *d_time, uint32_t t_offset,
                                    cudaStream_t st);
+// BATCH (ea_sweep.cu): K small sims per launch, blockIdx.y = sim
+void fill_batch_args(const ea_sim *s, int parity, void *out);
+size_t batch_args_bytes();
+cudaError_t launch_half_sweep_batch(int L, int n_replicas, bool always, bool heatbath, const void *d_args, unsigned n_sims,
+                                    uint32_t t_offset, cudaStream_t st);
+cudaError_t launch_bump_time_batch(uint64_t *const *d_times, unsigned n_sims, uint32_t n, cudaStream_t st);
 // ROWS_PERSISTENT (ea_sweep.cu; L = 16, 32, 64): n sweeps in one cooperative launch with a grid barrier per colour
 bool rows_persistent_valid(int L);
 cudaError_t launch_sweeps_rows_persistent(ea_sim *s, uint64_t t0, uint32_t n, cudaStream_t st);

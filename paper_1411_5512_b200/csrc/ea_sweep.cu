@@ -4,6 +4,7 @@
 // A kernel boundary is the colour barrier ("each half-step is performed in its own CUDA kernel call to
 // ensure global synchronization").  All variants are bit-identical (same stream contract).
 #include <cooperative_groups.h>
+#include <string.h>
 
 #include "ea_internal.h"
 #include "ea_sweep_common.cuh"
@@ -369,6 +370,95 @@ cudaError_t launch_half_sweep(ea_sim *s, int parity, uint64_t t, const uint64_t 
     a.t_offset = t_offset;
     a.th = s->th;
     return s->n_replicas == 2 ? launch_typed<uint32_t>(s, a, st) : launch_typed<uint64_t>(s, a, st);
+}
+
+// ---------------------------------------------------------------------------------------------
+// BATCH ("batched multi-sim driver"): K independent small sims (same L, same bond width, same
+// dynamics; own p, T, seed, t) in ONE launch per colour -- blockIdx.y picks the sim.  Lattices of L <= 64 are
+// launch-bound (a 32^3 half-sweep is a 32-CTA kernel behind a 2 us launch), and concurrent streams hit the launch
+// rate of the device (~0.4 us per kernel); fusing K sims into one grid removes both limits.
+// ---------------------------------------------------------------------------------------------
+template <int L, int M, typename BondT, bool ALWAYS, bool HB>
+__global__ void __launch_bounds__(128) k_sweep_rows_batch(const SweepArgs *__restrict__ args, const uint32_t t_offset)
+{
+    SweepArgs a = args[blockIdx.y];
+    a.t_offset = t_offset;
+    constexpr unsigned RL = L / 4, G = 32 / RL, YC = L / M;
+    const unsigned lane = threadIdx.x & 31, warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned k = lane % RL, grp = lane / RL;
+    const unsigned zg = warp / YC, yc = warp - zg * YC;
+    if (zg >= L / G) return;
+    const unsigned zpar = zg & 1, z = 2 * (G * (zg >> 1) + grp) + zpar, y0 = yc * M;
+    const int lane_m = (int)((lane & ~(RL - 1)) | ((k - 1) & (RL - 1))), lane_p = (int)((lane & ~(RL - 1)) | ((k + 1) & (RL - 1)));
+    const SweepRng g = make_sweep_rng(a.seed, sweep_time(a), (uint32_t)a.colour);
+    if ((a.colour ^ zpar) == 0) march_rows<L, M, 0, BondT, ALWAYS, HB>(a, g, y0, z, k, lane_m, lane_p);
+    else march_rows<L, M, 1, BondT, ALWAYS, HB>(a, g, y0, z, k, lane_m, lane_p);
+}
+
+__global__ void k_bump_time_batch(uint64_t *const *d_times, unsigned n_sims, uint32_t n)
+{
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n_sims) *d_times[i] += n;
+}
+
+template <int L, typename BondT, bool ALWAYS, bool HB>
+static void launch_rows_batch_L(const SweepArgs *d_args, unsigned n_sims, uint32_t t_offset, cudaStream_t st)
+{
+    constexpr int M = 2, G = 32 / (L / 4);
+    constexpr unsigned warps = (L / M) * (L / G), block = 128, grid = (warps * 32 + block - 1) / block;
+    k_sweep_rows_batch<L, M, BondT, ALWAYS, HB><<<dim3(grid, n_sims), block, 0, st>>>(d_args, t_offset);
+}
+
+template <typename BondT, bool ALWAYS, bool HB>
+static cudaError_t launch_rows_batch_typed(int L, const SweepArgs *d_args, unsigned n_sims, uint32_t t_offset, cudaStream_t st)
+{
+    switch (L) {
+    case 16: launch_rows_batch_L<16, BondT, ALWAYS, HB>(d_args, n_sims, t_offset, st); break;
+    case 32: launch_rows_batch_L<32, BondT, ALWAYS, HB>(d_args, n_sims, t_offset, st); break;
+    case 64: launch_rows_batch_L<64, BondT, ALWAYS, HB>(d_args, n_sims, t_offset, st); break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+// host copy of the launch arguments of one sim for one colour (time from the sim's device clock + t_offset)
+void fill_batch_args(const ea_sim *s, int parity, void *out /* SweepArgs */)
+{
+    SweepArgs a;
+    a.lat = s->lat;
+    a.colour = parity;
+    a.own = s->spins_c(parity);
+    a.oth = s->spins_c(1 - parity);
+    const size_t plane = (size_t)3 * s->lat.Nh * s->bond_bytes();
+    a.Jc = (const char *)s->bonds + (size_t)parity * plane;
+    a.Jo = (const char *)s->bonds + (size_t)(1 - parity) * plane;
+    a.seed = s->seed;
+    a.t = 0;
+    a.d_time = s->d_time;
+    a.t_offset = 0;
+    a.th = s->th;
+    memcpy(out, &a, sizeof(a));
+}
+size_t batch_args_bytes() { return sizeof(SweepArgs); }
+
+cudaError_t launch_half_sweep_batch(int L, int n_replicas, bool always, bool heatbath, const void *d_args, unsigned n_sims,
+                                    uint32_t t_offset, cudaStream_t st)
+{
+    const SweepArgs *a = (const SweepArgs *)d_args;
+    if (n_replicas == 2) {
+        if (heatbath) return launch_rows_batch_typed<uint32_t, false, true>(L, a, n_sims, t_offset, st);
+        return always ? launch_rows_batch_typed<uint32_t, true, false>(L, a, n_sims, t_offset, st)
+                      : launch_rows_batch_typed<uint32_t, false, false>(L, a, n_sims, t_offset, st);
+    }
+    if (heatbath) return launch_rows_batch_typed<uint64_t, false, true>(L, a, n_sims, t_offset, st);
+    return always ? launch_rows_batch_typed<uint64_t, true, false>(L, a, n_sims, t_offset, st)
+                  : launch_rows_batch_typed<uint64_t, false, false>(L, a, n_sims, t_offset, st);
+}
+
+cudaError_t launch_bump_time_batch(uint64_t *const *d_times, unsigned n_sims, uint32_t n, cudaStream_t st)
+{
+    k_bump_time_batch<<<(n_sims + 127) / 128, 128, 0, st>>>(d_times, n_sims, n);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_bump_time(ea_sim *s, uint32_t n, cudaStream_t st)

@@ -18,7 +18,7 @@ from . import binding, replicas
 class Scan:
     """points: iterable of dicts with keys L, p, T and optionally n_replicas (2), seed (0), n_slots (1), kernel."""
 
-    def __init__(self, points, rank=0, world_size=1, device=None):
+    def __init__(self, points, rank=0, world_size=1, device=None, fused="auto"):
         self.all_points = [dict(pt) for pt in points]
         self.index = replicas.shard(list(range(len(self.all_points))), rank, world_size)
         self.points = [self.all_points[k] for k in self.index]
@@ -27,13 +27,27 @@ class Scan:
             self.sims.append(binding.Sim(pt["L"], pt["p"], pt["T"], n_replicas=pt.get("n_replicas", 2),
                                          seed=pt.get("seed", 0), n_slots=pt.get("n_slots", 1),
                                          kernel=pt.get("kernel", "auto"), device=device))
+        # L <= 32: one kernel launch per colour for all points of equal shape (ea_batch_*: 0.108 ps/attempt aggregate at
+        # L = 32 with 64 points, against 0.38 for concurrent streams, which hit the launch rate); L = 64: streams are
+        # better (0.078 against 0.106).  fused=True / False overrides.
+        self.batches, self._solo = [], list(self.sims)
+        groups = {}
+        for s in self.sims:
+            if s.n_samples == binding.LANES and s.L in (16, 32, 64) and (fused is True or (fused == "auto" and s.L <= 32)):
+                groups.setdefault((s.L, s.n_replicas), []).append(s)
+        for members in groups.values():
+            if len(members) > 1:
+                self.batches.append(binding.Batch(members))
+                self._solo = [s for s in self._solo if s not in members]
 
     def __len__(self):
         return len(self.sims)
 
     def sweep(self, n):
         """n sweeps of every point; asynchronous (each sim on its own stream), so the points overlap."""
-        for s in self.sims:
+        for b in self.batches:
+            b.sweep(n)
+        for s in self._solo:
             s.sweep(n)
 
     def synchronize(self):
@@ -61,6 +75,9 @@ class Scan:
         return replicas.gather_lanes(np.stack([np.asarray(r[key]) for r in records]))
 
     def close(self):
+        for b in self.batches:
+            b.close()
+        self.batches = []
         for s in self.sims:
             s.close()
         self.sims = []

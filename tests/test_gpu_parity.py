@@ -665,3 +665,42 @@ def test_long_horizon_parity(name, sweeps):
         o.sweep(t - o.time)
         assert_same_state(g, o, "%s t=%d" % (name, t))
     assert_same_observables(g, o)
+
+
+def test_batch_of_small_sims_equals_the_oracle_member_by_member():
+    """ea_batch_*: K sims in one launch per colour (blockIdx.y = sim).  Different p, T (incl. T = inf: the always-masks
+    variant for everybody), seeds and CLOCKS; graph replays + direct launches; members stay ordinary sims."""
+    L = 32
+    pts = [(0.5, 0.8, 11), (0.77, 2.0, 12), (1.0, float("inf"), 13), (0.6, 0.0, 14), (0.9, 0.8, 15)]
+    sims = [binding.Sim(L, p, T, n_replicas=2, seed=wl.seed_for(6, sd), n_slots=1) for p, T, sd in pts]
+    orcs = [Oracle(L, p, T, n_replicas=2, seed=wl.seed_for(6, sd), n_slots=1) for p, T, sd in pts]
+    sims[1].sweep(3); orcs[1].sweep(3)            # members may start at different times
+    b = binding.Batch(sims)
+    for n in (1, 2, 40):
+        b.sweep(n)
+        for o in orcs:
+            o.sweep(n)
+        for k, (g, o) in enumerate(zip(sims, orcs)):
+            assert g.time == o.time
+            assert_same_state(g, o, "batch member %d after +%d" % (k, n))
+    sims[0].sweep(5); orcs[0].sweep(5)            # an ordinary call on a member, then the batch again
+    sims[2].set_temperature(0.8); orcs[2].set_temperature(0.8)
+    b.sweep(33)
+    for o in orcs:
+        o.sweep(33)
+    for k, (g, o) in enumerate(zip(sims, orcs)):
+        assert_same_state(g, o, "batch member %d at the end" % k)
+        assert np.array_equal(g.energy(), o.energy())
+    for s in sims:
+        s.set_dynamics("heatbath")
+    for o in orcs:
+        o.set_dynamics("heatbath")
+    b.sweep(34)
+    for k, (g, o) in enumerate(zip(sims, orcs)):
+        o.sweep(34)
+        assert_same_state(g, o, "batch member %d, heat bath" % k)
+    b.close()
+    with pytest.raises(binding.EAError):
+        binding.Batch([sims[0], binding.Sim(16, 0.5, 0.8, n_replicas=2)])     # mixed L
+    with pytest.raises(binding.EAError):
+        binding.Batch([binding.Sim(128, 0.5, 0.8, n_replicas=2, n_slots=0)])  # fills the device alone
