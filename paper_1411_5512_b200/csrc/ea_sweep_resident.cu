@@ -16,8 +16,6 @@
 //     dependency whose latency is hidden behind the interior update -- no grid-wide barrier, no relaunch.
 //   * global memory always holds the current boundary rows; interior rows are written back once at the end,
 //     so after the launch the global array is the full state at time t0 + n.
-#include <stdlib.h>
-
 #include <utility>
 #include <vector>
 
@@ -439,7 +437,7 @@ template <> struct Geom128Of<uint64_t> { typedef ResidentGeom<128, 16, 8, 8, 2> 
 typedef Geom128Of<uint32_t>::type Geom128; // tile shape, grid and flag layout are the same for both
 
 template <typename BondT, bool ALWAYS, bool RARE, bool HB = false>
-static cudaError_t launch_resident_typed(ea_sim *s, ResidentArgs &a, cudaStream_t st)
+static cudaError_t launch_resident_typed(ResidentArgs &a, cudaStream_t st)
 {
     typedef typename Geom128Of<BondT>::type G;
     static_assert(G::G == Geom128::G && G::SMEM_BYTES == Geom128::SMEM_BYTES, "one flag / shared-memory layout");
@@ -495,16 +493,16 @@ cudaError_t launch_sweeps_resident(ea_sim *s, uint64_t t0, uint32_t n, cudaStrea
     const bool rare = !always && a.th.thr[2] < RARE_THR2_MAX;
     cudaError_t e;
     if (s->dynamics == EA_DYN_HEATBATH) // heat bath (C-HB) carries its own always-masks; no rare branch
-        e = s->n_replicas == 2 ? launch_resident_typed<uint32_t, false, false, true>(s, a, st)
-                               : launch_resident_typed<uint64_t, false, false, true>(s, a, st);
+        e = s->n_replicas == 2 ? launch_resident_typed<uint32_t, false, false, true>(a, st)
+                               : launch_resident_typed<uint64_t, false, false, true>(a, st);
     else if (s->n_replicas == 2)
-        e = always ? launch_resident_typed<uint32_t, true, false>(s, a, st)
-            : rare ? launch_resident_typed<uint32_t, false, true>(s, a, st)
-                   : launch_resident_typed<uint32_t, false, false>(s, a, st);
+        e = always ? launch_resident_typed<uint32_t, true, false>(a, st)
+            : rare ? launch_resident_typed<uint32_t, false, true>(a, st)
+                   : launch_resident_typed<uint32_t, false, false>(a, st);
     else
-        e = always ? launch_resident_typed<uint64_t, true, false>(s, a, st)
-            : rare ? launch_resident_typed<uint64_t, false, true>(s, a, st)
-                   : launch_resident_typed<uint64_t, false, false>(s, a, st);
+        e = always ? launch_resident_typed<uint64_t, true, false>(a, st)
+            : rare ? launch_resident_typed<uint64_t, false, true>(a, st)
+                   : launch_resident_typed<uint64_t, false, false>(a, st);
     if (e == cudaSuccess) {
         s->resident_epoch += 2 * n;
         s->count_launch();
