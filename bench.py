@@ -85,8 +85,37 @@ class ClockSampler:
 
     def __init__(self, index):
         self.index, self.rows, self.proc, self.thread = index, [], None, None
+        self._nvml_stop, self._nvml_rows = None, None
+
+    def _nvml_loop(self, pynvml, handle):
+        """The same quantities straight from NVML every ~5 ms: the timed region of the default run lasts 0.1 s, which a
+        100 ms nvidia-smi loop samples once."""
+        bits = [("hw_slowdown", pynvml.nvmlClocksThrottleReasonHwSlowdown),
+                ("hw_thermal_slowdown", pynvml.nvmlClocksThrottleReasonHwThermalSlowdown),
+                ("sw_thermal_slowdown", pynvml.nvmlClocksThrottleReasonSwThermalSlowdown),
+                ("sw_power_cap", pynvml.nvmlClocksThrottleReasonSwPowerCap)]
+        mx = pynvml.nvmlDeviceGetMaxClockInfo(handle, pynvml.NVML_CLOCK_SM)
+        while not self._nvml_stop.is_set():
+            try:
+                sm = pynvml.nvmlDeviceGetClockInfo(handle, pynvml.NVML_CLOCK_SM)
+                pw = pynvml.nvmlDeviceGetPowerUsage(handle) / 1000.0
+                rs = pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(handle)
+                self._nvml_rows.append((float(sm), float(mx), pw, [n for n, b in bits if rs & b]))
+            except Exception:
+                pass
+            time.sleep(0.005)
 
     def start(self):
+        try:  # NVML first (fast), nvidia-smi as the fallback
+            import pynvml
+            pynvml.nvmlInit()
+            handle = pynvml.nvmlDeviceGetHandleByIndex(self._physical_index())
+            self._nvml_stop, self._nvml_rows = threading.Event(), []
+            self.thread = threading.Thread(target=self._nvml_loop, args=(pynvml, handle), daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self._nvml_stop, self._nvml_rows = None, None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
                                           "--format=csv,noheader,nounits", "-lms", "100"],
@@ -101,7 +130,25 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append([x.strip() for x in line.split(",")])
 
+    def _physical_index(self):
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+        if vis:
+            try:
+                return int(vis.split(",")[self.index])
+            except (ValueError, IndexError):
+                pass
+        return self.index
+
     def stop(self):
+        if self._nvml_stop is not None:
+            self._nvml_stop.set()
+            self.thread.join(timeout=2)
+            rows = self._nvml_rows
+            reasons = sorted({r for row in rows for r in row[3]})
+            return {"sm_mhz": float(np.median([r[0] for r in rows])) if rows else None,
+                    "sm_max_mhz": max(r[1] for r in rows) if rows else None,
+                    "power_w_max": max(r[2] for r in rows) if rows else None, "reasons": reasons, "samples": len(rows),
+                    "source": "nvml, every 5 ms during the timed region"}
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         self.proc.terminate()
