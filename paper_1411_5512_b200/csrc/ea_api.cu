@@ -183,6 +183,8 @@ ea_status ea_destroy(ea_sim *sim)
         DeviceGuard g(sim->device);
         cudaStreamSynchronize(sim->stream);
         destroy_graph(sim);
+        if (sim->c4v_jobs) cudaFree(sim->c4v_jobs);
+        if (sim->c4v_out) cudaFree(sim->c4v_out);
         if (sim->own_ws && sim->ws) cudaFree(sim->ws);
         if (sim->own_stream && sim->stream) cudaStreamDestroy(sim->stream);
     }

@@ -173,16 +173,25 @@ cudaError_t c4_vector_counts(ea_sim *s, size_t n, const int32_t *vec, unsigned l
     if ((e = cudaGetLastError()) != cudaSuccess) { if (Tr_own) cudaFree(Tr_own); return e; }
 
     const size_t JOBS_PER_PASS = 32768; // bounds the temporary buffers (grid.y <= 65535)
-    C4Job *d_jobs = nullptr;
-    unsigned long long *d_out = nullptr;
     std::vector<unsigned long long> h_out;
+    auto grow = [](void **p, size_t *have, size_t need) -> cudaError_t { // the sim's grow-only scratch (freed by ea_destroy)
+        if (*have >= need) return cudaSuccess;
+        if (*p) cudaFree(*p);
+        *p = nullptr;
+        *have = 0;
+        cudaError_t ge = cudaMalloc(p, need);
+        if (ge == cudaSuccess) *have = need;
+        return ge;
+    };
     for (size_t j0 = 0; j0 < jobs.size(); j0 += JOBS_PER_PASS) {
         const size_t nj = std::min(JOBS_PER_PASS, jobs.size() - j0);
         const size_t v0 = jobs[j0].out, v1 = (j0 + nj < jobs.size()) ? jobs[j0 + nj].out : n;
         std::vector<C4Job> pass(jobs.begin() + j0, jobs.begin() + j0 + nj);
         for (auto &jb : pass) jb.out -= (unsigned)v0;
-        if ((e = cudaMalloc((void **)&d_jobs, nj * sizeof(C4Job))) != cudaSuccess) break;
-        if ((e = cudaMalloc((void **)&d_out, (v1 - v0) * 32 * sizeof(unsigned long long))) != cudaSuccess) break;
+        if ((e = grow(&s->c4v_jobs, &s->c4v_jobs_bytes, nj * sizeof(C4Job))) != cudaSuccess) break;
+        if ((e = grow((void **)&s->c4v_out, &s->c4v_out_bytes, (v1 - v0) * 32 * sizeof(unsigned long long))) != cudaSuccess) break;
+        C4Job *d_jobs = (C4Job *)s->c4v_jobs;
+        unsigned long long *d_out = s->c4v_out;
         if ((e = cudaMemcpyAsync(d_jobs, pass.data(), nj * sizeof(C4Job), cudaMemcpyHostToDevice, s->stream)) != cudaSuccess) break;
         if ((e = cudaMemsetAsync(d_out, 0, (v1 - v0) * 32 * sizeof(unsigned long long), s->stream)) != cudaSuccess) break;
         const dim3 grid(C4V_ROWCHUNKS, (unsigned)nj);
@@ -199,11 +208,7 @@ cudaError_t c4_vector_counts(ea_sim *s, size_t n, const int32_t *vec, unsigned l
         if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) break; // also keeps `pass` alive long enough
         for (size_t k = v0; k < v1; ++k)
             std::copy(h_out.begin() + (k - v0) * 32, h_out.begin() + (k - v0 + 1) * 32, counts + v[k].idx * 32);
-        cudaFree(d_jobs); d_jobs = nullptr;
-        cudaFree(d_out); d_out = nullptr;
     }
-    if (d_jobs) cudaFree(d_jobs);
-    if (d_out) cudaFree(d_out);
     if (Tr_own) { cudaStreamSynchronize(s->stream); cudaFree(Tr_own); }
     return e;
 }

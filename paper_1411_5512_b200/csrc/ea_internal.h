@@ -53,6 +53,12 @@ struct ea_sim {
     uint64_t resident_min_sweeps = 1; // shorter ea_sweep calls use the ROWS launches (AUTO: 8)
     bool resident_used = false;       // a resident launch is in flight / unchecked: see check_resident()
 
+    // grow-only scratch of ea_c4_vectors / ea_c4_shells (job list, per-vector counters), owned by the sim
+    void *c4v_jobs = nullptr;
+    size_t c4v_jobs_bytes = 0;
+    unsigned long long *c4v_out = nullptr;
+    size_t c4v_out_bytes = 0;
+
     // kernels this sim has put on the device (a graph replay counts its kernel nodes); bench.py's gpu_launches
     uint64_t launches = 0;
     bool capturing = false;
