@@ -704,3 +704,26 @@ def test_batch_of_small_sims_equals_the_oracle_member_by_member():
         binding.Batch([sims[0], binding.Sim(16, 0.5, 0.8, n_replicas=2)])     # mixed L
     with pytest.raises(binding.EAError):
         binding.Batch([binding.Sim(128, 0.5, 0.8, n_replicas=2, n_slots=0)])  # fills the device alone
+
+
+def test_degenerate_calls():
+    """Zero sweeps, r_max = 0, a batch of one, p = 0 / p = 1 lattices at T = 0: nothing moves that must not."""
+    g, o = make_pair(16, 1.0, 0.0, 2, 5, n_slots=1)
+    before = g.get_spins()
+    g.sweep(0)
+    assert g.time == 0 and np.array_equal(g.get_spins(), before)
+    S, mult = g.c4_shells(0)
+    assert S.shape == (1, 32) and (S[0] == g.N).all() and int(mult[0]) == 1
+    B, q = g.c4(0, with_q=True)
+    assert B.shape == (3, 1, 32) and (B == g.N).all() and np.array_equal(q, o.overlap())
+    up = np.zeros(g.N, dtype=np.uint64)
+    g.set_spins(up); o.set_spins(up)              # p = 1 ground state at T = 0 is a fixed point (P6)
+    b = binding.Batch([g])
+    b.sweep(3); o.sweep(3)
+    assert (g.get_spins() == 0).all() and (g.energy() == -3 * g.N).all() and (g.magnetisation() == g.N).all()
+    assert_same_state(g, o, "ferromagnetic ground state")
+    b.close()
+    h, oh = make_pair(8, 0.0, 0.0, 1, 6)          # p = 0: all bonds -1
+    assert (h.get_bonds() == np.uint64(0xFFFFFFFFFFFFFFFF)).all()
+    h.sweep(5); oh.sweep(5)
+    assert_same_state(h, oh, "p = 0, T = 0")
