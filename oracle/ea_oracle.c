@@ -20,7 +20,10 @@
  * thresholds closed form, single-site acceptance, L=2 Boltzmann statistics by brute
  * force, energy bookkeeping, T=0 monotonicity, p=1 ground state, T=inf alternation,
  * exact gauge equivalence, order independence, lane independence, observables against
- * numpy (roll / FFT) restatements.  No function here is "parity unpinned".
+ * numpy (roll / FFT) restatements; full-vector C_4 against the 3-D FFT and closed-form
+ * anisotropic fields (P14); heat-bath thresholds, detailed-balance ratio and the L = 2
+ * transition matrix (P16).  The fp64 post-processing (C_4 curve, integral estimator,
+ * P15) lives in oracle/__init__.py.  No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
