@@ -17,7 +17,8 @@ which is what the paper's inputs are (random +-J bonds, random start; DESIGN.md 
 
 The JSON line: `value` = device-timed ps per attempt with the lattice resident in HBM; `e2e` = the same
 through the C ABI with HOST buffers (pinned): ea_set_bonds + ea_set_spins (H2D) -> sweeps -> observables ->
-ea_get_spins (D2H), wall clock; `roofline` = the half-sweep kernel against the measured HBM copy bandwidth;
+ea_get_spins (D2H), wall clock; `roofline` = the half-sweep kernel against the alu-pipe (LOP3) issue rate measured in the same run
+(ea_selftest_pipes), with the HBM figure as a secondary record; `protocol` / `cfg5` = SURVEY 8(d)'s sweeps-only windows;
 `cpu_baseline` = the CPU oracle on this box's host cores on a bounded sample.
 
 N > 1 (torchrun): replicas only -- every rank runs its own independent batch (seed + rank); no collective
@@ -45,19 +46,13 @@ UNIT = "ps/attempt"
 LANES = 64
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 
-# From the `ncu --set full` captures summarised in profiles/ (each .md names its command), per kernel variant:
-#   traffic  = dram__bytes_read.sum + dram__bytes_write.sum of ONE launch at the bench configuration (cold L2: ncu
-#              flushes the caches before the launch).  ROWS: one launch = one half-sweep.  RESIDENT: one launch =
-#              the whole ea_sweep(S) call (2 S half-sweeps): the lattice is read once and written back once.
-#   alu_inst = sm__inst_executed_pipe_alu.sum per half-sweep (warp instructions on the LOP3/ISETP pipe).
-NCU = {
-    "rows": {"traffic": 41996032, "alu_inst": None, "profile": "profiles/r01_ncu_full_k_sweep_rows.md"},
-    "resident": {"traffic": 42000000 + 255000, "alu_inst": 631011472 / 400.0,  # profiles/r01_launches_resident.md
-                 "profile": "profiles/r01_ncu_full_k_sweep_resident.md"},
-}
-# alu pipe: one warp instruction per 2 clocks per SM sub-partition (B300_MICROARCH "Pipe rates": rt_SMSP = 2),
-# 4 sub-partitions x 148 SMs, at the max SM clock of MEASURED_PEAKS.json (1965 MHz): DESIGN.md section 6
-ALU_PEAK_WARP_INST_PER_S = 148 * 4 * 0.5 * 1.965e9
+# Algorithmic alu-pipe work of one site word (64 attempts): 12 XOR3 (six unsatisfied-bond words per
+# 32-sample half) + 8 full-adder LOP3 + 4 flip-rule LOP3 + 2 for the rare-level test + 10 Philox XOR3 (one block per
+# two site words) = 36 LOP3-class instructions per lane, all on the alu pipe; addressing is not algorithmic.
+ALGORITHMIC_ALU_INST_PER_SITE_WORD = 36
+# fallback alu peak if ea_selftest_pipes fails: one warp instruction per 2 clocks per SM sub-partition (B300_MICROARCH
+# "Pipe rates": rt_SMSP = 2) x 4 x 148 SMs at 1965 MHz
+FALLBACK_ALU_WARP_INST_PER_S = 148 * 4 * 0.5 * 1.965e9
 
 
 def algorithmic_bytes_per_half_sweep(N, n_replicas):
@@ -279,6 +274,12 @@ def run_ours(args, cfg):
                       device=local_rank, stream=stream)
     flush = torch.empty(args.flush_mib << 20, dtype=torch.uint8, device=dev)
     r_max = L // 2
+    pipes = None
+    if rank == 0:  # the measured integer roofline, before the timed region
+        try:
+            pipes = binding.selftest_pipes(local_rank)
+        except binding.EAError as e:
+            sys.stderr.write("bench.py: ea_selftest_pipes failed (%s); using the guide's pipe rate\n" % e)
 
     def measure_point():
         sim.snapshot(0)
@@ -364,30 +365,89 @@ def run_ours(args, cfg):
         return 0
 
     # ---- roofline of the dominant kernel (the half-sweep), measured live above ------------------------------
-    peak, peak_src = measured_peak_gbs()
+    from paper_1411_5512_b200 import census
+    hbm_peak, hbm_src = measured_peak_gbs()
     t_half = t_sweeps / (2.0 * S * K)
-    alg = algorithmic_bytes_per_half_sweep(N, cfg.n_replicas)
-    achieved = alg / t_half / 1e9
+    alg_bytes = algorithmic_bytes_per_half_sweep(N, cfg.n_replicas)
     kname = binding_kernel_name(sim.kernel)
     resident = kname == "resident" and S >= 8  # AUTO sends shorter calls through the ROWS launches
     hs_per_launch = 2 * S if resident else 1
-    ncu = NCU.get(kname, {})
-    roofline = {"bound": "hbm", "kernel": "half-sweep (%s)" % kname,
-                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": ncu.get("traffic"), "half_sweeps_per_launch": hs_per_launch,
-                "algorithmic_bytes_per_launch": alg * hs_per_launch,
-                "us_per_launch": 1e6 * t_half * hs_per_launch, "us_per_half_sweep": 1e6 * t_half,
-                "peak_source": peak_src, "share_of_step": t_sweeps / t_steps, "profile": ncu.get("profile"),
-                "note": "achieved = algorithmic bytes per launch / mean launch duration (CUDA events on the sim's "
-                        "stream around ea_sweep(S)). north_star: the roofline is the slower of bytes / HBM bandwidth "
-                        "and integer ops / issue rate -- HBM (7.7 us per half-sweep) is the slower one, so bound = "
-                        "hbm; the lattice is L2-resident (ROWS) or shared-memory-resident (RESIDENT) inside a step, "
-                        "so frac exceeds 1 and the alu figure below is the bound that then applies (DESIGN.md 6)"}
-    if ncu.get("alu_inst"):
-        alu_rate = ncu["alu_inst"] / t_half
-        roofline["alu"] = {"achieved": alu_rate / 1e9, "peak": ALU_PEAK_WARP_INST_PER_S / 1e9,
-                           "unit": "G warp-inst/s (alu pipe)", "frac": alu_rate / ALU_PEAK_WARP_INST_PER_S,
-                           "alu_warp_inst_per_half_sweep": ncu["alu_inst"]}
+    thr = [int(x) for x in sim.thresholds]
+    variant = "always" if max(thr) >= 2 ** 32 else "rare" if thr[2] < 0x04000000 else "predicated"
+    ckey = "resident_%s_%s" % ("u32" if cfg.n_replicas == 2 else "u64", variant) if resident else "k_sweep_%s" % kname
+    cen, cen_note = census.lookup(ckey)
+    if pipes is not None:
+        alu_peak, alu_src = pipes["lop3_warp_inst_per_s"], "ea_selftest_pipes: dependent-free LOP3 stream on all SMs, measured in this run"
+    else:
+        alu_peak, alu_src = FALLBACK_ALU_WARP_INST_PER_S, "fallback: 148 SMs x 4 x 0.5 warp-inst/clk x 1.965 GHz (guide pipe rate)"
+    alg_alu = ALGORITHMIC_ALU_INST_PER_SITE_WORD * (N // 2) / 32.0   # warp instructions per half-sweep
+    roofline = {"bound": "alu", "kernel": "half-sweep (%s)" % ckey,
+                "unit": "G warp-inst/s (alu pipe)", "peak": alu_peak / 1e9, "peak_source": alu_src,
+                "achieved": None, "frac": None, "traffic": None,
+                "half_sweeps_per_launch": hs_per_launch, "us_per_launch": 1e6 * t_half * hs_per_launch,
+                "us_per_half_sweep": 1e6 * t_half, "share_of_step": t_sweeps / t_steps,
+                "census": cen_note,
+                "algorithmic": {"alu_warp_inst_per_half_sweep": alg_alu, "achieved": alg_alu / t_half / 1e9,
+                                "frac": alg_alu / t_half / alu_peak,
+                                "note": "%d alu-pipe instructions per site word is the method's own work (DESIGN.md 6); "
+                                        "addressing, compares and moves are not counted" % ALGORITHMIC_ALU_INST_PER_SITE_WORD},
+                "hbm": {"algorithmic_bytes_per_half_sweep": alg_bytes, "achieved_GBps": alg_bytes / t_half / 1e9,
+                        "peak_GBps": hbm_peak, "peak_source": hbm_src,
+                        "note": "secondary: inside a step the spins stay in shared memory and the bonds in L2, so the "
+                                "algorithmic bytes do not cross HBM and this rate may exceed the HBM peak; see `traffic`"},
+                "pipes_measured": pipes,
+                "note": "achieved = alu-pipe warp instructions executed per half-sweep (ncu count of THIS build, "
+                        "alu_census.json, refused if stale) / mean half-sweep duration (CUDA events on the sim's stream "
+                        "around ea_sweep(S)); frac = achieved / measured LOP3 issue rate of the whole chip"}
+    if cen is not None:
+        alu_rate = cen["alu_warp_inst_per_half_sweep"] / t_half
+        roofline.update({"achieved": alu_rate / 1e9, "frac": alu_rate / alu_peak,
+                         "alu_warp_inst_per_half_sweep": cen["alu_warp_inst_per_half_sweep"],
+                         "warp_inst_per_half_sweep": cen.get("warp_inst_per_half_sweep"),
+                         "traffic": cen.get("dram_bytes_per_launch"),
+                         "traffic_note": "dram bytes of the captured ncu launch (%g half-sweeps; cold L2): the lattice "
+                                         "comes in once per launch" % cen.get("half_sweeps_in_captured_launch", 0),
+                         "profile": cen.get("profile")})
+    # ---- SURVEY 8(d) timing protocol: sweeps only, windows of n sweeps, 5 repeats, median and best -------------
+    def sweep_window(sm, n, st):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(st):
+            e0.record(st)
+            sm.sweep(n)
+            e1.record(st)
+        e1.synchronize()
+        sm.synchronize()
+        return e0.elapsed_time(e1) * 1e-3
+
+    protocol = None
+    if args.protocol_window > 0:
+        ts = sorted(sweep_window(sim, args.protocol_window, stream) for _ in range(5))
+        per = lambda t: {"us_per_half_sweep": 1e6 * t / (2.0 * args.protocol_window),
+                         "ps_per_attempt": 1e12 * t / (args.protocol_window * float(N) * LANES)}
+        protocol = {"what": "SURVEY 8(d): CUDA events around ea_sweep(n), sweeps only, 5 repeats", "config": cfg.name,
+                    "n_sweeps": args.protocol_window, "median": per(ts[2]), "best": per(ts[0]), "worst": per(ts[4])}
+    # ---- cfg5: one window per (p, T) point of the paper's production family ------------------
+    cfg5 = None
+    if args.cfg5_window > 0 and ws == 1:
+        pts = []
+        for name in sorted(k for k in wl.CONFIGS if k.startswith("cfg5_")):
+            c5 = wl.CONFIGS[name]
+            s5 = binding.Sim(c5.L, c5.p, c5.T, n_replicas=c5.n_replicas, seed=c5.seed, n_slots=0, kernel=args.kernel,
+                             device=local_rank, stream=stream)
+            s5.sweep(100)  # warm-up 100 sweeps
+            s5.synchronize()
+            t5 = sweep_window(s5, args.cfg5_window, stream)
+            pts.append({"config": name, "p": c5.p, "T": c5.T, "kernel": binding_kernel_name(s5.kernel),
+                        "us_per_half_sweep": 1e6 * t5 / (2.0 * args.cfg5_window),
+                        "ps_per_attempt": 1e12 * t5 / (args.cfg5_window * float(c5.N) * LANES)})
+            s5.close()
+        by_T = {}
+        for q in pts:
+            by_T.setdefault(q["T"], []).append(q["us_per_half_sweep"])
+        cfg5 = {"what": "one %d-sweep window per (p, T) point of BASELINE.json configs[4], sweeps only, after 100 warm-up "
+                        "sweeps (the paper ran 10^8 sweeps per point, PAPER.md:108)" % args.cfg5_window,
+                "n_sweeps": args.cfg5_window, "points": pts,
+                "spread_in_p": {str(T): (max(v) - min(v)) / min(v) for T, v in by_T.items()}}
     # ---- SURVEY 8(f) rows built so far, timed on the same state (not part of `value`) -----------------------
     next_rows = None
     if cfg.n_replicas == 2 and not args.no_next_rows:
@@ -437,6 +497,8 @@ def run_ours(args, cfg):
         "gpu_launches": int(launches),
         "roofline": roofline,
         "cpu_baseline": cpu_baseline,
+        "protocol": protocol,
+        "cfg5": cfg5,
         "next_rows": next_rows,
         "wall_s_timed_loop": wall,
         "paper_context": "paper: ~8 ps per spin flip on a GeForce GTX 570 (PAPER.md:5, :92) -- other hardware, "
@@ -460,6 +522,10 @@ def main():
     ap.add_argument("--sweeps-per-step", type=int, default=1000)
     ap.add_argument("--kernel", default="auto")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the timing of the SURVEY 8(f) rows (c4_shells, scan)")
+    ap.add_argument("--protocol-window", type=int, default=10000,
+                    help="sweeps per window of the SURVEY 8(d) protocol (5 repeats, median / best); 0 = skip")
+    ap.add_argument("--cfg5-window", type=int, default=100000,
+                    help="sweeps per (p, T) point of the cfg5 family (SURVEY 8(d) asks for up to 10^6); 0 = skip")
     ap.add_argument("--flush-mib", type=int, default=256)
     ap.add_argument("--cpu-sweeps", type=int, default=12, help="oracle sweeps timed for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (profiler runs)")

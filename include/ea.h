@@ -14,6 +14,8 @@
  *   - ea_sweep / ea_snapshot are asynchronous on the sim's stream; every call that returns
  *     host data synchronises that stream before returning.
  *   - A handle is not thread-safe; distinct handles are independent.
+ *   - After EA_ERR_CUDA from a call that advances the dynamics the spin state is undefined (the device may
+ *     have run part of the request); t counts the sweeps whose launches were all queued.
  *   - Results depend only on (L, p, T, n_replicas, seed, t): never on the GPU, the kernel
  *     variant or the launch geometry.  ea_sweep(a); ea_sweep(b) == ea_sweep(a+b).
  *   - There is no CPU fallback: without a CUDA device every compute call returns EA_ERR_CUDA.
@@ -35,6 +37,7 @@ extern "C" {
 #endif
 
 #define EA_LANES 64 /* samples per multispin word (III) */
+#define EA_C4_MAX_VECTORS ((int64_t)1 << 24) /* ea_c4_vectors: most vectors per call (a full L = 128 torus has 2^21) */
 
 typedef struct ea_sim ea_sim; /* opaque; one batch of 64 samples on one L^3 lattice */
 
@@ -52,7 +55,11 @@ typedef enum {
     EA_KERNEL_SCALAR = 1, /* one site per thread, 64-bit loads; any even L >= 2           */
     EA_KERNEL_VEC2 = 2,   /* two sites per thread, 128-bit loads; L % 4 == 0              */
     EA_KERNEL_ROWS = 3,   /* warp marches along y with a register window; L % 4 == 0      */
-    EA_KERNEL_RESIDENT = 4, /* persistent cooperative kernel, many sweeps per launch (L = 128) */
+    EA_KERNEL_RESIDENT = 4, /* persistent cooperative kernel, many sweeps per launch (L = 128); needs a device with
+                               cooperative launch, >= 128 SMs and 187 KB of shared memory per CTA (ea_last_error /
+                               stderr say which is missing).  Its CTAs wait for their neighbours' step flags; a wait
+                               that sees nothing for EA_RESIDENT_TIMEOUT_MS (environment, read at ea_create;
+                               default 20000) gives up, and the next synchronising call returns EA_ERR_CUDA */
     EA_KERNEL_FOLD = 5,    /* what a sim with n_samples < 64 runs (not selectable)        */
     EA_KERNEL_ROWS_PERSISTENT = 6 /* ROWS with a grid barrier per colour, one launch per ea_sweep (L = 16, 32, 64);
                                      measured slower than the graph replays, never chosen by AUTO */
@@ -77,10 +84,13 @@ typedef struct ea_params {
     uint64_t seed;      /* Philox key (C-A6)                                               */
     int32_t device;     /* CUDA device ordinal; -1 = current device                        */
     int32_t kernel;     /* ea_kernel                                                       */
-    void *stream;       /* cudaStream_t to run on (caller-owned, not the legacy default
-                           stream); NULL = the library creates and owns a stream            */
-    void *d_workspace;  /* device memory, >= ea_workspace_bytes(...), 256-byte aligned,
-                           caller-owned and alive until ea_destroy; NULL = library allocates */
+    void *stream;       /* cudaStream_t to run on (caller-owned); NULL = the library creates and owns a
+                           non-blocking stream.  The legacy default stream (cudaStreamLegacy) cannot be
+                           captured into a CUDA graph and is refused with EA_ERR_INVALID                */
+    void *d_workspace;  /* device memory, >= ea_workspace_bytes(...), 256-byte aligned, anywhere in the
+                           address space, caller-owned and alive until ea_destroy; work queued on other
+                           streams that still touches it must be complete (or ordered before `stream`)
+                           when ea_create_ex is called; NULL = library allocates                         */
     size_t workspace_bytes;
 } ea_params;
 
@@ -131,7 +141,7 @@ ea_status ea_c4(ea_sim *sim, int r_max, int64_t *B, int64_t *q, double *c4_avg);
  * vector, periodic -- reading C-S8v; the paper's "all r >= 3" reference set, and Fig. 2):
  *   B[v*32 + b] = sum_i q_i q_{i + r_v},  r_v = (dxyz[3v], dxyz[3v+1], dxyz[3v+2]), any integers.
  * host arrays: dxyz 3 n_vec int32, B 32 n_vec int64.  EA_ERR_STATE on a 1-replica sim; EA_ERR_INVALID unless
- * L <= 32 or L in {64, 128}. */
+ * L <= 32 or L in {64, 128}, or n_vec > EA_C4_MAX_VECTORS; EA_ERR_NOMEM if a host buffer cannot be allocated. */
 ea_status ea_c4_vectors(ea_sim *sim, int64_t n_vec, const int32_t *dxyz, int64_t *B);
 /* Shell sums over the cube |dx|, |dy|, |dz| <= r_max (0 <= r_max <= L/2), by squared length d2 = 0 .. 3 r_max^2:
  *   S[d2*32 + b] = sum_{|r|^2 = d2} B_b(r),  mult[d2] = number of those vectors (0 for an empty shell),
@@ -176,6 +186,15 @@ ea_status ea_batch_destroy(ea_batch *batch);
 /* Host-only self-test (no device needed): the row schedules of the RESIDENT kernel -- every row of a tile exactly
  * once, boundary rows first, consecutive rows of a warp alternating in parity.  EA_OK or EA_ERR_STATE. */
 ea_status ea_selftest_host(void);
+
+/* Measured issue rates of the pipes that bound this library's kernels (the update is "boolean logic at
+ * the bit level" plus one random number, and the observables are popcounts, Eq. 3 and 7): dependent-free
+ * instruction streams on every SM of `device` (-1 = current), about 30 ms of device time, default stream.
+ *   out[0] = LOP3 (alu pipe), out[1] = IMAD.WIDE.U32 (fma pipe), out[2] = POPC  -- warp instructions per second;
+ *   out[3] = LOP3 rate while as many IMAD.WIDE.U32 are issued alongside (the two pipes of the sweep kernel together);
+ *   out[4] = SM clock in MHz during the LOP3 stream (clock64 / globaltimer), out[5] = number of SMs, out[6..7] = 0.
+ * host array of 8 doubles.  EA_ERR_CUDA without a device. */
+ea_status ea_selftest_pipes(int device, double out[8]);
 
 /* Philox4x32-10 block on the device (one thread), for the known-answer test of the GPU side (C-A6). */
 ea_status ea_philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);

@@ -70,6 +70,7 @@ SIGNATURES = {
     "ea_batch_sweep": (_i, [_vp, _u64]),
     "ea_batch_destroy": (_i, [_vp]),
     "ea_selftest_host": (_i, []),
+    "ea_selftest_pipes": (_i, [_i, C.POINTER(_dbl)]),
     "ea_philox_selftest": (_i, [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]),
     "ea_strerror": (C.c_char_p, [_i]),
     "ea_last_error": (C.c_char_p, [_vp]),
@@ -109,7 +110,10 @@ class Sim:
     """One batch of 64 samples on an L^3 lattice on the GPU.  Methods mirror the C entry points."""
 
     def __init__(self, L, p, T, n_replicas=1, seed=0, n_slots=2, kernel="auto", device=None, stream=None,
-                 torch_workspace=True, n_samples=LANES):
+                 torch_workspace=True, n_samples=LANES, workspace=None):
+        """workspace: (device pointer, owner) of caller-placed device memory of >= workspace_bytes(...) bytes,
+        256-byte aligned; `owner` is kept alive with the sim.  Default: a torch tensor (torch_workspace=True) or
+        the library's own cudaMalloc (torch_workspace=False)."""
         self._h = _vp()
         self.L, self.N, self.n_replicas, self.n_slots = int(L), int(L) ** 3, int(n_replicas), int(n_slots)
         self.n_samples = int(n_samples)
@@ -123,7 +127,12 @@ class Sim:
         if stream is not None:  # a torch.cuda.Stream: the library launches on it
             prm.stream = stream.cuda_stream
         nbytes = lib().ea_workspace_bytes_ex(int(L), int(n_samples), int(n_replicas), int(n_slots))
-        if torch_workspace and nbytes:
+        if workspace is not None:
+            ptr, self._ws = workspace
+            if int(ptr) % 256:
+                raise EAError(EA_ERR_INVALID, "workspace pointer must be 256-byte aligned")
+            prm.d_workspace, prm.workspace_bytes = int(ptr), nbytes
+        elif torch_workspace and nbytes:
             import torch  # device memory only
             if not torch.cuda.is_available():
                 raise EAError(EA_ERR_CUDA, "no CUDA device (there is no CPU fallback)")
@@ -132,6 +141,9 @@ class Sim:
             base = self._ws.data_ptr()
             prm.d_workspace = (base + 255) & ~255
             prm.workspace_bytes = nbytes
+            # the block may be recycled from a tensor that work queued on torch's current stream still uses, while
+            # the library writes it on its own stream: order the two once, here
+            torch.cuda.current_stream(dev).synchronize()
         st = lib().ea_create_ex(C.byref(prm), C.byref(self._h))
         if st != EA_OK:
             self._h = _vp()
@@ -347,6 +359,20 @@ def integral_estimator(r, c, e, k):
     if st != 0:
         raise EAError(st, "ea_integral_estimator: invalid argument")
     return tuple(float(x) for x in out)
+
+
+def workspace_bytes(L, n_replicas=1, n_slots=2, n_samples=LANES):
+    return int(lib().ea_workspace_bytes_ex(int(L), int(n_samples), int(n_replicas), int(n_slots)))
+
+
+def selftest_pipes(device=None):
+    """Measured issue rates (ea_selftest_pipes): dict of warp instructions per second and the SM clock."""
+    out = (_dbl * 8)()
+    st = lib().ea_selftest_pipes(-1 if device is None else int(device), out)
+    if st != EA_OK:
+        raise EAError(st, "ea_selftest_pipes: " + lib().ea_strerror(st).decode())
+    return {"lop3_warp_inst_per_s": out[0], "imad_wide_warp_inst_per_s": out[1], "popc_warp_inst_per_s": out[2],
+            "lop3_with_imad_wide_warp_inst_per_s": out[3], "sm_mhz": out[4], "n_sm": int(out[5])}
 
 
 def philox_selftest(ctr, key):

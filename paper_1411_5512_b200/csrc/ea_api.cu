@@ -2,8 +2,10 @@
 // launch sequencing.  No arithmetic of the method lives here except the acceptance thresholds (Eq. 9).
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
+#include <exception>
 #include <new>
 
 #include "ea_internal.h"
@@ -239,6 +241,11 @@ ea_status ea_create_ex(const ea_params *prm, ea_sim **out)
         if (!g.ok) { rc = EA_ERR_CUDA; break; }
         cudaDeviceGetAttribute(&s->n_sm, cudaDevAttrMultiProcessorCount, device);
         if (prm->stream) {
+            if ((cudaStream_t)prm->stream == cudaStreamLegacy) { // cannot be captured into a graph (ea_sweep would fail late)
+                fprintf(stderr, "ea_create_ex: the legacy default stream is not supported; pass NULL or a created stream\n");
+                rc = EA_ERR_INVALID;
+                break;
+            }
             s->stream = (cudaStream_t)prm->stream;
         } else { // own stream: the legacy default stream cannot be captured into a graph
             if ((e = cudaStreamCreateWithFlags(&s->stream, cudaStreamNonBlocking)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
@@ -261,10 +268,16 @@ ea_status ea_create_ex(const ea_params *prm, ea_sim **out)
         s->d_time = (uint64_t *)(s->ws + w.off_time);
         s->resident_flags = (unsigned *)(s->ws + w.off_flags);
         if ((e = cudaMemsetAsync(s->resident_flags, 0, resident_flag_bytes(), s->stream)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
-        if (prm->kernel == EA_KERNEL_AUTO && kernel_valid_for(EA_KERNEL_RESIDENT, L) && resident_supported(s)) {
+        if (const char *ms = getenv("EA_RESIDENT_TIMEOUT_MS")) {
+            const long long v = atoll(ms);
+            if (v > 0) s->resident_timeout_ns = (uint64_t)v * 1000000ull;
+        }
+        std::string why;
+        if (prm->kernel == EA_KERNEL_AUTO && kernel_valid_for(EA_KERNEL_RESIDENT, L) && resident_supported(s, &why)) {
             s->kernel = EA_KERNEL_RESIDENT; // long runs in one persistent launch, short ones as ROWS launches
             s->resident_min_sweeps = RESIDENT_AUTO_MIN_SWEEPS;
-        } else if (s->kernel == EA_KERNEL_RESIDENT && !resident_supported(s)) {
+        } else if (s->kernel == EA_KERNEL_RESIDENT && !resident_supported(s, &why)) {
+            fprintf(stderr, "ea_create_ex: %s\n", why.c_str()); // no handle to carry the message yet
             rc = EA_ERR_INVALID;
             break;
         }
@@ -465,8 +478,8 @@ ea_status ea_set_kernel(ea_sim *sim, int kernel)
         k = EA_KERNEL_RESIDENT;
         sim->resident_min_sweeps = RESIDENT_AUTO_MIN_SWEEPS;
     }
-    if (k == EA_KERNEL_RESIDENT && !resident_supported(sim))
-        EA_FAIL(sim, EA_ERR_INVALID, "resident kernel: device lacks cooperative launch, >= 128 SMs or 181 KB of shared memory per CTA");
+    std::string why;
+    if (k == EA_KERNEL_RESIDENT && !resident_supported(sim, &why)) EA_FAIL(sim, EA_ERR_INVALID, "%s", why.c_str());
     sim->kernel = k;
     return EA_OK;
 }
@@ -586,12 +599,17 @@ ea_status ea_c4_vectors(ea_sim *sim, int64_t n_vec, const int32_t *dxyz, int64_t
     if (!sim || n_vec < 0 || (n_vec && (!dxyz || !B))) return EA_ERR_INVALID;
     if (sim->n_replicas != 2) EA_FAIL(sim, EA_ERR_STATE, "ea_c4_vectors needs a 2-replica sim");
     if (!c4_vectors_supported(sim->lat.L)) EA_FAIL(sim, EA_ERR_INVALID, "ea_c4_vectors: L must be <= 32, 64 or 128");
+    if (n_vec > EA_C4_MAX_VECTORS) EA_FAIL(sim, EA_ERR_INVALID, "ea_c4_vectors: n_vec %lld > %lld", (long long)n_vec, (long long)EA_C4_MAX_VECTORS);
     DeviceGuard g(sim->device);
-    std::vector<unsigned long long> cnt((size_t)n_vec * 32);
-    EA_CUDA(sim, fold_ensure_unfolded(sim));
-    EA_CUDA(sim, c4_vector_counts(sim, (size_t)n_vec, dxyz, cnt.data()));
-    EA_SYNC(sim);
-    for (size_t k = 0; k < cnt.size(); ++k) B[k] = sim->N - 2 * (int64_t)cnt[k];
+    try { // host buffers are sized by the caller's n_vec: no exception may cross the C ABI
+        std::vector<unsigned long long> cnt((size_t)n_vec * 32);
+        EA_CUDA(sim, fold_ensure_unfolded(sim));
+        EA_CUDA(sim, c4_vector_counts(sim, (size_t)n_vec, dxyz, cnt.data()));
+        EA_SYNC(sim);
+        for (size_t k = 0; k < cnt.size(); ++k) B[k] = sim->N - 2 * (int64_t)cnt[k];
+    } catch (const std::exception &) {
+        EA_FAIL(sim, EA_ERR_NOMEM, "ea_c4_vectors: host allocation failed");
+    }
     return EA_OK;
 }
 
@@ -603,28 +621,32 @@ ea_status ea_c4_shells(ea_sim *sim, int r_max, int64_t *S, int64_t *mult)
     if (!c4_vectors_supported(sim->lat.L)) EA_FAIL(sim, EA_ERR_INVALID, "ea_c4_shells: L must be <= 32, 64 or 128");
     // B(r) = B(-r): the device visits one vector of every +-r pair (the half space dz > 0, or dz = 0 and dy > 0,
     // or dz = dy = 0 and dx > 0) and the shell receives it twice; r = 0 is B = N exactly
-    std::vector<int32_t> vec;
-    for (int dz = 0; dz <= r_max; ++dz)
-        for (int dy = (dz ? -r_max : 0); dy <= r_max; ++dy)
-            for (int dx = ((dz || dy) ? -r_max : 1); dx <= r_max; ++dx) {
-                vec.push_back(dx); vec.push_back(dy); vec.push_back(dz);
-            }
-    const size_t n = vec.size() / 3, n_bins = (size_t)3 * r_max * r_max + 1;
-    std::vector<unsigned long long> cnt(n * 32);
-    {
-        DeviceGuard g(sim->device);
-        EA_CUDA(sim, fold_ensure_unfolded(sim));
-        EA_CUDA(sim, c4_vector_counts(sim, n, vec.data(), cnt.data()));
-        EA_SYNC(sim);
-    }
-    for (size_t k = 0; k < n_bins * 32; ++k) S[k] = 0;
-    for (size_t k = 0; k < n_bins; ++k) mult[k] = 0;
-    for (int b = 0; b < 32; ++b) S[b] = sim->N;
-    mult[0] = 1;
-    for (size_t v = 0; v < n; ++v) {
-        const int64_t d2 = (int64_t)vec[3 * v] * vec[3 * v] + (int64_t)vec[3 * v + 1] * vec[3 * v + 1] + (int64_t)vec[3 * v + 2] * vec[3 * v + 2];
-        for (int b = 0; b < 32; ++b) S[d2 * 32 + b] += 2 * (sim->N - 2 * (int64_t)cnt[v * 32 + b]);
-        mult[d2] += 2;
+    try { // no exception may cross the C ABI
+        std::vector<int32_t> vec;
+        for (int dz = 0; dz <= r_max; ++dz)
+            for (int dy = (dz ? -r_max : 0); dy <= r_max; ++dy)
+                for (int dx = ((dz || dy) ? -r_max : 1); dx <= r_max; ++dx) {
+                    vec.push_back(dx); vec.push_back(dy); vec.push_back(dz);
+                }
+        const size_t n = vec.size() / 3, n_bins = (size_t)3 * r_max * r_max + 1;
+        std::vector<unsigned long long> cnt(n * 32);
+        {
+            DeviceGuard g(sim->device);
+            EA_CUDA(sim, fold_ensure_unfolded(sim));
+            EA_CUDA(sim, c4_vector_counts(sim, n, vec.data(), cnt.data()));
+            EA_SYNC(sim);
+        }
+        for (size_t k = 0; k < n_bins * 32; ++k) S[k] = 0;
+        for (size_t k = 0; k < n_bins; ++k) mult[k] = 0;
+        for (int b = 0; b < 32; ++b) S[b] = sim->N;
+        mult[0] = 1;
+        for (size_t v = 0; v < n; ++v) {
+            const int64_t d2 = (int64_t)vec[3 * v] * vec[3 * v] + (int64_t)vec[3 * v + 1] * vec[3 * v + 1] + (int64_t)vec[3 * v + 2] * vec[3 * v + 2];
+            for (int b = 0; b < 32; ++b) S[d2 * 32 + b] += 2 * (sim->N - 2 * (int64_t)cnt[v * 32 + b]);
+            mult[d2] += 2;
+        }
+    } catch (const std::exception &) {
+        EA_FAIL(sim, EA_ERR_NOMEM, "ea_c4_shells: host allocation failed");
     }
     return EA_OK;
 }
@@ -715,9 +737,9 @@ ea_status ea_get_bonds(ea_sim *sim, uint64_t *host)
     for (int d = 0; d < 3; ++d) {
         EA_CUDA(sim, launch_unpack_bonds(sim, d, sim->stage));
         EA_CUDA(sim, cudaMemcpyAsync(host + (size_t)d * sim->N, sim->stage, (size_t)sim->N * 8, cudaMemcpyDeviceToHost,
-                                     sim->stream));
-        EA_SYNC(sim);
+                                     sim->stream)); // stream order keeps unpack d+1 behind this copy of the staging buffer
     }
+    EA_SYNC(sim);
     return EA_OK;
 }
 
@@ -866,20 +888,40 @@ ea_status ea_batch_sweep(ea_batch *b, uint64_t n)
             b->graph_hb = hb;
         }
         while (left >= (uint64_t)GRAPH_SWEEPS) {
-            EA_CUDA(s0, cudaGraphLaunch(b->graph_exec, b->stream));
+            const cudaError_t e = cudaGraphLaunch(b->graph_exec, b->stream);
+            if (e != cudaSuccess) { // the members' clocks count the replays that were queued
+                for (ea_sim *s : b->sims) s->t += n - left;
+                EA_FAIL(s0, EA_ERR_CUDA, "cudaGraphLaunch: %s", cudaGetErrorString(e));
+            }
             s0->count_launch(2 * GRAPH_SWEEPS + 1);
             left -= GRAPH_SWEEPS;
         }
     }
-    if (left) {
+    for (ea_sim *s : b->sims) s->t += n - left;
+    if (left) { // a failure in here leaves the members' spins part-way through these `left` sweeps (undefined)
         for (uint32_t k = 0; k < (uint32_t)left; ++k) EA_CUDA(s0, batch_half_sweeps(b, always, hb, k));
         EA_CUDA(s0, launch_bump_time_batch(b->d_times, (unsigned)K, (uint32_t)left, b->stream));
         s0->count_launch(2 * (unsigned)left + 1);
+        for (ea_sim *s : b->sims) s->t += left;
     }
-    for (ea_sim *s : b->sims) s->t += n;
     EA_CUDA(s0, cudaEventRecord(b->ev, b->stream)); // later calls on the other sims' streams see the batch's work
     for (size_t i = 1; i < K; ++i)
         if (b->sims[i]->stream != b->stream) EA_CUDA(s0, cudaStreamWaitEvent(b->sims[i]->stream, b->ev, 0));
+    return EA_OK;
+}
+
+ea_status ea_selftest_pipes(int device, double out[8])
+{
+    if (!out) return EA_ERR_INVALID;
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) return EA_ERR_CUDA;
+    if (device < 0 && cudaGetDevice(&device) != cudaSuccess) return EA_ERR_CUDA;
+    if (device >= n_dev) return EA_ERR_INVALID;
+    DeviceGuard g(device);
+    if (!g.ok) return EA_ERR_CUDA;
+    double r[8];
+    if (pipe_rates(device, r) != cudaSuccess) return EA_ERR_CUDA;
+    memcpy(out, r, sizeof(r));
     return EA_OK;
 }
 

@@ -52,6 +52,7 @@ struct ea_sim {
     uint32_t resident_epoch = 0;
     uint64_t resident_min_sweeps = 1; // shorter ea_sweep calls use the ROWS launches (AUTO: 8)
     bool resident_used = false;       // a resident launch is in flight / unchecked: see check_resident()
+    uint64_t resident_timeout_ns = 20000000000ull; // neighbour wait gives up after this (EA_RESIDENT_TIMEOUT_MS)
 
     // grow-only scratch of ea_c4_vectors / ea_c4_shells (job list, per-vector counters), owned by the sim
     void *c4v_jobs = nullptr;
@@ -103,7 +104,7 @@ cudaError_t launch_bump_time_batch(uint64_t *const *d_times, unsigned n_sims, ui
 bool rows_persistent_valid(int L);
 cudaError_t launch_sweeps_rows_persistent(ea_sim *s, uint64_t t0, uint32_t n, cudaStream_t st);
 // RESIDENT (ea_sweep_resident.cu): n sweeps from sweep index t0 in one cooperative launch
-bool resident_supported(const ea_sim *s);
+bool resident_supported(const ea_sim *s, std::string *why = nullptr);
 size_t resident_flag_bytes();
 bool resident_tables_ok();
 cudaError_t launch_sweeps_resident(ea_sim *s, uint64_t t0, uint32_t n, cudaStream_t st);
@@ -123,6 +124,7 @@ cudaError_t launch_count_c4(ea_sim *s, int r_max); // counters[(d*(r_max+1)+r)*3
 bool c4_vectors_supported(int L);
 cudaError_t c4_vector_counts(ea_sim *s, size_t n, const int32_t *vec, unsigned long long *counts);
 
+cudaError_t pipe_rates(int device, double out[8]);
 cudaError_t philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 
 } // namespace ea

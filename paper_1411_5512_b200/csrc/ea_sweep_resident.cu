@@ -33,6 +33,7 @@ struct ResidentArgs {
     uint32_t epoch0;     // flag value before this launch; step h publishes epoch0 + h + 1
     unsigned *flags;     // [G][32]: one 128-byte line per CTA
     unsigned *abort_flag;// set by any CTA whose wait timed out; everybody then leaves
+    unsigned long long timeout_ns; // a neighbour that never shows up: give up after this long
     Thresholds th;
 };
 
@@ -102,7 +103,6 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
 
 enum { BAR_BOUNDARY = 1, BAR_STEP = 2 };
 constexpr uint32_t RARE_THR2_MAX = 0x04000000u; // P(r < thr[2]) < 1/64: the warp-level branch of metropolis_word pays
-constexpr unsigned long long RESIDENT_TIMEOUT_NS = 2000000000ull; // a neighbour that never shows up: give up after 2 s
 
 // Row schedule of one CTA (built on the host, build_row_table): compute warp w updates rows row[w][0..RPW-1]
 // (yy | zz << 8, tile coordinates 1..TY, 1..TZ), boundary rows first (n_bnd[w] of them), and consecutive rows
@@ -133,16 +133,16 @@ __device__ __forceinline__ uint4 make_row_desc(unsigned yy, unsigned zz, unsigne
     return d;
 }
 
-// The kernel is bound by the alu pipe (LOP3), and 64-bit address arithmetic costs IADD3 / LEA.HI.X pairs on that
-// pipe for every row.  The host guarantees (resident_supported) that neither the bond nor the spin array
-// straddles a 4 GiB boundary, so inside the row loop an address is {constant high word, low word + offset}.
+// Row addresses are "64-bit per-lane base + 32-bit element offset from the row descriptor": one IMAD.WIDE.U32 on the
+// fma pipe (the kernel is bound by the alu pipe, where a 64-bit add would cost an IADD3 / IADD3.X pair per row).
+// The base is a full 64-bit pointer, so the arrays may lie anywhere in the address space.
 struct Ptr32 {
-    uint32_t lo, hi;
+    const char *base;
     __device__ __forceinline__ Ptr32() {}
-    __device__ __forceinline__ explicit Ptr32(const void *p) : lo((uint32_t)(uintptr_t)p), hi((uint32_t)((uintptr_t)p >> 32)) {}
+    __device__ __forceinline__ explicit Ptr32(const void *p) : base((const char *)p) {}
     template <typename T> __device__ __forceinline__ T *at(unsigned elem_off) const
     {
-        return (T *)(((uintptr_t)hi << 32) | (uintptr_t)(lo + elem_off * (unsigned)sizeof(T)));
+        return (T *)(base + (size_t)elem_off * sizeof(T));
     }
 };
 
@@ -308,7 +308,7 @@ __global__ void __launch_bounds__(G::THREADS, 1) k_sweep_resident(const Resident
                 unsigned spins = 0;
                 while ((int)(ld_acquire_gpu(f) - epoch) < 0) {
                     if ((++spins & 63u) == 0) {
-                        if (*(volatile unsigned *)a.abort_flag || globaltimer_ns() - t_start > RESIDENT_TIMEOUT_NS) {
+                        if (*(volatile unsigned *)a.abort_flag || globaltimer_ns() - t_start > a.timeout_ns) {
                             ok = false;
                             break;
                         }
@@ -451,17 +451,16 @@ static cudaError_t launch_resident_typed(ResidentArgs &a, cudaStream_t st)
     return cudaLaunchCooperativeKernel((void *)kern, dim3(G::G), dim3(G::THREADS), args, G::SMEM_BYTES, st);
 }
 
-bool resident_supported(const ea_sim *s)
+bool resident_supported(const ea_sim *s, std::string *why)
 {
-    if (s->lat.L != 128) return false;
+    auto no = [&](const char *msg) { if (why) *why = msg; return false; };
+    if (s->lat.L != 128) return no("resident kernel: L must be 128");
     cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) return false;
-    // the row loop does 32-bit address arithmetic (Ptr32): no array may straddle a 4 GiB boundary
-    const uintptr_t b0 = (uintptr_t)s->bonds, b1 = b0 + (size_t)6 * s->lat.Nh * s->bond_bytes() - 1;
-    const uintptr_t s0 = (uintptr_t)s->spins, s1 = s0 + (size_t)2 * s->lat.Nh * 8 - 1;
-    if ((b0 >> 32) != (b1 >> 32) || (s0 >> 32) != (s1 >> 32)) return false;
-    return prop.cooperativeLaunch && prop.multiProcessorCount >= Geom128::G &&
-           prop.sharedMemPerBlockOptin >= Geom128::SMEM_BYTES;
+    if (cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) return no("resident kernel: cudaGetDeviceProperties failed");
+    if (!prop.cooperativeLaunch) return no("resident kernel: the device has no cooperative launch");
+    if (prop.multiProcessorCount < Geom128::G) return no("resident kernel: the device has fewer than 128 SMs");
+    if (prop.sharedMemPerBlockOptin < Geom128::SMEM_BYTES) return no("resident kernel: the device has less than 187 KB of shared memory per CTA");
+    return true;
 }
 
 // host-only check of the row schedules of both geometries (every row once, boundary rows first, alternating parity)
@@ -487,6 +486,7 @@ cudaError_t launch_sweeps_resident(ea_sim *s, uint64_t t0, uint32_t n, cudaStrea
     a.epoch0 = s->resident_epoch;
     a.flags = s->resident_flags;
     a.abort_flag = s->resident_flags + Geom128::G * 32;
+    a.timeout_ns = s->resident_timeout_ns;
     a.th = s->th;
     const bool always = a.th.always[0] | a.th.always[1] | a.th.always[2];
     // low temperature: energy-raising moves are rare enough for a warp-level branch (see metropolis_word)

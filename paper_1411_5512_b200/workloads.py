@@ -46,12 +46,12 @@ CONFIGS = {
     "cfg3b": Config("cfg3b", 64, 0.7, 0.8, 2, 10 ** 6, seed_for(3, 1), 300),
     "cfg4": Config("cfg4", 128, 0.77, 0.8, 2, 10 ** 7, seed_for(4), 48),
     "cfg5_p0.5_T0.8": Config("cfg5_p0.5_T0.8", 128, 0.5, 0.8, 2, 10 ** 8, seed_for(5, 0), 8),
-    "cfg5_p0.8_T0.8": Config("cfg5_p0.8_T0.8", 128, 0.8, 0.8, 2, 10 ** 8, seed_for(5, 1), 4),
-    "cfg5_p0.9_T0.8": Config("cfg5_p0.9_T0.8", 128, 0.9, 0.8, 2, 10 ** 8, seed_for(5, 2), 4),
-    "cfg5_p1.0_T0.8": Config("cfg5_p1.0_T0.8", 128, 1.0, 0.8, 2, 10 ** 8, seed_for(5, 3), 4),
-    "cfg5_p0.5_T2.0": Config("cfg5_p0.5_T2.0", 128, 0.5, 2.0, 2, 10 ** 8, seed_for(5, 4), 4),
-    "cfg5_p0.8_T2.0": Config("cfg5_p0.8_T2.0", 128, 0.8, 2.0, 2, 10 ** 8, seed_for(5, 5), 4),
-    "cfg5_p0.9_T2.0": Config("cfg5_p0.9_T2.0", 128, 0.9, 2.0, 2, 10 ** 8, seed_for(5, 6), 4),
+    "cfg5_p0.8_T0.8": Config("cfg5_p0.8_T0.8", 128, 0.8, 0.8, 2, 10 ** 8, seed_for(5, 1), 8),
+    "cfg5_p0.9_T0.8": Config("cfg5_p0.9_T0.8", 128, 0.9, 0.8, 2, 10 ** 8, seed_for(5, 2), 8),
+    "cfg5_p1.0_T0.8": Config("cfg5_p1.0_T0.8", 128, 1.0, 0.8, 2, 10 ** 8, seed_for(5, 3), 8),
+    "cfg5_p0.5_T2.0": Config("cfg5_p0.5_T2.0", 128, 0.5, 2.0, 2, 10 ** 8, seed_for(5, 4), 8),
+    "cfg5_p0.8_T2.0": Config("cfg5_p0.8_T2.0", 128, 0.8, 2.0, 2, 10 ** 8, seed_for(5, 5), 8),
+    "cfg5_p0.9_T2.0": Config("cfg5_p0.9_T2.0", 128, 0.9, 2.0, 2, 10 ** 8, seed_for(5, 6), 8),
     "cfg5_p1.0_T2.0": Config("cfg5_p1.0_T2.0", 128, 1.0, 2.0, 2, 10 ** 8, seed_for(5, 7), 8),
 }
 

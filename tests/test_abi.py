@@ -135,3 +135,24 @@ def test_resident_row_schedules_are_consistent_on_the_host():
     """The RESIDENT kernel's host-built row tables satisfy their invariants; no device needed."""
     from paper_1411_5512_b200 import binding
     assert binding.lib().ea_selftest_host() == binding.EA_OK
+
+
+def test_pipe_microbenchmark_streams_hold_exactly_the_counted_instructions():
+    """ea_selftest_pipes reports warp instructions per second; the count it divides by is 8 (ILP) x 16 (unroll) per
+    loop trip.  Checked here, without a GPU, in the SASS of the library: each stream's loop body holds exactly 128
+    instructions of its kind (LOP3 / IMAD.WIDE.U32 / POPC; the mix holds 128 + 128) -- ptxas has not folded any."""
+    import subprocess
+    want = {0: {"LOP3": 128}, 1: {"IMAD.WIDE": 128}, 2: {"POPC": 128}, 3: {"LOP3": 128, "IMAD.WIDE": 128}}
+    for kind, ops in want.items():
+        name = "_ZN2ea13k_pipe_streamILi%dEEEvPjiPy" % kind
+        out = subprocess.run(["cuobjdump", "-sass", "-fun", name, binding.LIB_PATH], capture_output=True, text=True).stdout
+        lines = [m.groups() for m in re.finditer(r"/\*([0-9a-f]{4})\*/\s+(?:@!?U?P\d+\s+)?([A-Z0-9_.]+)([^;]*);", out)]
+        assert lines, "kernel %s not found in the library" % name
+        # the timed loop = from the target of the one backward branch to that branch
+        back = [(int(a, 16), int(re.search(r"0x([0-9a-f]+)", rest).group(1), 16)) for a, op, rest in lines
+                if op.startswith("BRA") and re.search(r"0x([0-9a-f]+)", rest) and int(re.search(r"0x([0-9a-f]+)", rest).group(1), 16) < int(a, 16)]
+        assert len(back) == 1, back
+        hi, lo = back[0]
+        body = [op for a, op, _ in lines if lo <= int(a, 16) <= hi]
+        for op, n in ops.items():
+            assert sum(1 for o in body if o.startswith(op)) == n, (kind, op, sum(1 for o in body if o.startswith(op)))

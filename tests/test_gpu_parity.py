@@ -170,21 +170,63 @@ def test_cfg3_energy_and_c4(name):
     assert_same_observables(g, o)
 
 
-@pytest.mark.parametrize("name", ["cfg4", "cfg5_p0.5_T0.8", "cfg5_p1.0_T2.0"])
+@pytest.mark.parametrize("name", ["cfg4"] + sorted(k for k in wl.CONFIGS if k.startswith("cfg5_")))
 def test_full_size_L128_every_word(name):
-    """The bench configuration (L=128, 32 x 2 replicas), AUTO kernel as bench.py launches it: every spin word
-    and every integer observable after a few sweeps."""
+    """cfg4 (the bench configuration) and ALL EIGHT (p, T) points of cfg5 (L=128, 32 x 2 replicas),
+    AUTO kernel exactly as bench.py launches it -- which must be the persistent RESIDENT kernel, in one launch of
+    >= 8 sweeps: the initial lattice, every spin word and every integer observable against the oracle."""
     c = wl.CONFIGS[name]
+    assert c.parity_sweeps >= 8                      # shorter AUTO calls go through the per-colour launches
     g, o = make_pair(c.L, c.p, c.T, c.n_replicas, c.seed, n_slots=1)
+    assert g.kernel == binding.EA_KERNEL_RESIDENT
     assert np.array_equal(g.get_bonds(), o.get_bonds())
     assert np.array_equal(g.get_spins(), o.get_spins())
     g.snapshot(0)
     o.snapshot(0)
     n = c.parity_sweeps
+    launches = g.launch_count
     g.sweep(n)
+    assert g.launch_count == launches + 1            # one persistent launch, not 2 n per-colour ones
     o.sweep(n)
     assert_same_state(g, o, "%s t=%d" % (name, n))
     assert_same_observables(g, o, slot=0)
+
+
+@pytest.mark.parametrize("which", ["spins", "bonds"])
+def test_resident_kernel_on_a_workspace_laid_across_a_4GiB_boundary(which):
+    """The persistent kernel must not depend on where the caller's workspace lies (round 1's did: its 32-bit address
+    arithmetic needed every array inside one 4 GiB window, and AUTO fell back silently otherwise).  Here the workspace
+    is placed so that the spin array / the bond array straddles a multiple of 4 GiB: RESIDENT must still be chosen
+    and must still match the oracle word for word."""
+    import torch
+    c = wl.CONFIGS["cfg4"]
+    need = binding.workspace_bytes(c.L, c.n_replicas, 0)
+    G4 = 1 << 32
+    buf = torch.empty(G4 + 2 * need + 4096, dtype=torch.uint8, device="cuda")
+    edge = (buf.data_ptr() + need + G4 - 1) // G4 * G4          # a 4 GiB line with >= `need` bytes on either side
+    spin_bytes, bond_bytes = 8 * c.N, 4 * 3 * c.N              # workspace layout: spins first, then the bond planes
+    start = edge - spin_bytes // 2 if which == "spins" else edge - spin_bytes - bond_bytes // 2
+    assert start % 256 == 0 and buf.data_ptr() <= start and start + need <= buf.data_ptr() + buf.numel()
+    torch.cuda.synchronize()
+    g = binding.Sim(c.L, c.p, c.T, n_replicas=c.n_replicas, seed=c.seed, n_slots=0, workspace=(start, buf))
+    o = Oracle(c.L, c.p, c.T, n_replicas=c.n_replicas, seed=c.seed, n_slots=0)
+    assert g.kernel == binding.EA_KERNEL_RESIDENT
+    g.sweep(8)
+    o.sweep(8)
+    assert_same_state(g, o, "workspace across a 4 GiB line (%s)" % which)
+    assert np.array_equal(g.energy(), o.energy())
+    g.close()
+
+
+def test_measured_pipe_rates_are_sane():
+    """ea_selftest_pipes (the measured integer roofline of bench.py): LOP3 on the alu pipe must come out near one warp
+    instruction per 2 clocks per sub-partition, and Philox's IMAD.WIDE must overlap with it (separate pipes)."""
+    r = binding.selftest_pipes()
+    per_clk_smsp = r["lop3_warp_inst_per_s"] / (r["n_sm"] * 4 * r["sm_mhz"] * 1e6)
+    assert 0.35 < per_clk_smsp < 0.55, r
+    assert r["imad_wide_warp_inst_per_s"] > 0.2 * r["lop3_warp_inst_per_s"], r
+    assert r["popc_warp_inst_per_s"] > 0.1 * r["lop3_warp_inst_per_s"], r
+    assert r["lop3_with_imad_wide_warp_inst_per_s"] > 0.5 * r["lop3_warp_inst_per_s"], r
 
 
 @pytest.mark.parametrize("n_rep,T,p", [(2, 0.8, 0.77), (1, 0.8, 0.5), (2, 2.0, 0.9), (2, float("inf"), 0.5), (1, 0.0, 0.6)])
