@@ -111,7 +111,7 @@ def parse_ncu_csv(path):
         except (TypeError, ValueError):
             continue
         scale = {"Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "byte": 1.0, "usecond": 1e-6, "msecond": 1e-3,
-                 "nsecond": 1e-9, "second": 1.0}.get(unit, 1.0)
+                 "nsecond": 1e-9, "ns": 1e-9, "us": 1e-6, "ms": 1e-3, "second": 1.0}.get(unit, 1.0)
         out[name] = v * scale
         out.setdefault("_kernel", row.get("Kernel Name"))
     return out

@@ -26,7 +26,7 @@ WorkspaceLayout workspace_layout(int L, int n_samples, int n_replicas, int n_slo
     w.off_stage = off;    off = align_up(off + N * 8);
     w.off_counters = off; off = align_up(off + w.n_counters * 8);
     w.off_time = off;     off = align_up(off + 8);
-    w.off_flags = off;    off = align_up(off + resident_flag_bytes());
+    w.off_flags = off;    off = align_up(off + resident_aux_bytes());
     w.off_fold = off;     off = align_up(off + fold_bytes(L, n_samples));
     w.total = off;
     return w;
@@ -273,6 +273,11 @@ ea_status ea_create_ex(const ea_params *prm, ea_sim **out)
             if (v > 0) s->resident_timeout_ns = (uint64_t)v * 1000000ull;
         }
         std::string why;
+        if (kernel_valid_for(EA_KERNEL_RESIDENT, L) && resident_supported(s, &why) && (e = resident_prepare(s, &why)) != cudaSuccess) {
+            fprintf(stderr, "ea_create_ex: %s\n", why.c_str());
+            rc = EA_ERR_CUDA;
+            break;
+        }
         if (prm->kernel == EA_KERNEL_AUTO && kernel_valid_for(EA_KERNEL_RESIDENT, L) && resident_supported(s, &why)) {
             s->kernel = EA_KERNEL_RESIDENT; // long runs in one persistent launch, short ones as ROWS launches
             s->resident_min_sweeps = RESIDENT_AUTO_MIN_SWEEPS;

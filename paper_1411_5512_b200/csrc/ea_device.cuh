@@ -160,6 +160,16 @@ struct Thresholds {
     uint32_t hb_always[7];
 };
 
+// one LOP3 with truth table LUT over (a, b, c) = (0xF0, 0xCC, 0xAA); plain asm (not volatile): free to schedule, but the
+// compiler cannot take the expression apart into two-input operations
+template <int LUT> __device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c)
+{
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(d) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+    return d;
+}
+constexpr int LUT_XOR3 = 0x96, LUT_MAJ = 0xE8, LUT_MAJ_NA = 0x8E; // a ^ b ^ c;  maj(a, b, c);  maj(~a, b, c)
+
 __device__ __forceinline__ uint32_t xor3(uint32_t a, uint32_t b, uint32_t c) { return a ^ b ^ c; }
 __device__ __forceinline__ uint32_t maj3(uint32_t a, uint32_t b, uint32_t c) { return (a & b) | (c & (a | b)); }
 
@@ -178,6 +188,14 @@ __device__ __forceinline__ HalfCount count_half(uint32_t u1, uint32_t u2, uint32
     HalfCount h;
     h.sa = xor3(u1, u2, u3); h.ka = maj3(u1, u2, u3);
     h.sb = xor3(u4, u5, u6); h.kb = maj3(u4, u5, u6);
+    return h;
+}
+
+__device__ __forceinline__ HalfCount count_half_lop3(uint32_t u1, uint32_t u2, uint32_t u3, uint32_t u4, uint32_t u5, uint32_t u6)
+{
+    HalfCount h;
+    h.sa = lop3<LUT_XOR3>(u1, u2, u3); h.ka = lop3<LUT_MAJ>(u1, u2, u3);
+    h.sb = lop3<LUT_XOR3>(u4, u5, u6); h.kb = lop3<LUT_MAJ>(u4, u5, u6);
     return h;
 }
 
@@ -259,16 +277,30 @@ __device__ __forceinline__ uint64_t metropolis_word(uint64_t s, uint64_t n1, uin
         return mk64(sl ^ fl, sh ^ fh);
     }
     if (RARE && !ALWAYS) {
-        const HalfCount hl = count_half(bond_lo(j1) ^ sl ^ lo32(n1), bond_lo(j2) ^ sl ^ lo32(n2), bond_lo(j3) ^ sl ^ lo32(n3),
-                                        bond_lo(j4) ^ sl ^ lo32(n4), bond_lo(j5) ^ sl ^ lo32(n5), bond_lo(j6) ^ sl ^ lo32(n6));
-        const HalfCount hh = count_half(bond_hi(j1) ^ sh ^ hi32(n1), bond_hi(j2) ^ sh ^ hi32(n2), bond_hi(j3) ^ sh ^ hi32(n3),
-                                        bond_hi(j4) ^ sh ^ hi32(n4), bond_hi(j5) ^ sh ^ hi32(n5), bond_hi(j6) ^ sh ^ hi32(n6));
-        uint32_t fl = maj3(hl.ka, hl.kb, hl.sa | hl.sb), fh = maj3(hh.ka, hh.kb, hh.sa | hh.sb);
+        // In terms of a_d = j_d ^ n_d (J S_nbr = -1 seen from an up spin) and n_a = their number, n_u = n_a for s = 0 and
+        // 6 - n_a for s = 1, so the NEW spin is  s' = [n_a >= 3 - l] (s = 0),  [n_a >= 4 + l] (s = 1),  l = 0..3 the number
+        // of thresholds above r.  With the two full adders n_a = sa + sb + 2 (ka + kb) and M(x; a, b) = maj(x, a, b)
+        // (x = 1: a | b, x = 0: a & b):   l = 0:  s' = maj(ka, kb, M(~s; sa, sb))      -- 12 LOP3 per half, no s ^ f
+        //   l = 1:  s' = M(~s; M(~s; ka, kb), M(s; sa, sb))     l = 2:  s' = M(~s; M(~s; ka, kb), M(~s; sa, sb))     l = 3:  ~s
+        const HalfCount hl = count_half_lop3(bond_lo(j1) ^ lo32(n1), bond_lo(j2) ^ lo32(n2), bond_lo(j3) ^ lo32(n3),
+                                             bond_lo(j4) ^ lo32(n4), bond_lo(j5) ^ lo32(n5), bond_lo(j6) ^ lo32(n6));
+        const HalfCount hh = count_half_lop3(bond_hi(j1) ^ hi32(n1), bond_hi(j2) ^ hi32(n2), bond_hi(j3) ^ hi32(n3),
+                                             bond_hi(j4) ^ hi32(n4), bond_hi(j5) ^ hi32(n5), bond_hi(j6) ^ hi32(n6));
+        const uint32_t tl = lop3<LUT_MAJ_NA>(sl, hl.sa, hl.sb), th_ = lop3<LUT_MAJ_NA>(sh, hh.sa, hh.sb);
+        uint32_t nl = lop3<LUT_MAJ>(hl.ka, hl.kb, tl), nh = lop3<LUT_MAJ>(hh.ka, hh.kb, th_);
         if (min(r_lo, r_hi) < th.thr[2]) {
-            fl = raise_half(fl, hl, r_lo, th);
-            fh = raise_half(fh, hh, r_hi, th);
+            if (r_lo < th.thr[2]) {
+                const uint32_t u = r_lo < th.thr[1] ? tl : lop3<LUT_MAJ>(sl, hl.sa, hl.sb);
+                nl = lop3<LUT_MAJ_NA>(sl, lop3<LUT_MAJ_NA>(sl, hl.ka, hl.kb), u);
+                if (r_lo < th.thr[0]) nl = ~sl;
+            }
+            if (r_hi < th.thr[2]) {
+                const uint32_t u = r_hi < th.thr[1] ? th_ : lop3<LUT_MAJ>(sh, hh.sa, hh.sb);
+                nh = lop3<LUT_MAJ_NA>(sh, lop3<LUT_MAJ_NA>(sh, hh.ka, hh.kb), u);
+                if (r_hi < th.thr[0]) nh = ~sh;
+            }
         }
-        return mk64(sl ^ fl, sh ^ fh);
+        return mk64(nl, nh);
     }
     const uint32_t fl = flip_half<ALWAYS>(bond_lo(j1) ^ sl ^ lo32(n1), bond_lo(j2) ^ sl ^ lo32(n2),
                                           bond_lo(j3) ^ sl ^ lo32(n3), bond_lo(j4) ^ sl ^ lo32(n4),

@@ -50,6 +50,7 @@ struct ea_sim {
     // RESIDENT kernel (L = 128): per-CTA step flags + abort word in the workspace, and the flag epoch
     unsigned *resident_flags = nullptr;
     uint32_t resident_epoch = 0;
+    int resident_tiles = 0;           // CTAs of the partition whose tile table sits behind the flags (0: none)
     uint64_t resident_min_sweeps = 1; // shorter ea_sweep calls use the ROWS launches (AUTO: 8)
     bool resident_used = false;       // a resident launch is in flight / unchecked: see check_resident()
     uint64_t resident_timeout_ns = 20000000000ull; // neighbour wait gives up after this (EA_RESIDENT_TIMEOUT_MS)
@@ -105,7 +106,9 @@ bool rows_persistent_valid(int L);
 cudaError_t launch_sweeps_rows_persistent(ea_sim *s, uint64_t t0, uint32_t n, cudaStream_t st);
 // RESIDENT (ea_sweep_resident.cu): n sweeps from sweep index t0 in one cooperative launch
 bool resident_supported(const ea_sim *s, std::string *why = nullptr);
-size_t resident_flag_bytes();
+size_t resident_flag_bytes();   // flag lines + abort line
+size_t resident_aux_bytes();    // flags + the tile table behind them (workspace)
+cudaError_t resident_prepare(ea_sim *s, std::string *why = nullptr); // build + upload the tile table (stream-ordered)
 bool resident_tables_ok();
 cudaError_t launch_sweeps_resident(ea_sim *s, uint64_t t0, uint32_t n, cudaStream_t st);
 

@@ -39,8 +39,10 @@ __global__ void __launch_bounds__(1024, 1) k_pipe_stream(uint32_t *out, const in
                     if (u & 1) asm volatile("lop3.b32 %0, %0, %1, %2, 0xe8;" : "+r"(a[i]) : "r"(a[(i + 1) % PIPE_ILP]), "r"(c));
                     else asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[i]) : "r"(a[(i + 1) % PIPE_ILP]), "r"(c));
                 }
-                if (KIND == PIPE_IMAD_WIDE || KIND == PIPE_MIX) // w = hi32(w) * M: the 32 x 32 -> 64 product of a Philox round (the high
-                    // word feeds the next one, so the chain cannot be folded into one multiply)
+                // w = hi32(w) * M: the 32 x 32 -> 64 product of a Philox round (the high word feeds the next one, so the
+                // chain cannot be folded into one multiply).  The mix issues one per four LOP3: the sweep kernel's ratio
+                // (ncu: 16 fma-pipe to 48 alu-pipe instructions per site word), where IMAD.WIDE (4 clocks) does not bind.
+                if (KIND == PIPE_IMAD_WIDE || (KIND == PIPE_MIX && i % 4 == 0))
                     asm volatile("mul.wide.u32 %0, %1, %2;" : "=l"(w[i]) : "r"((uint32_t)(w[i] >> 32)), "r"(0xD2511F53u));
                 if (KIND == PIPE_POPC)
                     asm volatile("popc.b32 %0, %0;" : "+r"(a[i]));
@@ -104,7 +106,7 @@ cudaError_t pipe_rates(int device, double out[8])
     e = time_stream<PIPE_LOP3>(n_sm, d_out, d_ticks, trips, &out[0], &mhz);
     if (e == cudaSuccess) e = time_stream<PIPE_IMAD_WIDE>(n_sm, d_out, d_ticks, trips, &out[1], nullptr);
     if (e == cudaSuccess) e = time_stream<PIPE_POPC>(n_sm, d_out, d_ticks, trips / 4, &out[2], nullptr);
-    if (e == cudaSuccess) e = time_stream<PIPE_MIX>(n_sm, d_out, d_ticks, trips, &out[3], nullptr); // LOP3 count; as many IMAD.WIDE
+    if (e == cudaSuccess) e = time_stream<PIPE_MIX>(n_sm, d_out, d_ticks, trips, &out[3], nullptr); // LOP3 count; one IMAD.WIDE per four LOP3 alongside
     out[4] = mhz;
     out[5] = (double)n_sm;
     out[6] = out[7] = 0.0;

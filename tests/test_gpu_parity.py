@@ -226,7 +226,8 @@ def test_measured_pipe_rates_are_sane():
     assert 0.35 < per_clk_smsp < 0.55, r
     assert r["imad_wide_warp_inst_per_s"] > 0.2 * r["lop3_warp_inst_per_s"], r
     assert r["popc_warp_inst_per_s"] > 0.1 * r["lop3_warp_inst_per_s"], r
-    assert r["lop3_with_imad_wide_warp_inst_per_s"] > 0.5 * r["lop3_warp_inst_per_s"], r
+    # one IMAD.WIDE (4 clocks on the fma pipe) per four LOP3 (2 clocks each on the alu pipe): the LOP3 rate must not drop
+    assert r["lop3_with_imad_wide_warp_inst_per_s"] > 0.85 * r["lop3_warp_inst_per_s"], r
 
 
 @pytest.mark.parametrize("n_rep,T,p", [(2, 0.8, 0.77), (1, 0.8, 0.5), (2, 2.0, 0.9), (2, float("inf"), 0.5), (1, 0.0, 0.6)])
