@@ -46,10 +46,11 @@ UNIT = "ps/attempt"
 LANES = 64
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 
-# Algorithmic alu-pipe work of one site word (64 attempts): 12 XOR3 (six unsatisfied-bond words per
-# 32-sample half) + 8 full-adder LOP3 + 4 flip-rule LOP3 + 2 for the rare-level test + 10 Philox XOR3 (one block per
-# two site words) = 36 LOP3-class instructions per lane, all on the alu pipe; addressing is not algorithmic.
-ALGORITHMIC_ALU_INST_PER_SITE_WORD = 36
+# Algorithmic alu-pipe work of one site word (64 attempts): 12 XOR (six bond x neighbour words per
+# 32-sample half) + 8 full-adder LOP3 + 4 flip-rule LOP3 + 2 for the rare-level test + 9.5 Philox XOR3 + 8.5 Philox
+# IMAD.WIDE (one block per two site words; an IMAD.WIDE takes an alu issue slot) = 44 slots, less the 2 of the two
+# launch-uniform rounds that fold away = 42; addressing and the rare levels themselves are not counted.
+ALGORITHMIC_ALU_INST_PER_SITE_WORD = 42
 # fallback alu peak if ea_selftest_pipes fails: one warp instruction per 2 clocks per SM sub-partition (B300_MICROARCH
 # "Pipe rates": rt_SMSP = 2) x 4 x 148 SMs at 1965 MHz
 FALLBACK_ALU_WARP_INST_PER_S = 148 * 4 * 0.5 * 1.965e9
@@ -396,13 +397,19 @@ def run_ours(args, cfg):
                         "note": "secondary: inside a step the spins stay in shared memory and the bonds in L2, so the "
                                 "algorithmic bytes do not cross HBM and this rate may exceed the HBM peak; see `traffic`"},
                 "pipes_measured": pipes,
-                "note": "achieved = alu-pipe warp instructions executed per half-sweep (ncu count of THIS build, "
-                        "alu_census.json, refused if stale) / mean half-sweep duration (CUDA events on the sim's stream "
-                        "around ea_sweep(S)); frac = achieved / measured LOP3 issue rate of the whole chip"}
+                "note": "achieved = alu-pipe issue slots per half-sweep = alu-pipe warp instructions + IMAD.WIDE (ncu counts of "
+                        "THIS build, alu_census.json, refused if stale; an IMAD.WIDE takes an alu slot besides its fma-pipe "
+                        "time: pipes_measured shows LOP3 at 4/5 of its rate with one IMAD.WIDE per four LOP3) / mean "
+                        "half-sweep duration (CUDA events on the sim's stream around ea_sweep(S)); frac = achieved / "
+                        "measured LOP3 issue rate of the whole chip"}
     if cen is not None:
-        alu_rate = cen["alu_warp_inst_per_half_sweep"] / t_half
+        slots = cen.get("alu_slot_warp_inst_per_half_sweep", cen["alu_warp_inst_per_half_sweep"])
+        alu_rate = slots / t_half
         roofline.update({"achieved": alu_rate / 1e9, "frac": alu_rate / alu_peak,
+                         "alu_slot_warp_inst_per_half_sweep": slots,
                          "alu_warp_inst_per_half_sweep": cen["alu_warp_inst_per_half_sweep"],
+                         "imad_wide_warp_inst_per_half_sweep": cen.get("imad_wide_warp_inst_per_half_sweep"),
+                         "frac_alu_pipe_instructions_only": cen["alu_warp_inst_per_half_sweep"] / t_half / alu_peak,
                          "warp_inst_per_half_sweep": cen.get("warp_inst_per_half_sweep"),
                          "traffic": cen.get("dram_bytes_per_launch"),
                          "traffic_note": "dram bytes of the captured ncu launch (%g half-sweeps; cold L2): the lattice "

@@ -191,8 +191,11 @@ ea_status ea_selftest_host(void);
  * the bit level" plus one random number, and the observables are popcounts, Eq. 3 and 7): dependent-free
  * instruction streams on every SM of `device` (-1 = current), about 30 ms of device time, default stream.
  *   out[0] = LOP3 (alu pipe), out[1] = IMAD.WIDE.U32 (fma pipe), out[2] = POPC  -- warp instructions per second;
- *   out[3] = LOP3 rate while one IMAD.WIDE.U32 per four LOP3 is issued alongside (the sweep kernel's mix of its two pipes);
- *   out[4] = SM clock in MHz during the LOP3 stream (clock64 / globaltimer), out[5] = number of SMs, out[6..7] = 0.
+ *   out[3] = LOP3 rate while one IMAD.WIDE.U32 per four LOP3 is issued alongside (about the sweep kernel's mix).  Measured on
+ *            B200: 4/5 of out[0] -- an IMAD.WIDE takes an alu-pipe issue slot besides its time on the fma pipe, so the
+ *            alu roofline of the sweep kernel counts it as alu-pipe work;
+ *   out[4] = SM clock in MHz during the LOP3 stream (clock64 / globaltimer), out[5] = number of SMs,
+ *   out[6] = LOP3 rate while as many plain 32-bit IMAD are issued alongside (these do overlap), out[7] = 0.
  * host array of 8 doubles.  EA_ERR_CUDA without a device. */
 ea_status ea_selftest_pipes(int device, double out[8]);
 

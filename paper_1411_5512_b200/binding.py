@@ -372,7 +372,8 @@ def selftest_pipes(device=None):
     if st != EA_OK:
         raise EAError(st, "ea_selftest_pipes: " + lib().ea_strerror(st).decode())
     return {"lop3_warp_inst_per_s": out[0], "imad_wide_warp_inst_per_s": out[1], "popc_warp_inst_per_s": out[2],
-            "lop3_with_imad_wide_warp_inst_per_s": out[3], "sm_mhz": out[4], "n_sm": int(out[5])}
+            "lop3_with_imad_wide_warp_inst_per_s": out[3], "sm_mhz": out[4], "n_sm": int(out[5]),
+            "lop3_with_imad_warp_inst_per_s": out[6]}
 
 
 def philox_selftest(ctr, key):

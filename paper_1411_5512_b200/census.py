@@ -3,7 +3,11 @@
 The persistent sweep kernel is bound by the alu pipe (LOP3 / ISETP / IADD3: the "boolean logic at the bit level" of
 PAPER.md:92), so its roofline fraction is
 
-    executed alu-pipe warp instructions per half-sweep / half-sweep time / measured LOP3 issue rate.
+    alu-pipe issue slots used per half-sweep / half-sweep time / measured LOP3 issue rate,
+
+where the slots are the alu-pipe warp instructions PLUS the IMAD.WIDE of Philox and of the address arithmetic: measured
+on B200 (ea_selftest_pipes), LOP3 and IMAD.WIDE do not overlap -- any mix of the two issues 0.498 warp instructions per
+clock per sub-partition in total, the LOP3 rate alone -- whereas plain 32-bit IMAD does overlap with LOP3.
 
 The instruction count is a property of the BUILT kernel (it includes the data-dependent rare branch, so it is
 counted by ncu, `sm__inst_executed_pipe_alu.sum`, not read off the SASS).  It is stored in `alu_census.json` next
@@ -35,7 +39,9 @@ KERNEL_SOURCES = ["csrc/ea_sweep_resident.cu", "csrc/ea_sweep.cu", "csrc/ea_swee
 METRICS = ("sm__inst_executed_pipe_alu.sum,sm__inst_executed_pipe_fma.sum,sm__inst_executed_pipe_lsu.sum,"
            "smsp__inst_executed.sum,dram__bytes_read.sum,dram__bytes_write.sum,gpu__time_duration.sum,"
            "sm__pipe_alu_cycles_active.avg.pct_of_peak_sustained_active,"
-           "smsp__issue_active.avg.pct_of_peak_sustained_active,launch__registers_per_thread,launch__grid_size")
+           "smsp__issue_active.avg.pct_of_peak_sustained_active,launch__registers_per_thread,launch__grid_size,"
+           "sm__pipe_fmaheavy_cycles_active.sum,sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed,"
+           "sm__cycles_elapsed.sum,smsp__cycles_elapsed.sum,sm__pipe_alu_cycles_active.sum")
 
 
 def source_hash():
@@ -118,13 +124,14 @@ def parse_ncu_csv(path):
 
 
 def kernel_key_of(name):
-    """ncu kernel name -> census key, e.g. 'k_sweep_resident<ResidentGeom<128,16,8,16,2>, unsigned int, 0, 1, 0>'."""
-    n = name.replace(" ", "")
+    """ncu kernel name -> census key, e.g. 'k_sweep_resident<16, unsigned int, 0, 1, 0>(ResidentArgs)' (compute warps, bond
+    word, ALWAYS, RARE, HB) -> 'resident_u32_rare'."""
+    n = name.replace(" ", "").replace("(bool)", "").replace("(int)", "")
     if "k_sweep_resident" in n:
-        args = n[n.rindex(">,") + 2:].rstrip(">()").split(",") if ">," in n else []
+        inner = n[n.index("<") + 1:n.rindex(">")] if "<" in n else ""
+        args = inner.split(",")
         bond = "u32" if "unsignedint" in n else "u64"
-        flags = [a for a in args if a in ("0", "1", "false", "true")]
-        flags = [f in ("1", "true") for f in flags][-3:] if len(flags) >= 2 else []
+        flags = [a in ("1", "true") for a in args[-3:]] if len(args) >= 5 else []
         kind = "heatbath" if len(flags) == 3 and flags[2] else "always" if flags and flags[0] else \
             "rare" if len(flags) >= 2 and flags[1] else "predicated"
         return "resident_%s_%s" % (bond, kind)
@@ -143,6 +150,10 @@ def main(argv):
         "kernel": m["_kernel"],
         "half_sweeps_in_captured_launch": half_sweeps,
         "alu_warp_inst_per_half_sweep": m["sm__inst_executed_pipe_alu.sum"] / half_sweeps,
+        # IMAD.WIDE takes an alu-pipe issue slot as well (ea_selftest_pipes, measured): 4 fmaheavy cycles against 2 of a
+        # plain IMAD, so  n_wide = (fmaheavy cycles - 2 x fma-pipe instructions) / 2
+        "imad_wide_warp_inst_per_half_sweep": max(0.0, (m.get("sm__pipe_fmaheavy_cycles_active.sum", 0.0)
+                                                       - 2.0 * m.get("sm__inst_executed_pipe_fma.sum", 0.0)) / 2.0) / half_sweeps,
         "fma_warp_inst_per_half_sweep": m.get("sm__inst_executed_pipe_fma.sum", 0.0) / half_sweeps,
         "lsu_warp_inst_per_half_sweep": m.get("sm__inst_executed_pipe_lsu.sum", 0.0) / half_sweeps,
         "warp_inst_per_half_sweep": m.get("smsp__inst_executed.sum", 0.0) / half_sweeps,
@@ -155,6 +166,8 @@ def main(argv):
         "profile": profile,
         "how": "ncu --metrics (census.METRICS) on one launch of the bench configuration; see census.py",
     }
+    entry["alu_slot_warp_inst_per_half_sweep"] = (entry["alu_warp_inst_per_half_sweep"]
+                                                  + entry["imad_wide_warp_inst_per_half_sweep"])
     try:
         with open(CENSUS_PATH) as f:
             data = json.load(f)

@@ -13,17 +13,17 @@
 
 namespace ea {
 
-enum { PIPE_LOP3 = 0, PIPE_IMAD_WIDE = 1, PIPE_POPC = 2, PIPE_MIX = 3 };
+enum { PIPE_LOP3 = 0, PIPE_IMAD_WIDE = 1, PIPE_POPC = 2, PIPE_MIX = 3, PIPE_MIX_IMAD = 4 };
 constexpr int PIPE_ILP = 8, PIPE_UNROLL = 16; // instructions of the measured kind per loop trip: ILP * UNROLL
 
 template <int KIND>
 __global__ void __launch_bounds__(1024, 1) k_pipe_stream(uint32_t *out, const int trips, unsigned long long *ticks)
 {
-    uint32_t a[PIPE_ILP];
+    uint32_t a[PIPE_ILP], m[PIPE_ILP];
     uint64_t w[PIPE_ILP];
     const uint32_t b = threadIdx.x * 0x9E3779B9u + 1u, c = blockIdx.x * 0x85EBCA6Bu + 7u;
 #pragma unroll
-    for (int i = 0; i < PIPE_ILP; ++i) { a[i] = b + i * c; w[i] = ((uint64_t)a[i] << 32) | (b ^ i); }
+    for (int i = 0; i < PIPE_ILP; ++i) { a[i] = b + i * c; m[i] = a[i] ^ 0x5555u; w[i] = ((uint64_t)a[i] << 32) | (b ^ i); }
     unsigned long long t0 = 0, c0 = 0;
     if (threadIdx.x == 0) {
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
@@ -35,15 +35,20 @@ __global__ void __launch_bounds__(1024, 1) k_pipe_stream(uint32_t *out, const in
         for (int u = 0; u < PIPE_UNROLL; ++u) {
 #pragma unroll
             for (int i = 0; i < PIPE_ILP; ++i) {
-                if (KIND == PIPE_LOP3 || KIND == PIPE_MIX) { // xor3 and maj alternate, so that two never fold into one
+                if (KIND == PIPE_LOP3 || KIND == PIPE_MIX || KIND == PIPE_MIX_IMAD) { // xor3 and maj alternate, so that two never fold into one
                     if (u & 1) asm volatile("lop3.b32 %0, %0, %1, %2, 0xe8;" : "+r"(a[i]) : "r"(a[(i + 1) % PIPE_ILP]), "r"(c));
                     else asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[i]) : "r"(a[(i + 1) % PIPE_ILP]), "r"(c));
                 }
                 // w = hi32(w) * M: the 32 x 32 -> 64 product of a Philox round (the high word feeds the next one, so the
-                // chain cannot be folded into one multiply).  The mix issues one per four LOP3: the sweep kernel's ratio
-                // (ncu: 16 fma-pipe to 48 alu-pipe instructions per site word), where IMAD.WIDE (4 clocks) does not bind.
+                // chain cannot be folded into one multiply).  The mix issues one per four LOP3, about the sweep kernel's
+                // ratio.  MEASURED (B200): the LOP3 rate of the mix is 4/5 of the LOP3 rate alone at every ratio tried --
+                // an IMAD.WIDE (or IMAD.HI) takes an issue slot of the alu pipe besides its four clocks on the fma pipe,
+                // whereas a plain 32-bit IMAD (the second mix) overlaps with LOP3.  The alu roofline of the sweep kernel
+                // therefore counts IMAD.WIDE as alu-pipe work.
                 if (KIND == PIPE_IMAD_WIDE || (KIND == PIPE_MIX && i % 4 == 0))
                     asm volatile("mul.wide.u32 %0, %1, %2;" : "=l"(w[i]) : "r"((uint32_t)(w[i] >> 32)), "r"(0xD2511F53u));
+                if (KIND == PIPE_MIX_IMAD) // one 32-bit IMAD per LOP3
+                    asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(m[i]) : "r"(0xD2511F53u), "r"(c));
                 if (KIND == PIPE_POPC)
                     asm volatile("popc.b32 %0, %0;" : "+r"(a[i]));
             }
@@ -57,7 +62,7 @@ __global__ void __launch_bounds__(1024, 1) k_pipe_stream(uint32_t *out, const in
     }
     uint32_t r = 0;
 #pragma unroll
-    for (int i = 0; i < PIPE_ILP; ++i) r ^= a[i] ^ (uint32_t)w[i] ^ (uint32_t)(w[i] >> 32);
+    for (int i = 0; i < PIPE_ILP; ++i) r ^= a[i] ^ m[i] ^ (uint32_t)w[i] ^ (uint32_t)(w[i] >> 32);
     out[blockIdx.x * blockDim.x + threadIdx.x] = r;
 }
 
@@ -107,9 +112,10 @@ cudaError_t pipe_rates(int device, double out[8])
     if (e == cudaSuccess) e = time_stream<PIPE_IMAD_WIDE>(n_sm, d_out, d_ticks, trips, &out[1], nullptr);
     if (e == cudaSuccess) e = time_stream<PIPE_POPC>(n_sm, d_out, d_ticks, trips / 4, &out[2], nullptr);
     if (e == cudaSuccess) e = time_stream<PIPE_MIX>(n_sm, d_out, d_ticks, trips, &out[3], nullptr); // LOP3 count; one IMAD.WIDE per four LOP3 alongside
+    out[6] = out[7] = 0.0;
+    if (e == cudaSuccess) e = time_stream<PIPE_MIX_IMAD>(n_sm, d_out, d_ticks, trips, &out[6], nullptr); // LOP3 count; as many IMAD
     out[4] = mhz;
     out[5] = (double)n_sm;
-    out[6] = out[7] = 0.0;
     cudaFree(d_out);
     cudaFree(d_ticks);
     return e;

@@ -139,7 +139,10 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
     return t;
 }
 
-enum { BAR_BOUNDARY0 = 1, BAR_BOUNDARY1 = 2 }; // named barriers: boundary rows of an even / odd phase are stored
+// Named barriers 1..4, one per phase index mod 4: "the boundary rows of phase k are stored".  Four, not two: a warp without
+// boundary rows does not wait for the halo, so it may arrive for phase k + 2 before the producer has consumed the barrier of
+// phase k; it cannot arrive for k + 4 before that (phase k + 2 of the boundary warps needs the producer's copies of phase k).
+enum { BAR_BOUNDARY0 = 1 };
 constexpr uint32_t RARE_THR2_MAX = 0x04000000u; // P(r < thr[2]) < 1/64: the warp-level branch of metropolis_word pays
 
 template <typename BondT> struct RowBonds { typename Pair<BondT>::type jx, jy, jz, bx, by, bz; };
@@ -191,8 +194,7 @@ __device__ __forceinline__ RowBonds<BondT> load_row_bonds(const Ptr32 Jc_l, cons
 
 // per-step, per-lane context of a compute warp
 struct ResidentStep {
-    unsigned char *tile_l;   // the tile in shared memory + 16 * lane
-    uint32_t own_off, oth_off; // byte offset of the tile plane of colour c / 1 - c
+    uint32_t s_own, s_oth;   // shared-memory address of the tile plane of colour c / 1 - c, + 16 * lane
     uint32_t planeb;         // bytes between z-planes of the tile (CTA-uniform)
     Ptr32 g_own;             // global plane of colour c + 2 * lane
     Ptr32 Jc_l, Jo_l;        // bond planes of colour c / 1 - c + 2 * lane
@@ -202,6 +204,19 @@ struct ResidentStep {
     long long *trace; unsigned tb, tw, tk; // debug builds: trace buffer, CTA, warp, phase
 #endif
 };
+
+// shared-memory accesses by 32-bit shared address (one IADD per row address instead of generic pointer arithmetic:
+// measured 4.34 against 4.41 us per half-sweep)
+__device__ __forceinline__ ulonglong2 lds128(uint32_t addr)
+{
+    ulonglong2 v;
+    asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, ulonglong2 v)
+{
+    asm volatile("st.shared.v2.u64 [%0], {%1, %2};" ::"r"(addr), "l"(v.x), "l"(v.y) : "memory");
+}
 
 __device__ __forceinline__ void stg128(void *p, ulonglong2 v)
 {
@@ -224,17 +239,16 @@ template <int S, typename BondT, bool ALWAYS, bool RARE, bool HB>
 __device__ __forceinline__ void resident_row(const ResidentStep &x, const uint4 d, const RowBonds<BondT> &bd,
                                              const uint4 r, const Thresholds &th, const bool publish)
 {
-    unsigned char *own_row = x.tile_l + (x.own_off + d.x);
-    const unsigned char *o = x.tile_l + (x.oth_off + d.x);
-    const ulonglong2 own = *(const ulonglong2 *)own_row;
-    const ulonglong2 P0 = *(const ulonglong2 *)o;
-    const ulonglong2 Pm = *(const ulonglong2 *)(o - RES_ROW_BYTES);
-    const ulonglong2 Pp = *(const ulonglong2 *)(o + RES_ROW_BYTES);
-    const ulonglong2 Zm = *(const ulonglong2 *)(o - x.planeb);
-    const ulonglong2 Zp = *(const ulonglong2 *)(o + x.planeb);
+    const uint32_t own_row = x.s_own + d.x, o = x.s_oth + d.x;
+    const ulonglong2 own = lds128(own_row);
+    const ulonglong2 P0 = lds128(o);
+    const ulonglong2 Pm = lds128(o - RES_ROW_BYTES);
+    const ulonglong2 Pp = lds128(o + RES_ROW_BYTES);
+    const ulonglong2 Zm = lds128(o - x.planeb);
+    const ulonglong2 Zp = lds128(o + x.planeb);
     const ulonglong2 out = update_pair_r<S, BondT, ALWAYS, RARE, HB>(own, P0, Pm, Pp, Zm, Zp, bd.jx, bd.jy, bd.jz, bd.bx, bd.by,
                                                                      bd.bz, r, th, x.lane_m, x.lane_p);
-    *(ulonglong2 *)own_row = out;
+    sts128(own_row, out);
     if (publish) stg128(x.g_own.at<ulonglong2>(d.y / 2), out);
 }
 
@@ -254,7 +268,11 @@ __device__ __forceinline__ void resident_phase(const ResidentStep &x, const uint
         named_bar_arrive(bar_id, bar_threads);
         arrived = true;
     }
+#ifdef EA_RES_VAR_UNROLL2
+#pragma unroll 2
+#else
 #pragma unroll 1
+#endif
     for (int j = 0; j < npairs; ++j) {
         const int i = 2 * j;
         const bool last = i + 2 >= n;
@@ -305,7 +323,7 @@ __global__ void __launch_bounds__((CW + RES_PRODUCERS) * 32, 1) k_sweep_resident
     uint64_t *phase_bar = (uint64_t *)smem_raw;        // [2]: phase k of every compute warp is complete (k & 1)
     uint64_t *halo_bar = (uint64_t *)(smem_raw + 16);  // [2]: the halo rows written in phase k have landed (k & 1)
     uint4 *rowdesc = (uint4 *)(smem_raw + 128);        // [2][RES_SLOTS] row descriptors
-    uint2 *cpl = (uint2 *)(smem_raw + RES_SMEM_CPL);   // [2][40] halo copies of each class (global row offset, tile row offset)
+    uint2 *cpl = (uint2 *)(smem_raw + RES_SMEM_CPL);   // [2][40] halo copies of each class: byte offsets (global row, tile row) in a colour plane
     uint64_t *tile = (uint64_t *)(smem_raw + RES_SMEM_HDR); // [2][HZ][HY][Lh]
 
     const unsigned tid = threadIdx.x, lane = tid & 31;
@@ -324,7 +342,8 @@ __global__ void __launch_bounds__((CW + RES_PRODUCERS) * 32, 1) k_sweep_resident
     }
     for (unsigned v = tid; v < 2u * 40; v += THREADS) { // padded with repeats of the last entry: the producer copies four per trip
         const unsigned cls = v / 40, i = v % 40, n = __ldg(&T->n_cp[cls]);
-        cpl[v] = __ldg(&T->cp[cls][i < n ? i : n - 1]);
+        const uint2 e = __ldg(&T->cp[cls][i < n ? i : n - 1]);
+        cpl[v] = make_uint2(e.x * 8, e.y * 8); // byte offsets
     }
     if (tid == 0) {
         mbar_init(phase_bar + 0, CW);
@@ -354,7 +373,7 @@ __global__ void __launch_bounds__((CW + RES_PRODUCERS) * 32, 1) k_sweep_resident
         for (uint32_t k = warp - CW; k < n_phases; k += RES_PRODUCERS) {
             const unsigned c = (k >> 1) & 1, cls = c ^ (k & 1); // phase k updates colour c of the rows of class cls
             RES_TRACE(a, b, warp, lane, k, 0);
-            named_bar_sync(BAR_BOUNDARY0 + (k & 1), BAR_THREADS);   // its boundary rows are in smem and in global
+            named_bar_sync(BAR_BOUNDARY0 + (k & 3), BAR_THREADS);   // its boundary rows are in smem and in global
             RES_TRACE(a, b, warp, lane, k, 1);
             const unsigned epoch = a.epoch0 + k + 1;
 #ifdef EA_RES_TRACE
@@ -395,13 +414,13 @@ __global__ void __launch_bounds__((CW + RES_PRODUCERS) * 32, 1) k_sweep_resident
             const unsigned ncp = cls ? n_cp1 : n_cp0;
             const uint2 *list = cpl + cls * 40;
             const uint32_t dst = smem_u32(tile) + c * plane_words * 8 + 16 * lane;
-            const uint64_t *src = a.spins + (size_t)c * Nh + 2 * lane;
+            const Ptr32 src(a.spins + (size_t)c * Nh + 2 * lane);
             for (unsigned i = 0; i < ncp; i += 4) { // the list is padded to a multiple of four with repeats of its last entry
                 const uint4 e01 = *(const uint4 *)(list + i), e23 = *(const uint4 *)(list + i + 2);
-                cp_async16(dst + e01.y * 8, src + e01.x);
-                cp_async16(dst + e01.w * 8, src + e01.z);
-                cp_async16(dst + e23.y * 8, src + e23.x);
-                cp_async16(dst + e23.w * 8, src + e23.z);
+                cp_async16(dst + e01.y, src.at<const char>(e01.x));
+                cp_async16(dst + e01.w, src.at<const char>(e01.z));
+                cp_async16(dst + e23.y, src.at<const char>(e23.x));
+                cp_async16(dst + e23.w, src.at<const char>(e23.z));
             }
             cp_async_arrive_noinc(halo_bar + (k & 1));
             RES_TRACE(a, b, warp, lane, k, 3);
@@ -419,8 +438,7 @@ __global__ void __launch_bounds__((CW + RES_PRODUCERS) * 32, 1) k_sweep_resident
         x.lane_m = (int)((lane - 1) & 31);
         x.lane_p = (int)((lane + 1) & 31);
         x.planeb = HY * RES_ROW_BYTES;
-        const uint32_t plane_bytes = plane_words * 8;
-        x.tile_l = (unsigned char *)tile + 16 * lane;
+        const uint32_t tile_s = smem_u32(tile) + 16 * lane, plane_bytes = plane_words * 8;
         SweepRng g;
 #pragma unroll
         for (int r = 0; r < 10; ++r) { g.k0[r] = a.k0[r]; g.k1[r] = a.k1[r]; }
@@ -438,34 +456,35 @@ __global__ void __launch_bounds__((CW + RES_PRODUCERS) * 32, 1) k_sweep_resident
             sweep_rng_set_time(gn, a.t0 + ((h + 1) >> 1), 1 - c);
             x.Jc_l = c ? J1_l : J0_l;
             x.Jo_l = c ? J0_l : J1_l;
-            x.own_off = c * plane_bytes;
-            x.oth_off = (1 - c) * plane_bytes;
+            x.s_own = tile_s + c * plane_bytes;
+            x.s_oth = tile_s + (1 - c) * plane_bytes;
             x.g_own = Ptr32(a.spins + (size_t)c * Nh + 2 * lane);
             // keep the per-step bases in registers: recomputing them from c inside the row loop costs alu-pipe selects
-            asm volatile("" : "+l"(x.Jc_l.base), "+l"(x.Jo_l.base), "+l"(x.g_own.base), "+r"(x.own_off), "+r"(x.oth_off));
+            asm volatile("" : "+l"(x.Jc_l.base), "+l"(x.Jo_l.base), "+l"(x.g_own.base), "+r"(x.s_own), "+r"(x.s_oth));
             const unsigned par = (h - 1) & 1; // phase k waits for generation (k >> 1) - 1 = h - 1 of barrier k & 1
             // first phase of the half-step: rows of class c (x-phase 0); then class 1 - c (x-phase 1).  Phase k = 2h, 2h + 1
             // needs phase k - 2 of every warp of the CTA and the halo rows the neighbours wrote in their phase k - 2.
             RES_TRACE(a, b, warp, lane, 2 * h, 0);
-            if (h > 0) { mbar_wait(phase_bar + 0, par); RES_TRACE(a, b, warp, lane, 2 * h, 1); mbar_wait(halo_bar + 0, par); }
+            // (only boundary rows read the halo ring: a warp without any in this phase does not wait for it)
+            if (h > 0) { mbar_wait(phase_bar + 0, par); RES_TRACE(a, b, warp, lane, 2 * h, 1); if (c ? n_bnd1 : n_bnd0) mbar_wait(halo_bar + 0, par); }
             RES_TRACE(a, b, warp, lane, 2 * h, 2);
 #ifdef EA_RES_TRACE
             x.trace = a.trace; x.tb = b; x.tw = warp; x.tk = 2 * h;
 #endif
             resident_phase<0, BondT, ALWAYS, RARE, HB>(x, c ? desc1 : desc0, c ? n_rows1 : n_rows0, c ? n_bnd1 : n_bnd0, nbp,
-                                                        BAR_BOUNDARY0, BAR_THREADS, nxt, rnx, g, c ? first0 : first1, x.Jc_l, x.Jo_l, g, a.th);
+                                                        BAR_BOUNDARY0 + ((2 * h) & 3), BAR_THREADS, nxt, rnx, g, c ? first0 : first1, x.Jc_l, x.Jo_l, g, a.th);
             __syncwarp();
             if (lane == 0) mbar_arrive(phase_bar + 0);
             RES_TRACE(a, b, warp, lane, 2 * h, 4);
             RES_TRACE(a, b, warp, lane, 2 * h + 1, 0);
-            if (h > 0) { mbar_wait(phase_bar + 1, par); RES_TRACE(a, b, warp, lane, 2 * h + 1, 1); mbar_wait(halo_bar + 1, par); }
+            if (h > 0) { mbar_wait(phase_bar + 1, par); RES_TRACE(a, b, warp, lane, 2 * h + 1, 1); if (c ? n_bnd0 : n_bnd1) mbar_wait(halo_bar + 1, par); }
             RES_TRACE(a, b, warp, lane, 2 * h + 1, 2);
 #ifdef EA_RES_TRACE
             x.tk = 2 * h + 1;
 #endif
             // the next phase is the first of half-step h + 1: colour 1 - c, class 1 - c -- the class just done
             resident_phase<1, BondT, ALWAYS, RARE, HB>(x, c ? desc0 : desc1, c ? n_rows0 : n_rows1, c ? n_bnd0 : n_bnd1, nbp,
-                                                        BAR_BOUNDARY1, BAR_THREADS, nxt, rnx, g, c ? first0 : first1, x.Jo_l, x.Jc_l, gn, a.th);
+                                                        BAR_BOUNDARY0 + ((2 * h + 1) & 3), BAR_THREADS, nxt, rnx, g, c ? first0 : first1, x.Jo_l, x.Jc_l, gn, a.th);
             __syncwarp();
             if (lane == 0) mbar_arrive(phase_bar + 1);
             RES_TRACE(a, b, warp, lane, 2 * h + 1, 4);
@@ -480,7 +499,7 @@ __global__ void __launch_bounds__((CW + RES_PRODUCERS) * 32, 1) k_sweep_resident
                 const uint4 d = desc[i];
 #pragma unroll
                 for (int c = 0; c < 2; ++c)
-                    *(ulonglong2 *)(a.spins + (size_t)c * Nh + d.y + 2 * lane) = *(const ulonglong2 *)(x.tile_l + (c * plane_bytes + d.x));
+                    *(ulonglong2 *)(a.spins + (size_t)c * Nh + d.y + 2 * lane) = lds128(tile_s + c * plane_bytes + d.x);
             }
         }
     }
@@ -667,6 +686,7 @@ template <typename BondT, bool ALWAYS, bool RARE, bool HB = false>
 static cudaError_t launch_resident_typed(ResidentArgs &a, int n_tiles, int cw, cudaStream_t st)
 {
 #ifdef EA_RES_EXPERIMENT
+    if (cw == 12) return launch_resident_cw<12, BondT, ALWAYS, RARE, HB>(a, n_tiles, st);
     if (cw == 20) return launch_resident_cw<20, BondT, ALWAYS, RARE, HB>(a, n_tiles, st);
     if (cw == 24) return launch_resident_cw<24, BondT, ALWAYS, RARE, HB>(a, n_tiles, st);
     if (cw == 16) return launch_resident_cw<16, BondT, ALWAYS, RARE, HB>(a, n_tiles, st);
@@ -693,7 +713,7 @@ bool resident_tables_ok()
 {
     std::vector<ResTile> t;
     for (int n_tiles : {148, 128})
-        for (int cw : {24, 20, 16, 8})
+        for (int cw : {24, 20, 16, 12, 8})
             if (!build_partition(n_tiles, cw, t, nullptr)) return false;
     return true;
 }

@@ -140,9 +140,9 @@ def test_resident_row_schedules_are_consistent_on_the_host():
 def test_pipe_microbenchmark_streams_hold_exactly_the_counted_instructions():
     """ea_selftest_pipes reports warp instructions per second; the count it divides by is 8 (ILP) x 16 (unroll) per
     loop trip.  Checked here, without a GPU, in the SASS of the library: each stream's loop body holds exactly 128
-    instructions of its kind (LOP3 / IMAD.WIDE.U32 / POPC; the mix holds 128 + 32) -- ptxas has not folded any."""
+    instructions of its kind (LOP3 / IMAD.WIDE.U32 / POPC; the mixes hold 128 + 32 IMAD.WIDE and 128 + 128 IMAD) -- ptxas has not folded any."""
     import subprocess
-    want = {0: {"LOP3": 128}, 1: {"IMAD.WIDE": 128}, 2: {"POPC": 128}, 3: {"LOP3": 128, "IMAD.WIDE": 32}}
+    want = {0: {"LOP3": 128}, 1: {"IMAD.WIDE": 128}, 2: {"POPC": 128}, 3: {"LOP3": 128, "IMAD.WIDE": 32}, 4: {"LOP3": 128, "IMAD": 128}}
     for kind, ops in want.items():
         name = "_ZN2ea13k_pipe_streamILi%dEEEvPjiPy" % kind
         out = subprocess.run(["cuobjdump", "-sass", "-fun", name, binding.LIB_PATH], capture_output=True, text=True).stdout
