@@ -61,8 +61,12 @@ typedef enum {
                                that sees nothing for EA_RESIDENT_TIMEOUT_MS (environment, read at ea_create;
                                default 20000) gives up, and the next synchronising call returns EA_ERR_CUDA */
     EA_KERNEL_FOLD = 5,    /* what a sim with n_samples < 64 runs (not selectable)        */
-    EA_KERNEL_ROWS_PERSISTENT = 6 /* ROWS with a grid barrier per colour, one launch per ea_sweep (L = 16, 32, 64);
+    EA_KERNEL_ROWS_PERSISTENT = 6, /* ROWS with a grid barrier per colour, one launch per ea_sweep (L = 16, 32, 64);
                                      measured slower than the graph replays, never chosen by AUTO */
+    EA_KERNEL_SMALL = 7   /* small lattices (L % 4 == 0, L <= 32): spins and bonds resident in the shared memory of one
+                             CTA (L <= 16) or of one thread-block cluster (L = 32: 16 CTAs, neighbouring planes read
+                             through distributed shared memory, cluster barrier per colour); one launch per ea_sweep.
+                             AUTO uses it for ea_sweep(n >= 2); shorter calls go as per-colour launches */
 } ea_kernel;
 
 /* Single-spin dynamics.  The paper uses Metropolis (Eq. 9); heat bath is the variant of SURVEY 8(f)

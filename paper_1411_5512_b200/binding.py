@@ -13,8 +13,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libea_b200.so")
 
 EA_OK, EA_ERR_INVALID, EA_ERR_CUDA, EA_ERR_NOMEM, EA_ERR_STATE = range(5)
-EA_KERNEL_AUTO, EA_KERNEL_SCALAR, EA_KERNEL_VEC2, EA_KERNEL_ROWS, EA_KERNEL_RESIDENT, EA_KERNEL_FOLD, EA_KERNEL_ROWS_PERSISTENT = range(7)
-KERNEL_NAMES = {"auto": 0, "scalar": 1, "vec2": 2, "rows": 3, "resident": 4, "rows_persistent": 6}
+EA_KERNEL_AUTO, EA_KERNEL_SCALAR, EA_KERNEL_VEC2, EA_KERNEL_ROWS, EA_KERNEL_RESIDENT, EA_KERNEL_FOLD, EA_KERNEL_ROWS_PERSISTENT, \
+    EA_KERNEL_SMALL = range(8)
+KERNEL_NAMES = {"auto": 0, "scalar": 1, "vec2": 2, "rows": 3, "resident": 4, "rows_persistent": 6, "small": 7}
 LANES = 64
 
 

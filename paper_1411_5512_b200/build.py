@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libea_b200.so")
-SOURCES = ["ea_api.cu", "ea_sweep.cu", "ea_sweep_resident.cu", "ea_setup.cu", "ea_observables.cu",
+SOURCES = ["ea_api.cu", "ea_sweep.cu", "ea_sweep_resident.cu", "ea_sweep_small.cu", "ea_setup.cu", "ea_observables.cu",
            "ea_c4_vectors.cu", "ea_fold.cu", "ea_pipes.cu"]
 HEADERS = ["ea_device.cuh", "ea_sweep_common.cuh", "ea_internal.h", os.path.join("..", "..", "include", "ea.h")]
 ARCH_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a"]

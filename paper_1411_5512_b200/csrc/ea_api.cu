@@ -120,6 +120,7 @@ static ea_status stream_sync(ea_sim *s)
     } while (0)
 
 static const uint64_t RESIDENT_AUTO_MIN_SWEEPS = 8;     // AUTO: below this the prologue/epilogue of the persistent kernel does not pay
+static const uint64_t SMALL_AUTO_MIN_SWEEPS = 2;         // AUTO: a single sweep is two direct launches
 static const uint64_t PERSISTENT_MIN_SWEEPS = 4;         // ROWS_PERSISTENT: below this the per-colour launches are as good
 static const uint64_t RESIDENT_MAX_SWEEPS = 1u << 20;   // sweeps per persistent launch (about 10 s of device time)
 
@@ -133,6 +134,7 @@ static bool kernel_valid_for(int kernel, int L)
     case EA_KERNEL_ROWS: return L == 16 || L == 32 || L == 64 || L == 128;
     case EA_KERNEL_RESIDENT: return L == 128; // plus a device check (resident_supported) once the sim exists
     case EA_KERNEL_ROWS_PERSISTENT: return rows_persistent_valid(L);
+    case EA_KERNEL_SMALL: return small_cluster_size(L, 1) > 0; // plus a device check (small_supported)
     case EA_KERNEL_FOLD: return false;        // not selectable: it is what a sim with n_samples < 64 runs
     default: return false;
     }
@@ -285,6 +287,13 @@ ea_status ea_create_ex(const ea_params *prm, ea_sim **out)
             fprintf(stderr, "ea_create_ex: %s\n", why.c_str()); // no handle to carry the message yet
             rc = EA_ERR_INVALID;
             break;
+        } else if (prm->kernel == EA_KERNEL_AUTO && prm->n_samples == EA_LANES && kernel_valid_for(EA_KERNEL_SMALL, L) && small_supported(s)) {
+            s->kernel = EA_KERNEL_SMALL; // calls of two sweeps or more in one launch, lattice in shared memory
+            s->resident_min_sweeps = SMALL_AUTO_MIN_SWEEPS;
+        } else if (s->kernel == EA_KERNEL_SMALL && !small_supported(s, &why)) {
+            fprintf(stderr, "ea_create_ex: %s\n", why.c_str());
+            rc = EA_ERR_INVALID;
+            break;
         }
         s->h_counters.resize(w.n_counters);
         if ((e = launch_init_bonds(s)) != cudaSuccess) { rc = EA_ERR_CUDA; break; }
@@ -362,6 +371,15 @@ ea_status ea_sweep(ea_sim *sim, uint64_t n)
             const uint32_t chunk = (uint32_t)(left < RESIDENT_MAX_SWEEPS ? left : RESIDENT_MAX_SWEEPS);
             EA_CUDA(sim, launch_sweeps_resident(sim, sim->t, chunk, sim->stream));
             sim->resident_used = true;
+            sim->t += chunk;
+            left -= chunk;
+        }
+        return EA_OK;
+    }
+    if (sim->kernel == EA_KERNEL_SMALL && n >= sim->resident_min_sweeps) {
+        while (left) {
+            const uint32_t chunk = (uint32_t)(left < RESIDENT_MAX_SWEEPS ? left : RESIDENT_MAX_SWEEPS);
+            EA_CUDA(sim, launch_sweeps_small(sim, sim->t, chunk, sim->stream));
             sim->t += chunk;
             left -= chunk;
         }
@@ -483,8 +501,13 @@ ea_status ea_set_kernel(ea_sim *sim, int kernel)
         k = EA_KERNEL_RESIDENT;
         sim->resident_min_sweeps = RESIDENT_AUTO_MIN_SWEEPS;
     }
+    else if (kernel == EA_KERNEL_AUTO && kernel_valid_for(EA_KERNEL_SMALL, sim->lat.L) && small_supported(sim)) {
+        k = EA_KERNEL_SMALL;
+        sim->resident_min_sweeps = SMALL_AUTO_MIN_SWEEPS;
+    }
     std::string why;
     if (k == EA_KERNEL_RESIDENT && !resident_supported(sim, &why)) EA_FAIL(sim, EA_ERR_INVALID, "%s", why.c_str());
+    if (k == EA_KERNEL_SMALL && !small_supported(sim, &why)) EA_FAIL(sim, EA_ERR_INVALID, "%s", why.c_str());
     sim->kernel = k;
     return EA_OK;
 }

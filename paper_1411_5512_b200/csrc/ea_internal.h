@@ -51,7 +51,7 @@ struct ea_sim {
     unsigned *resident_flags = nullptr;
     uint32_t resident_epoch = 0;
     int resident_tiles = 0;           // CTAs of the partition whose tile table sits behind the flags (0: none)
-    uint64_t resident_min_sweeps = 1; // shorter ea_sweep calls use the ROWS launches (AUTO: 8)
+    uint64_t resident_min_sweeps = 1; // shorter ea_sweep calls use the ROWS launches (AUTO: 8; SMALL under AUTO: 2)
     bool resident_used = false;       // a resident launch is in flight / unchecked: see check_resident()
     uint64_t resident_timeout_ns = 20000000000ull; // neighbour wait gives up after this (EA_RESIDENT_TIMEOUT_MS)
 
@@ -104,6 +104,11 @@ cudaError_t launch_bump_time_batch(uint64_t *const *d_times, unsigned n_sims, ui
 // ROWS_PERSISTENT (ea_sweep.cu; L = 16, 32, 64): n sweeps in one cooperative launch with a grid barrier per colour
 bool rows_persistent_valid(int L);
 cudaError_t launch_sweeps_rows_persistent(ea_sim *s, uint64_t t0, uint32_t n, cudaStream_t st);
+// SMALL (ea_sweep_small.cu; L % 4 == 0, L <= 32): n sweeps in one launch, lattice resident in the shared memory of one
+// CTA or one thread-block cluster
+int small_cluster_size(int L, int n_replicas); // 0: not valid for this shape
+bool small_supported(const ea_sim *s, std::string *why = nullptr);
+cudaError_t launch_sweeps_small(ea_sim *s, uint64_t t0, uint32_t n, cudaStream_t st);
 // RESIDENT (ea_sweep_resident.cu): n sweeps from sweep index t0 in one cooperative launch
 bool resident_supported(const ea_sim *s, std::string *why = nullptr);
 size_t resident_flag_bytes();   // flag lines + abort line

@@ -323,7 +323,10 @@ static cudaError_t launch_typed(ea_sim *s, const SweepArgs &a, cudaStream_t st)
 {
     const Lattice &lat = s->lat;
     const bool pow2 = lat.log2L >= 0;
-    if (s->kernel == EA_KERNEL_ROWS || s->kernel == EA_KERNEL_RESIDENT || s->kernel == EA_KERNEL_ROWS_PERSISTENT) { // RESIDENT: single half-sweeps go as ROWS
+    // RESIDENT / SMALL: single half-sweeps and short calls go as per-colour launches of the best variant valid for L
+    const bool rows_ok = lat.L == 16 || lat.L == 32 || lat.L == 64 || lat.L == 128;
+    const int kernel = s->kernel == EA_KERNEL_SMALL ? (rows_ok ? (int)EA_KERNEL_ROWS : (int)EA_KERNEL_VEC2) : s->kernel;
+    if (kernel == EA_KERNEL_ROWS || kernel == EA_KERNEL_RESIDENT || kernel == EA_KERNEL_ROWS_PERSISTENT) {
         switch (lat.L) {
         case 16: launch_rows<16, BondT, ALWAYS, HB>(a, st); break;
         case 32: launch_rows<32, BondT, ALWAYS, HB>(a, st); break;
@@ -331,7 +334,7 @@ static cudaError_t launch_typed(ea_sim *s, const SweepArgs &a, cudaStream_t st)
         case 128: launch_rows<128, BondT, ALWAYS, HB>(a, st); break;
         default: return cudaErrorInvalidValue;
         }
-    } else if (s->kernel == EA_KERNEL_VEC2) {
+    } else if (kernel == EA_KERNEL_VEC2) {
         unsigned n = lat.Nh / 2, block = 256, grid = (n + block - 1) / block;
         if (pow2) k_sweep_vec2<BondT, true, ALWAYS, HB><<<grid, block, 0, st>>>(a);
         else k_sweep_vec2<BondT, false, ALWAYS, HB><<<grid, block, 0, st>>>(a);

@@ -14,12 +14,12 @@ from paper_1411_5512_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = ["scalar", "vec2", "rows", "rows_persistent"]
+KERNELS = ["scalar", "vec2", "rows", "rows_persistent", "small"]
 
 
 def kernels_for(L):
     return [k for k in KERNELS if k == "scalar" or (k == "vec2" and L % 4 == 0) or (k == "rows" and L in (16, 32, 64, 128))
-            or (k == "rows_persistent" and L in (16, 32, 64))]
+            or (k == "rows_persistent" and L in (16, 32, 64)) or (k == "small" and L % 4 == 0 and L <= 32 and L != 28)]
 
 
 def make_pair(L, p, T, n_rep, seed, n_slots=2, kernel="auto"):
@@ -672,6 +672,28 @@ def test_rows_persistent_long_run_matches_the_graph_replays():
             a.sweep(k)
             b.sweep(k)
             assert np.array_equal(a.get_spins(), b.get_spins()), "L=%d after %d sweeps" % (L, a.time)
+
+
+def test_small_lattice_kernel_auto_choice_and_long_runs():
+    """SMALL (lattice resident in the shared memory of one CTA, or of one thread-block cluster with the neighbouring planes
+    read through distributed shared memory): AUTO picks it for L = 8, 16, 32; launches of 2, 3 and n sweeps (ea_sweep(1)
+    goes as per-colour launches) against the per-colour kernels over cfg1's, cfg2's and a longer horizon; both bond
+    widths.  (The oracle follows the first sweeps in the every-kernel test and in the cfg1 / cfg2 tests.)"""
+    for L, n_rep, n in ((8, 1, 1000), (16, 2, 3000), (32, 2, 3000), (32, 1, 500), (24, 2, 500)):
+        ref = "rows" if L in (16, 32) else "vec2"
+        a = binding.Sim(L, 0.5, 0.8, n_replicas=n_rep, seed=wl.seed_for(2, L), n_slots=0, kernel=ref)
+        b = binding.Sim(L, 0.5, 0.8, n_replicas=n_rep, seed=wl.seed_for(2, L), n_slots=0)
+        assert b.kernel == binding.EA_KERNEL_SMALL
+        for k in (1, 2, 3, n):
+            a.sweep(k)
+            b.sweep(k)
+            assert np.array_equal(a.get_spins(), b.get_spins()), "L=%d after %d sweeps" % (L, a.time)
+        a.close()
+        b.close()
+    with pytest.raises(binding.EAError):
+        binding.Sim(64, 0.5, 0.8, n_replicas=2, kernel="small")  # 64 x 64 x 4 pairs do not fit a cluster of 16
+    with pytest.raises(binding.EAError):
+        binding.Sim(10, 0.5, 0.8, n_replicas=2, kernel="small")  # needs L % 4 == 0
 
 
 def test_ageing_protocol_driver_matches_the_oracle_step_by_step():
