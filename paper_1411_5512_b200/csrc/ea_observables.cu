@@ -43,17 +43,56 @@ struct LaneCounter {
     __device__ __forceinline__ void add32(uint32_t w, unsigned lane) { lo += __popc(warp_transpose32(w, lane)); }
 };
 
-// block reduce -> 64 (or 32) global counters
+// block reduce -> 64 (or 32) global counters.  After the warp-shuffle transposition a lane holds the counts of ITS two samples
+// (lane, lane + 32), so nothing is left to reduce across lanes; the warps of the CTA are summed through shared memory
+// (one slot per warp and sample, no atomics) and one thread per sample adds the CTA's total to the global counter.
 __device__ __forceinline__ void flush_counts(const LaneCounter &k, unsigned long long *out, bool both_halves)
 {
-    __shared__ unsigned acc[64];
-    if (threadIdx.x < 64) acc[threadIdx.x] = 0;
+    __shared__ unsigned acc[8][64]; // launch bounds: 256 threads
+    const unsigned lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    acc[warp][lane] = k.lo;
+    acc[warp][32 + lane] = k.hi;
     __syncthreads();
-    unsigned lane = threadIdx.x & 31;
-    atomicAdd(&acc[lane], k.lo);
-    if (both_halves) atomicAdd(&acc[32 + lane], k.hi);
-    __syncthreads();
-    if (threadIdx.x < (both_halves ? 64 : 32)) atomicAdd(&out[threadIdx.x], (unsigned long long)acc[threadIdx.x]);
+    if (threadIdx.x < (both_halves ? 64u : 32u)) {
+        unsigned long long t = 0;
+        for (unsigned w = 0; w < nw; ++w) t += acc[w][threadIdx.x];
+        if (t) atomicAdd(&out[threadIdx.x], t);
+    }
+}
+
+// Carry-save front end of the per-sample counters: eight 64-sample words go through seven 3:2 compressors (Harley-Seal)
+// into bit-sliced ones / twos / fours planes kept per thread; only the "eights" word they emit -- and, once at the end,
+// the three planes -- pays for the 32 x 32 bit transposition and the POPC: one transposition per eight words, not eight.
+struct Csa8 {
+    uint64_t ones = 0, twos = 0, fours = 0;
+    static __device__ __forceinline__ void csa(uint64_t &h, uint64_t &l, uint64_t a, uint64_t b, uint64_t c)
+    {
+        h = mk64(lop3<LUT_MAJ>(lo32(a), lo32(b), lo32(c)), lop3<LUT_MAJ>(hi32(a), hi32(b), hi32(c)));
+        l = mk64(lop3<LUT_XOR3>(lo32(a), lo32(b), lo32(c)), lop3<LUT_XOR3>(hi32(a), hi32(b), hi32(c)));
+    }
+    __device__ __forceinline__ uint64_t add8(const uint64_t (&x)[8]) // returns the eights word
+    {
+        uint64_t tA, tB, tC, tD, fA, fB, e;
+        csa(tA, ones, ones, x[0], x[1]);
+        csa(tB, ones, ones, x[2], x[3]);
+        csa(fA, twos, twos, tA, tB);
+        csa(tC, ones, ones, x[4], x[5]);
+        csa(tD, ones, ones, x[6], x[7]);
+        csa(fB, twos, twos, tC, tD);
+        csa(e, fours, fours, fA, fB);
+        return e;
+    }
+};
+
+// weights 8 (eights words), then the planes once: lo / hi = counts of samples lane and lane + 32
+__device__ __forceinline__ void csa_finish(const Csa8 &a, const LaneCounter &k8, unsigned lane, LaneCounter &out)
+{
+    LaneCounter k1, k2, k4;
+    k1.add64(a.ones, lane);
+    k2.add64(a.twos, lane);
+    k4.add64(a.fours, lane);
+    out.lo = 8 * k8.lo + 4 * k4.lo + 2 * k2.lo + k1.lo;
+    out.hi = 8 * k8.hi + 4 * k4.hi + 2 * k2.hi + k1.hi;
 }
 
 // cnt_b over all N words of sigma ^ other (other may be null): autocorrelation / magnetisation.
@@ -62,13 +101,19 @@ __global__ void __launch_bounds__(256) k_count_spins(Lattice lat, const uint64_t
 {
     const unsigned lane = threadIdx.x & 31, N = 2 * lat.Nh;
     const unsigned stride = gridDim.x * blockDim.x;
-    LaneCounter k;
-    for (unsigned base = blockIdx.x * blockDim.x; base < N; base += stride) { // block-uniform trip count
-        unsigned e = base + threadIdx.x;
-        uint64_t w = 0;
-        if (e < N) w = other ? (spins[e] ^ other[e]) : spins[e];
-        k.add64(w, lane);
+    Csa8 acc;
+    LaneCounter k8;
+    for (unsigned base = blockIdx.x * blockDim.x; base < N; base += 8 * stride) { // block-uniform trip count
+        uint64_t w[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const unsigned e = base + j * stride + threadIdx.x;
+            w[j] = e < N ? (other ? (spins[e] ^ other[e]) : spins[e]) : 0;
+        }
+        k8.add64(acc.add8(w), lane);
     }
+    LaneCounter k;
+    csa_finish(acc, k8, lane, k);
     flush_counts(k, out, true);
 }
 
@@ -79,27 +124,32 @@ __global__ void __launch_bounds__(256) k_count_energy(Lattice lat, const uint64_
 {
     const unsigned lane = threadIdx.x & 31, N = 2 * lat.Nh;
     const unsigned stride = gridDim.x * blockDim.x;
-    const unsigned L = lat.L, Lh = lat.Lh;
-    LaneCounter k;
-    for (unsigned base = blockIdx.x * blockDim.x; base < N; base += stride) {
-        unsigned e = base + threadIdx.x;
-        uint64_t u0 = 0, u1 = 0, u2 = 0;
-        if (e < N) {
-            Coord q = coord_of(lat, e);
-            unsigned i = e - q.c * lat.Nh, x = 2 * q.xh + ((q.c ^ (q.y + q.z)) & 1u);
-            unsigned xp = (x + 1 == L) ? 0 : x + 1, yp = (q.y + 1 == L) ? 0 : q.y + 1, zp = (q.z + 1 == L) ? 0 : q.z + 1;
-            uint64_t sg = spins[e];
-            const BondT *J = bonds + (size_t)q.c * 3 * lat.Nh;
-            BondT j0 = J[i], j1 = J[lat.Nh + i], j2 = J[2 * lat.Nh + i];
-            u0 = mk64(bond_lo(j0), bond_hi(j0)) ^ sg ^ spins[flat_of(lat, xp, q.y, q.z)];
-            u1 = mk64(bond_lo(j1), bond_hi(j1)) ^ sg ^ spins[flat_of(lat, x, yp, q.z)];
-            u2 = mk64(bond_lo(j2), bond_hi(j2)) ^ sg ^ spins[flat_of(lat, x, q.y, zp)];
-            (void)Lh;
+    const unsigned L = lat.L;
+    Csa8 acc;
+    LaneCounter k8;
+    for (unsigned base = blockIdx.x * blockDim.x; base < N; base += 8 * stride) { // eight sites = three groups of eight words
+        uint64_t u[3][8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const unsigned e = base + j * stride + threadIdx.x;
+            u[0][j] = u[1][j] = u[2][j] = 0;
+            if (e < N) {
+                Coord q = coord_of(lat, e);
+                unsigned i = e - q.c * lat.Nh, x = 2 * q.xh + ((q.c ^ (q.y + q.z)) & 1u);
+                unsigned xp = (x + 1 == L) ? 0 : x + 1, yp = (q.y + 1 == L) ? 0 : q.y + 1, zp = (q.z + 1 == L) ? 0 : q.z + 1;
+                uint64_t sg = spins[e];
+                const BondT *J = bonds + (size_t)q.c * 3 * lat.Nh;
+                BondT j0 = J[i], j1 = J[lat.Nh + i], j2 = J[2 * lat.Nh + i];
+                u[0][j] = mk64(bond_lo(j0), bond_hi(j0)) ^ sg ^ spins[flat_of(lat, xp, q.y, q.z)];
+                u[1][j] = mk64(bond_lo(j1), bond_hi(j1)) ^ sg ^ spins[flat_of(lat, x, yp, q.z)];
+                u[2][j] = mk64(bond_lo(j2), bond_hi(j2)) ^ sg ^ spins[flat_of(lat, x, q.y, zp)];
+            }
         }
-        k.add64(u0, lane);
-        k.add64(u1, lane);
-        k.add64(u2, lane);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) k8.add64(acc.add8(u[d]), lane);
     }
+    LaneCounter k;
+    csa_finish(acc, k8, lane, k);
     flush_counts(k, out, true);
 }
 
@@ -153,11 +203,22 @@ __global__ void __launch_bounds__(256) k_q_transpose(const uint64_t *__restrict_
     const unsigned lane = threadIdx.x & 31;
     const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
     unsigned cnt = 0;
-    for (unsigned w = warp; w < NW; w += nwarps) { // warp-uniform trip count
-        const uint64_t sg = spins[(size_t)w * 32 + lane];
-        const uint32_t t = warp_transpose32(lo32(sg) ^ hi32(sg), lane);
-        Tq[(size_t)w * 32 + lane] = t;
-        cnt += __popc(t);
+    for (unsigned w0 = warp; w0 < NW; w0 += 4 * nwarps) { // warp-uniform trip count; four loads in flight
+        uint64_t sg[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const unsigned w = w0 + j * nwarps;
+            sg[j] = w < NW ? spins[(size_t)w * 32 + lane] : 0;
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const unsigned w = w0 + j * nwarps;
+            if (w < NW) {
+                const uint32_t t = warp_transpose32(lo32(sg[j]) ^ hi32(sg[j]), lane);
+                Tq[(size_t)w * 32 + lane] = t;
+                cnt += __popc(t);
+            }
+        }
     }
     __shared__ unsigned acc[32];
     if (threadIdx.x < 32) acc[threadIdx.x] = 0;
@@ -181,28 +242,69 @@ __device__ __forceinline__ void flush_r_counts(const unsigned (&cnt)[NR], unsign
         if ((int)(k >> 5) <= r_max && (&acc[0][0])[k]) atomicAdd(&out[k], (unsigned long long)(&acc[0][0])[k]);
 }
 
-// AXIS = 1 (y) or 2 (z)
+// AXIS = 1 (y) or 2 (z).  One CTA of four warps stages one COLUMN of the transposed field -- the L rows along the axis
+// at fixed (z or y, xb), both colours, 32 KB, by cp.async -- in shared memory and handles 16 of the L/2 distances: a warp
+// takes eight distances and the own rows of one colour.
+// For a block of eight rows the own words stay in registers while each distance streams its eight partner rows in
+// (rows L .. L+7 repeat rows 0 .. 7, so a block never wraps); the eight XOR words of a (block, distance) go through a
+// carry-save adder tree (Harley-Seal: seven 3:2 compressors = 14 LOP3) into bit-sliced ones / twos / fours planes per
+// distance, and only the "eights" word is popcounted: one POPC per eight site words instead of eight, which moves the
+// kernel from the POPC rate (one warp instruction per 8 clocks) to the LOP3 rate.
 template <int L, int AXIS>
-__global__ void __launch_bounds__(256) k_c4_yz(const uint32_t *__restrict__ Tq, int r_max, unsigned long long *out)
+__global__ void __launch_bounds__(128) k_c4_yz(const uint32_t *__restrict__ Tq, int r_max, unsigned long long *out)
 {
-    constexpr unsigned XB = L / 64, RW = XB * 32, PL = L * RW, CW = L * PL, NT = 2 * L * L * XB;
-    constexpr int NR = L / 2 + 1;
-    const unsigned lane = threadIdx.x & 31;
-    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
-    unsigned cnt[NR];
-#pragma unroll
-    for (int r = 0; r < NR; ++r) cnt[r] = 0;
-    for (unsigned t = warp; t < NT; t += nwarps) {
-        const unsigned xb = t % XB, y = (t / XB) % L, z = (t / (XB * L)) % L, c = t / (XB * L * L);
-        const uint32_t own = __ldg(Tq + c * CW + z * PL + y * RW + xb * 32 + lane);
-#pragma unroll
-        for (int r = 1; r < NR; ++r) {
-            const unsigned cp = c ^ (r & 1);
-            const unsigned yy = AXIS == 1 ? ((y + r) & (L - 1)) : y, zz = AXIS == 2 ? ((z + r) & (L - 1)) : z;
-            cnt[r] += __popc(own ^ __ldg(Tq + cp * CW + zz * PL + yy * RW + xb * 32 + lane));
-        }
+    constexpr unsigned XB = L / 64, RW = XB * 32, PL = L * RW, CW = L * PL;
+    constexpr int NR = L / 2, RPW = 8, RPC = 16, NCHUNK = NR / RPC, BLK = 8;
+    static_assert(NR % RPC == 0 && L % BLK == 0, "distances and rows come in whole blocks");
+    __shared__ __align__(16) uint32_t col[2][L + BLK][32];
+    const unsigned tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const unsigned chunk = blockIdx.x % NCHUNK, colid = blockIdx.x / NCHUNK;
+    const unsigned xb = colid % XB, u = colid / XB; // u = z (AXIS 1) or y (AXIS 2)
+    // a row of the column is 128 contiguous bytes of Tq: eight threads x 16 bytes
+    for (unsigned i = tid; i < 2u * (L + BLK) * 8; i += 128) {
+        const unsigned q = i & 7, rowx = (i >> 3) % (L + BLK), c = (i >> 3) / (L + BLK), row = rowx & (L - 1);
+        const unsigned idx = (AXIS == 1 ? c * CW + u * PL + row * RW : c * CW + row * PL + u * RW) + xb * 32 + 4 * q;
+        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&col[c][rowx][4 * q]);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(Tq + idx) : "memory");
     }
-    flush_r_counts<NR>(cnt, lane, r_max, out);
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    __syncthreads();
+    const unsigned c = warp & 1; // colour of the own rows
+    const unsigned r0 = 1 + chunk * RPC + (warp >> 1) * RPW; // odd: distance r0 + ri flips the colour iff ri is even
+    uint32_t ones[RPW], twos[RPW], fours[RPW], cnt[RPW];
+#pragma unroll
+    for (int ri = 0; ri < RPW; ++ri) ones[ri] = twos[ri] = fours[ri] = cnt[ri] = 0;
+#pragma unroll 1
+    for (unsigned y0 = 0; y0 < (unsigned)L; y0 += BLK) {
+            uint32_t own[BLK];
+#pragma unroll
+            for (int j = 0; j < BLK; ++j) own[j] = col[c][y0 + j][lane];
+#pragma unroll
+            for (int ri = 0; ri < RPW; ++ri) {
+                const uint32_t *pr = &col[c ^ ((1 + ri) & 1)][(y0 + r0 + ri) & (L - 1)][lane];
+                uint32_t x[BLK];
+#pragma unroll
+                for (int j = 0; j < BLK; ++j) x[j] = own[j] ^ pr[j * 32];
+                // carry-save: (ones, x0, x1) -> ones, twosA; ... ; (fours, foursA, foursB) -> fours, eights
+                const uint32_t tA = lop3<LUT_MAJ>(ones[ri], x[0], x[1]), o1 = lop3<LUT_XOR3>(ones[ri], x[0], x[1]);
+                const uint32_t tB = lop3<LUT_MAJ>(o1, x[2], x[3]), o2 = lop3<LUT_XOR3>(o1, x[2], x[3]);
+                const uint32_t fA = lop3<LUT_MAJ>(twos[ri], tA, tB), t1 = lop3<LUT_XOR3>(twos[ri], tA, tB);
+                const uint32_t tC = lop3<LUT_MAJ>(o2, x[4], x[5]), o3 = lop3<LUT_XOR3>(o2, x[4], x[5]);
+                const uint32_t tD = lop3<LUT_MAJ>(o3, x[6], x[7]), o4 = lop3<LUT_XOR3>(o3, x[6], x[7]);
+                const uint32_t fB = lop3<LUT_MAJ>(t1, tC, tD), t2 = lop3<LUT_XOR3>(t1, tC, tD);
+                const uint32_t e = lop3<LUT_MAJ>(fours[ri], fA, fB);
+                fours[ri] = lop3<LUT_XOR3>(fours[ri], fA, fB);
+                ones[ri] = o4;
+                twos[ri] = t2;
+                cnt[ri] += __popc(e);
+            }
+        }
+#pragma unroll
+    for (int ri = 0; ri < RPW; ++ri) {
+        const unsigned r = r0 + ri;
+        const unsigned total = 8 * cnt[ri] + 4 * __popc(fours[ri]) + 2 * __popc(twos[ri]) + __popc(ones[ri]);
+        if ((int)r <= r_max && total) atomicAdd(&out[r * 32 + lane], (unsigned long long)total);
+    }
 }
 
 template <int L> struct RowBits;
@@ -255,9 +357,10 @@ static cudaError_t launch_c4_fast(ea_sim *s, int r_max)
     s->count_launch();
     k_c4_x<L><<<grid, 256, 0, s->stream>>>(Tq, r_max, s->counters);
     s->count_launch();
-    k_c4_yz<L, 1><<<grid, 256, 0, s->stream>>>(Tq, r_max, s->counters + n_r * 32);
+    constexpr unsigned grid_yz = (unsigned)L * (L / 64) * ((L / 2) / 16); // columns x chunks of 16 distances
+    k_c4_yz<L, 1><<<grid_yz, 128, 0, s->stream>>>(Tq, r_max, s->counters + n_r * 32);
     s->count_launch();
-    k_c4_yz<L, 2><<<grid, 256, 0, s->stream>>>(Tq, r_max, s->counters + 2 * n_r * 32);
+    k_c4_yz<L, 2><<<grid_yz, 128, 0, s->stream>>>(Tq, r_max, s->counters + 2 * n_r * 32);
     return cudaGetLastError();
 }
 
