@@ -12,6 +12,10 @@ LIB = os.path.join(HERE, "libea_oracle.so")
 
 
 def build(force: bool = False) -> str:
+    # tests/test_oracle_mutants.py points the loader at a deliberately broken build to show that the pins catch it
+    override = os.environ.get("EA_ORACLE_LIB")
+    if override:
+        return override
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
