@@ -55,9 +55,9 @@ typedef enum {
     EA_KERNEL_SCALAR = 1, /* one site per thread, 64-bit loads; any even L >= 2           */
     EA_KERNEL_VEC2 = 2,   /* two sites per thread, 128-bit loads; L % 4 == 0              */
     EA_KERNEL_ROWS = 3,   /* warp marches along y with a register window; L % 4 == 0      */
-    EA_KERNEL_RESIDENT = 4, /* persistent cooperative kernel, many sweeps per launch (L = 128); needs a device with
-                               cooperative launch, >= 128 SMs and 187 KB of shared memory per CTA (ea_last_error /
-                               stderr say which is missing).  Its CTAs wait for their neighbours' step flags; a wait
+    EA_KERNEL_RESIDENT = 4, /* persistent cooperative kernel, many sweeps per launch (L = 128): 148 tiles on a 148-SM part,
+                               128 otherwise; needs a device with cooperative launch, >= 128 SMs and 170 (185) KB of
+                               shared memory per CTA (ea_last_error / stderr say which is missing).  Its CTAs wait for their neighbours' step flags; a wait
                                that sees nothing for EA_RESIDENT_TIMEOUT_MS (environment, read at ea_create;
                                default 20000) gives up, and the next synchronising call returns EA_ERR_CUDA */
     EA_KERNEL_FOLD = 5,    /* what a sim with n_samples < 64 runs (not selectable)        */
@@ -187,8 +187,9 @@ ea_status ea_batch_create(ea_sim *const *sims, int n_sims, ea_batch **out);
 ea_status ea_batch_sweep(ea_batch *batch, uint64_t n);
 ea_status ea_batch_destroy(ea_batch *batch);
 
-/* Host-only self-test (no device needed): the row schedules of the RESIDENT kernel -- every row of a tile exactly
- * once, boundary rows first, consecutive rows of a warp alternating in parity.  EA_OK or EA_ERR_STATE. */
+/* Host-only self-test (no device needed): the tables of the RESIDENT kernel for both tile partitions (148 and 128 tiles) and
+ * every number of compute warps -- the tiles cover the lattice exactly once, every row of a tile is scheduled exactly once in
+ * its class with the boundary rows first, every halo row has an owner.  EA_OK or EA_ERR_STATE. */
 ea_status ea_selftest_host(void);
 
 /* Measured issue rates of the pipes that bound this library's kernels (the update is "boolean logic at
