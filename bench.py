@@ -488,6 +488,20 @@ def run_ours(args, cfg):
         next_rows["scan"] = {"L": Ls, "sims": Ks, "sweeps": n_sc, "ps_per_attempt_aggregate": 1e12 * t_sc / (Ks * n_sc * Ls ** 3 * 64.0),
                              "note": "NEXT-4 driver: K independent L=64 sims, one stream + CUDA graph each, issued back to back"}
 
+    if next_rows is not None and ws == 1:
+        # single small lattices (BASELINE configs[0..1] and the paper's scans at L = 32): SMALL keeps spins and
+        # bonds in the shared memory of one CTA / one thread-block cluster for the whole ea_sweep call
+        small = []
+        for name, Ls, n_rep, n_sm in (("cfg1", 8, 1, 20000), ("L16", 16, 2, 20000), ("cfg2", 32, 2, 20000)):
+            ss = binding.Sim(Ls, 0.5, cfg.T, n_replicas=n_rep, seed=seed + 2000 + Ls, n_slots=0, device=local_rank, stream=stream)
+            ss.sweep(100)
+            ss.synchronize()
+            t_s = sweep_window(ss, n_sm, stream)
+            small.append({"config": name, "L": Ls, "n_replicas": n_rep, "kernel": binding_kernel_name(ss.kernel),
+                          "us_per_half_sweep": 1e6 * t_s / (2.0 * n_sm), "ps_per_attempt": 1e12 * t_s / (n_sm * float(Ls) ** 3 * LANES)})
+            ss.close()
+        next_rows["small_lattices"] = {"what": "one sim alone, CUDA events around ea_sweep(20000) after 100 warm-up sweeps", "points": small}
+
     cpu_baseline = None
     if ws == 1 and not args.no_cpu_baseline:
         base, _ = time_oracle(cfg, S, steps=args.cpu_sweeps, warmup=1)
@@ -516,7 +530,7 @@ def run_ours(args, cfg):
 
 
 def binding_kernel_name(k):
-    return {1: "scalar", 2: "vec2", 3: "rows", 4: "resident"}.get(int(k), str(k))
+    return {1: "scalar", 2: "vec2", 3: "rows", 4: "resident", 5: "fold", 6: "rows_persistent", 7: "small"}.get(int(k), str(k))
 
 
 def main():

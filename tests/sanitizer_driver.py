@@ -2,7 +2,8 @@
 
     compute-sanitizer --tool memcheck|racecheck|synccheck python tests/sanitizer_driver.py
 
-(`profiles/r02_sanitizer.md` records the results.)  Not collected by pytest; it checks nothing itself except that
+(`profiles/r02_sanitizer.md` records the results.)  `python tests/sanitizer_driver.py profile` is the short run that
+`profiles/r02_ncu_small_and_observables.md` was taken from.  Not collected by pytest; it checks nothing itself except that
 the runs finish and agree with each other where two kernels compute the same thing.
 """
 import os
@@ -16,7 +17,23 @@ import numpy as np  # noqa: E402
 from paper_1411_5512_b200 import binding  # noqa: E402
 
 
+def profile_run():
+    """The short run behind profiles/r02_ncu_small_and_observables.md: SMALL at L = 8, 16, 32 (1000 sweeps each), then one
+    measure point at L = 128."""
+    for L, nrep in ((8, 1), (16, 2), (32, 2)):
+        g = binding.Sim(L, 0.5, 0.8, n_replicas=nrep, seed=3, n_slots=1)
+        g.sweep(1000)
+        g.synchronize()
+        g.close()
+    g = binding.Sim(128, 0.77, 0.8, n_replicas=2, seed=3, n_slots=1)
+    g.sweep(8); g.snapshot(0); g.sweep(8)
+    g.autocorr(0); g.c4(64, with_q=True); g.energy(); g.magnetisation()
+    g.close()
+
+
 def main():
+    if sys.argv[1:] == ["profile"]:
+        return profile_run()
     which = sys.argv[1:] or ["resident", "rows", "fold", "observables", "c4vec", "batch"]
     if "resident" in which:  # persistent kernel: inter-CTA release/acquire flags, named barriers, mbarriers, cp.async
         a = binding.Sim(128, 0.77, 0.8, n_replicas=2, seed=7, n_slots=0, kernel="rows")
