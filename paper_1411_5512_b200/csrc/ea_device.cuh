@@ -302,6 +302,22 @@ __device__ __forceinline__ uint64_t metropolis_word(uint64_t s, uint64_t n1, uin
         }
         return mk64(nl, nh);
     }
+    if (!ALWAYS) { // every temperature: the same new-spin formulation with the three levels predicated (no branch)
+        const HalfCount hl = count_half_lop3(bond_lo(j1) ^ lo32(n1), bond_lo(j2) ^ lo32(n2), bond_lo(j3) ^ lo32(n3),
+                                             bond_lo(j4) ^ lo32(n4), bond_lo(j5) ^ lo32(n5), bond_lo(j6) ^ lo32(n6));
+        const HalfCount hh = count_half_lop3(bond_hi(j1) ^ hi32(n1), bond_hi(j2) ^ hi32(n2), bond_hi(j3) ^ hi32(n3),
+                                             bond_hi(j4) ^ hi32(n4), bond_hi(j5) ^ hi32(n5), bond_hi(j6) ^ hi32(n6));
+        const uint32_t tl = lop3<LUT_MAJ_NA>(sl, hl.sa, hl.sb), th_ = lop3<LUT_MAJ_NA>(sh, hh.sa, hh.sb);
+        uint32_t nl = lop3<LUT_MAJ>(hl.ka, hl.kb, tl), nh = lop3<LUT_MAJ>(hh.ka, hh.kb, th_);
+        const uint32_t xl = lop3<LUT_MAJ_NA>(sl, hl.ka, hl.kb), xh = lop3<LUT_MAJ_NA>(sh, hh.ka, hh.kb);
+        if (r_lo < th.thr[2]) nl = lop3<LUT_MAJ_NA>(sl, xl, lop3<LUT_MAJ>(sl, hl.sa, hl.sb));
+        if (r_lo < th.thr[1]) nl = lop3<LUT_MAJ_NA>(sl, xl, tl);
+        if (r_lo < th.thr[0]) nl = ~sl;
+        if (r_hi < th.thr[2]) nh = lop3<LUT_MAJ_NA>(sh, xh, lop3<LUT_MAJ>(sh, hh.sa, hh.sb));
+        if (r_hi < th.thr[1]) nh = lop3<LUT_MAJ_NA>(sh, xh, th_);
+        if (r_hi < th.thr[0]) nh = ~sh;
+        return mk64(nl, nh);
+    }
     const uint32_t fl = flip_half<ALWAYS>(bond_lo(j1) ^ sl ^ lo32(n1), bond_lo(j2) ^ sl ^ lo32(n2),
                                           bond_lo(j3) ^ sl ^ lo32(n3), bond_lo(j4) ^ sl ^ lo32(n4),
                                           bond_lo(j5) ^ sl ^ lo32(n5), bond_lo(j6) ^ sl ^ lo32(n6), r_lo, th);

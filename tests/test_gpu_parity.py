@@ -252,6 +252,22 @@ def test_resident_kernel_L128_against_the_oracle(n_rep, T, p):
     assert_same_observables(g, o, slot=0)
 
 
+def test_resident_kernel_on_the_128_tile_partition(monkeypatch):
+    """The persistent kernel is table-driven: on a part with fewer than 148 SMs it runs 128 tiles of 16 x 8 rows instead of
+    144 of 14 x 8 plus 4 of 2 x 32.  EA_RESIDENT_TILES=128 (read when the sim is created) forces that partition here: 8 + 40
+    sweeps against the oracle / the per-colour launches, both bond widths."""
+    monkeypatch.setenv("EA_RESIDENT_TILES", "128")
+    for n_rep in (2, 1):
+        c = wl.CONFIGS["cfg4"]
+        g, o = make_pair(c.L, c.p, c.T, n_rep, c.seed + n_rep, n_slots=0, kernel="resident")
+        a = binding.Sim(c.L, c.p, c.T, n_replicas=n_rep, seed=c.seed + n_rep, n_slots=0, kernel="rows")
+        g.sweep(8); o.sweep(8); a.sweep(8)
+        assert_same_state(g, o, "128 tiles, n_rep=%d" % n_rep)
+        g.sweep(40); a.sweep(40)
+        assert np.array_equal(g.get_spins(), a.get_spins())
+        g.close(); a.close()
+
+
 def test_resident_kernel_long_run_is_identical_to_the_per_colour_launches():
     """Kernel variants are bit-identical by contract: 3000 sweeps of the bench configuration through RESIDENT
     (launches of 1, 7, 500 and 2492 sweeps) against the ROWS launches (oracle-checked above and too slow to
