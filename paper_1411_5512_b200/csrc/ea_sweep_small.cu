@@ -300,8 +300,31 @@ bool small_supported(const ea_sim *s, std::string *why)
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) return no("small-lattice kernel: cudaGetDeviceProperties failed");
     if (prop.major < 9 && C > 1) return no("small-lattice kernel: the device has no thread-block clusters");
-    if (prop.sharedMemPerBlockOptin < small_smem_bytes(s->lat.L, s->lat.L / C, s->bond_bytes()))
-        return no("small-lattice kernel: the device has too little shared memory per CTA");
+    const size_t smem = small_smem_bytes(s->lat.L, s->lat.L / C, s->bond_bytes());
+    if (prop.sharedMemPerBlockOptin < smem) return no("small-lattice kernel: the device has too little shared memory per CTA");
+    if (C > 1) { // can the device co-schedule one cluster of this shape at all (MIG slices, small parts)?
+        auto kern = k_sweep_small<uint32_t, false, true, false, true>;
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+            (C > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess))
+            return no("small-lattice kernel: the device rejects the cluster configuration");
+        const unsigned pairs = (unsigned)((size_t)s->lat.L * s->lat.L * (s->lat.L / C) / 4);
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = dim3((unsigned)C);
+        cfg.blockDim = dim3((pairs + 31) / 32 * 32);
+        cfg.dynamicSmemBytes = smem;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = (unsigned)C;
+        attr[0].val.clusterDim.y = attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        int n_clusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&n_clusters, kern, &cfg) != cudaSuccess || n_clusters < 1) {
+            cudaGetLastError(); // clear
+            return no("small-lattice kernel: the device cannot co-schedule a thread-block cluster of this size");
+        }
+    }
     return true;
 }
 
