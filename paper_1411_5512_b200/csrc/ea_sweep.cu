@@ -30,6 +30,29 @@ __device__ __forceinline__ uint64_t sweep_time(const SweepArgs &a)
     return (a.d_time ? *a.d_time : a.t) + a.t_offset;
 }
 
+// Programmatic dependent launch: consecutive half-sweep launches depend on each other completely (the colour barrier,
+// PAPER.md:86), but the NEXT launch's grid can be brought onto the SMs while this one still runs: every sweep kernel lets
+// its dependents launch at once and waits for its own predecessor before it reads anything the predecessor wrote.  The
+// launches carry cudaLaunchAttributeProgrammaticStreamSerialization (a programmatic edge when captured into a graph).
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+
 template <bool POW2>
 __device__ __forceinline__ void decode_row(const Lattice &lat, unsigned tid, unsigned log2W, unsigned W, unsigned &k,
                                            unsigned &y, unsigned &z)
@@ -55,6 +78,7 @@ __device__ __forceinline__ void decode_row(const Lattice &lat, unsigned tid, uns
 template <typename BondT, bool POW2, bool ALWAYS, bool HB>
 __global__ void __launch_bounds__(256) k_sweep_scalar(const SweepArgs a)
 {
+    pdl_launch_dependents();
     const Lattice lat = a.lat;
     const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= lat.Nh) return;
@@ -75,12 +99,13 @@ __global__ void __launch_bounds__(256) k_sweep_scalar(const SweepArgs a)
     const BondT *__restrict__ Jc = (const BondT *)a.Jc;
     const BondT *__restrict__ Jo = (const BondT *)a.Jo;
     const unsigned Nh = lat.Nh;
+    const BondT j_xp = __ldg(Jc + i), j_yp = __ldg(Jc + Nh + i), j_zp = __ldg(Jc + 2 * Nh + i); // bonds never change:
+    const BondT j_xm = __ldg(Jo + jm), j_ym = __ldg(Jo + Nh + iym), j_zm = __ldg(Jo + 2 * Nh + izm); // before the wait
+    pdl_wait(); // the previous half-sweep is complete; spins through L2 (the read-only path may predate it)
     const uint64_t sg = a.own[i];
-    const uint64_t n_xp = __ldg(a.oth + jp), n_xm = __ldg(a.oth + jm);
-    const uint64_t n_yp = __ldg(a.oth + iyp), n_ym = __ldg(a.oth + iym);
-    const uint64_t n_zp = __ldg(a.oth + izp), n_zm = __ldg(a.oth + izm);
-    const BondT j_xp = __ldg(Jc + i), j_yp = __ldg(Jc + Nh + i), j_zp = __ldg(Jc + 2 * Nh + i);
-    const BondT j_xm = __ldg(Jo + jm), j_ym = __ldg(Jo + Nh + iym), j_zm = __ldg(Jo + 2 * Nh + izm);
+    const uint64_t n_xp = __ldcg(a.oth + jp), n_xm = __ldcg(a.oth + jm);
+    const uint64_t n_yp = __ldcg(a.oth + iyp), n_ym = __ldcg(a.oth + iym);
+    const uint64_t n_zp = __ldcg(a.oth + izp), n_zm = __ldcg(a.oth + izm);
 
     const SweepRng g = make_sweep_rng(a.seed, sweep_time(a), (uint32_t)a.colour);
     const uint32_t site = (2 * xh + s) + L * (y + L * z); // canonical site index
@@ -98,6 +123,7 @@ __global__ void __launch_bounds__(256) k_sweep_scalar(const SweepArgs a)
 template <typename BondT, bool POW2, bool ALWAYS, bool HB>
 __global__ void __launch_bounds__(256) k_sweep_vec2(const SweepArgs a)
 {
+    pdl_launch_dependents();
     const Lattice lat = a.lat;
     const unsigned tid = blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= lat.Nh / 2) return;
@@ -118,18 +144,7 @@ __global__ void __launch_bounds__(256) k_sweep_vec2(const SweepArgs a)
     const BondT *__restrict__ Jc = (const BondT *)a.Jc;
     const BondT *__restrict__ Jo = (const BondT *)a.Jo;
 
-    uint64_t sg0, sg1, A0, A1, yp0, yp1, ym0, ym1, zp0, zp1, zm0, zm1;
-    {
-        ulonglong2 v = *(const ulonglong2 *)(a.own + i0);
-        sg0 = v.x; sg1 = v.y;
-    }
-    ld_pair<uint64_t>(a.oth + i0, A0, A1);
-    const uint64_t ex = __ldg(a.oth + ie);
-    ld_pair<uint64_t>(a.oth + iyp, yp0, yp1);
-    ld_pair<uint64_t>(a.oth + iym, ym0, ym1);
-    ld_pair<uint64_t>(a.oth + izp, zp0, zp1);
-    ld_pair<uint64_t>(a.oth + izm, zm0, zm1);
-    BondT jx0, jx1, jy0, jy1, jz0, jz1, B0, B1, by0, by1, bz0, bz1;
+    BondT jx0, jx1, jy0, jy1, jz0, jz1, B0, B1, by0, by1, bz0, bz1; // bonds never change: loaded before the wait
     ld_pair<BondT>(Jc + i0, jx0, jx1);
     ld_pair<BondT>(Jc + Nh + i0, jy0, jy1);
     ld_pair<BondT>(Jc + 2 * Nh + i0, jz0, jz1);
@@ -137,6 +152,14 @@ __global__ void __launch_bounds__(256) k_sweep_vec2(const SweepArgs a)
     const BondT Jex = __ldg(Jo + ie);
     ld_pair<BondT>(Jo + Nh + iym, by0, by1);
     ld_pair<BondT>(Jo + 2 * Nh + izm, bz0, bz1);
+
+    pdl_wait(); // the previous half-sweep is complete; spins through L2 (the read-only path may predate it)
+    const ulonglong2 vs = *(const ulonglong2 *)(a.own + i0), vA = __ldcg((const ulonglong2 *)(a.oth + i0));
+    const ulonglong2 vyp = __ldcg((const ulonglong2 *)(a.oth + iyp)), vym = __ldcg((const ulonglong2 *)(a.oth + iym));
+    const ulonglong2 vzp = __ldcg((const ulonglong2 *)(a.oth + izp)), vzm = __ldcg((const ulonglong2 *)(a.oth + izm));
+    const uint64_t ex = __ldcg(a.oth + ie);
+    const uint64_t sg0 = vs.x, sg1 = vs.y, A0 = vA.x, A1 = vA.y, yp0 = vyp.x, yp1 = vyp.y, ym0 = vym.x, ym1 = vym.y;
+    const uint64_t zp0 = vzp.x, zp1 = vzp.y, zm0 = vzm.x, zm1 = vzm.y;
 
     // (+x neighbour, -x neighbour, backward x bond) of the two words, by row phase s
     const uint64_t np0 = s ? A1 : A0, nm0 = s ? A0 : ex;
@@ -208,6 +231,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs &a, const SweepRng &g
 template <int L, int M, typename BondT, bool ALWAYS, bool HB>
 __global__ void __launch_bounds__(128) k_sweep_rows(const SweepArgs a)
 {
+    pdl_launch_dependents();
     constexpr unsigned RL = L / 4, G = 32 / RL; // lanes per row, rows per warp
     constexpr unsigned YC = L / M;              // y-chunks
     const unsigned lane = threadIdx.x & 31, warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -216,11 +240,12 @@ __global__ void __launch_bounds__(128) k_sweep_rows(const SweepArgs a)
     if (zg >= L / G) return;
     const unsigned zpar = zg & 1, z = 2 * (G * (zg >> 1) + grp) + zpar, y0 = yc * M;
     const int lane_m = (int)((lane & ~(RL - 1)) | ((k - 1) & (RL - 1))), lane_p = (int)((lane & ~(RL - 1)) | ((k + 1) & (RL - 1)));
+    pdl_wait(); // the previous half-sweep is complete; spins of the other colour through L2 (the read-only path may predate it)
     const SweepRng g = make_sweep_rng(a.seed, sweep_time(a), (uint32_t)a.colour);
-    if ((a.colour ^ zpar) == 0) // phase of row y0 (even): warp-uniform
-        march_rows<L, M, 0, BondT, ALWAYS, HB>(a, g, y0, z, k, lane_m, lane_p);
+    if (((a.colour ^ zpar ^ y0) & 1u) == 0) // phase of row y0: warp-uniform
+        march_rows<L, M, 0, BondT, ALWAYS, HB, true>(a, g, y0, z, k, lane_m, lane_p);
     else
-        march_rows<L, M, 1, BondT, ALWAYS, HB>(a, g, y0, z, k, lane_m, lane_p);
+        march_rows<L, M, 1, BondT, ALWAYS, HB, true>(a, g, y0, z, k, lane_m, lane_p);
 }
 
 // ROWS_PERSISTENT (L = 16, 32, 64; SURVEY 8(f) NEXT-2 "grid-barrier persistent kernels for L <= 64"): all 2n
@@ -309,12 +334,16 @@ cudaError_t launch_sweeps_rows_persistent(ea_sim *s, uint64_t t0, uint32_t n, cu
     return e;
 }
 
+// rows a warp marches along y: 4 at L = 128 (the register window pays), 2 below (measured with one row per warp: L = 64 2.82
+// against 2.47 us per half-sweep, L = 16 1.57 against 2.00 -- but L <= 32 runs the SMALL kernel anyway)
+template <int L> struct ROWS_M { static constexpr int value = L >= 128 ? 4 : 2; };
+
 template <int L, typename BondT, bool ALWAYS, bool HB>
 static void launch_rows(const SweepArgs &a, cudaStream_t st)
 {
-    constexpr int M = (L >= 128) ? 4 : 2, G = 32 / (L / 4);
+    constexpr int M = ROWS_M<L>::value, G = 32 / (L / 4);
     constexpr unsigned warps = (L / M) * (L / G), block = 128, grid = (warps * 32 + block - 1) / block;
-    k_sweep_rows<L, M, BondT, ALWAYS, HB><<<grid, block, 0, st>>>(a);
+    launch_pdl(k_sweep_rows<L, M, BondT, ALWAYS, HB>, dim3(grid), dim3(block), st, a);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -336,12 +365,12 @@ static cudaError_t launch_typed(ea_sim *s, const SweepArgs &a, cudaStream_t st)
         }
     } else if (kernel == EA_KERNEL_VEC2) {
         unsigned n = lat.Nh / 2, block = 256, grid = (n + block - 1) / block;
-        if (pow2) k_sweep_vec2<BondT, true, ALWAYS, HB><<<grid, block, 0, st>>>(a);
-        else k_sweep_vec2<BondT, false, ALWAYS, HB><<<grid, block, 0, st>>>(a);
+        if (pow2) launch_pdl(k_sweep_vec2<BondT, true, ALWAYS, HB>, dim3(grid), dim3(block), st, a);
+        else launch_pdl(k_sweep_vec2<BondT, false, ALWAYS, HB>, dim3(grid), dim3(block), st, a);
     } else {
         unsigned n = lat.Nh, block = 256, grid = (n + block - 1) / block;
-        if (pow2) k_sweep_scalar<BondT, true, ALWAYS, HB><<<grid, block, 0, st>>>(a);
-        else k_sweep_scalar<BondT, false, ALWAYS, HB><<<grid, block, 0, st>>>(a);
+        if (pow2) launch_pdl(k_sweep_scalar<BondT, true, ALWAYS, HB>, dim3(grid), dim3(block), st, a);
+        else launch_pdl(k_sweep_scalar<BondT, false, ALWAYS, HB>, dim3(grid), dim3(block), st, a);
     }
     s->count_launch();
     return cudaGetLastError();
