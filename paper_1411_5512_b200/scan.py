@@ -27,16 +27,21 @@ class Scan:
             self.sims.append(binding.Sim(pt["L"], pt["p"], pt["T"], n_replicas=pt.get("n_replicas", 2),
                                          seed=pt.get("seed", 0), n_slots=pt.get("n_slots", 1),
                                          kernel=pt.get("kernel", "auto"), device=device))
-        # L <= 32: one kernel launch per colour for all points of equal shape (ea_batch_*: 0.108 ps/attempt aggregate at
-        # L = 32 with 64 points, against 0.38 for concurrent streams, which hit the launch rate); L = 64: streams are
-        # better (0.078 against 0.106).  fused=True / False overrides.
+        # Which points share launches (measured on B200, 2000-sweep calls, us per sweep of ALL points):
+        #   L <= 16: every point alone on its stream -- AUTO runs SMALL (lattice in the shared memory of one CTA / cluster, one
+        #            launch per call): L = 16: 1.47 (16 points) / 2.00 (64) against 5.19 / 5.92 for the fused launches;
+        #   L = 32:  SMALL takes a 16-CTA cluster per point, so few run at once: 4.11 / 6.17 / 20.6 with 8 / 16 / 64 points
+        #            against 5.94 / 6.94 / 14.7 fused (ea_batch_*: one launch per colour for all points) -> fuse from 32 points;
+        #   L = 64:  streams of graph replays (10.2 for 8 points against 14 fused).
+        # fused=True / False overrides.
         self.batches, self._solo = [], list(self.sims)
         groups = {}
         for s in self.sims:
-            if s.n_samples == binding.LANES and s.L in (16, 32, 64) and (fused is True or (fused == "auto" and s.L <= 32)):
+            if s.n_samples == binding.LANES and s.L in (16, 32, 64):
                 groups.setdefault((s.L, s.n_replicas), []).append(s)
-        for members in groups.values():
-            if len(members) > 1:
+        for (L, _), members in groups.items():
+            fuse = fused is True or (fused == "auto" and L == 32 and len(members) >= 32)
+            if fuse and len(members) > 1:
                 self.batches.append(binding.Batch(members))
                 self._solo = [s for s in self._solo if s not in members]
 

@@ -544,16 +544,19 @@ def test_c4_vectors_argument_errors():
         g3.c4_shells(2)
 
 
-def test_scan_of_concurrent_sims_matches_the_oracle_point_by_point():
-    """NEXT-4 driver: a p-scan at L = 16 and 32 (each sim on its own stream, graphs replayed back to back) --
-    every point must be the trajectory the oracle computes for that point alone."""
+@pytest.mark.parametrize("fused", ["auto", True])
+def test_scan_of_concurrent_sims_matches_the_oracle_point_by_point(fused):
+    """NEXT-4 driver: a p-scan at L = 16 and 32 -- "auto": every point alone on its own stream (SMALL kernels of different
+    cluster sizes interleaving); True: the points of one shape fused into one launch per colour (ea_batch_*).  Every point
+    must be the trajectory the oracle computes for that point alone."""
     from paper_1411_5512_b200.scan import Scan
     points = [{"L": L, "p": p, "T": 0.8, "seed": wl.seed_for(4, k)} for k, (L, p) in
               enumerate([(16, 0.5), (16, 0.77), (32, 0.6), (16, 1.0), (32, 0.9)])]
-    sc = Scan(points)
+    sc = Scan(points, fused=fused)
+    assert len(sc.batches) == (2 if fused is True else 0)
     sc.sweep(3)
     sc.snapshot(0)
-    sc.sweep(37)          # 32-sweep graph replay + direct launches, interleaved over the five streams
+    sc.sweep(37)          # fused: 32-sweep graph replay + direct launches; auto: one SMALL launch per point and call
     recs = sc.measure(slot=0, r_max=8)
     for pt, sim, rec in zip(points, sc.sims, recs):
         o = Oracle(pt["L"], pt["p"], pt["T"], n_replicas=2, seed=pt["seed"], n_slots=1)
