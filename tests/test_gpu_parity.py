@@ -715,6 +715,40 @@ def test_small_lattice_kernel_auto_choice_and_long_runs():
         binding.Sim(10, 0.5, 0.8, n_replicas=2, kernel="small")  # needs L % 4 == 0
 
 
+def test_randomised_differential_run_of_the_resident_kernels_against_the_per_colour_launches():
+    """Seeded random walk through the API on pairs of sims that differ only in the kernel: SMALL (L = 4 .. 32) / RESIDENT
+    (L = 128) against SCALAR / ROWS -- random chunking of the sweeps (1 .. 70 per call, so single-launch, graph and
+    persistent paths alternate), temperature changes (incl. T = 0 and T = inf), clock jumps (also across 2^32), dynamics
+    switches, spins written back through the API.  The per-colour kernels are oracle-checked elsewhere; here every call
+    sequence must leave both sims in the same state."""
+    rng = np.random.default_rng(0x14115512)
+    cases = [(int(L), int(n_rep)) for L in (4, 8, 12, 16, 20, 24, 32) for n_rep in (1, 2)] + [(128, 2)]
+    for L, n_rep in cases:
+        ref, fast = ("rows", "resident") if L == 128 else ("scalar", "small")
+        seed, p = int(rng.integers(1, 2 ** 62)), float(rng.choice([0.5, 0.77, 1.0, 0.0]))
+        a = binding.Sim(L, p, 0.8, n_replicas=n_rep, seed=seed, n_slots=0, kernel=ref)
+        b = binding.Sim(L, p, 0.8, n_replicas=n_rep, seed=seed, n_slots=0, kernel=fast)
+        for step in range(6 if L == 128 else 10):
+            op = int(rng.integers(0, 5))
+            if op == 0:
+                T = float(rng.choice([0.0, 0.5, 0.8, 1.1, 2.0, 4.5, float("inf")]))
+                a.set_temperature(T); b.set_temperature(T)
+            elif op == 1:
+                t = int(rng.choice([0, 7, 2 ** 32 - 3, 2 ** 40 + 5]))
+                a.time = t; b.time = t
+            elif op == 2 and L != 128:
+                dyn = str(rng.choice(["metropolis", "heatbath"]))
+                a.set_dynamics(dyn); b.set_dynamics(dyn)
+            elif op == 3:
+                w = wl.random_words(a.N, int(rng.integers(1, 2 ** 31)))
+                a.set_spins(w); b.set_spins(w)
+            n = int(rng.integers(1, 71)) if L != 128 else int(rng.integers(1, 25))
+            a.sweep(n); b.sweep(n)
+            assert a.time == b.time
+            assert np.array_equal(a.get_spins(), b.get_spins()), "L=%d n_rep=%d step %d (op %d, n %d)" % (L, n_rep, step, op, n)
+        a.close(); b.close()
+
+
 def test_ageing_protocol_driver_matches_the_oracle_step_by_step():
     """The paper's protocol (t_w = 1, 10, 100; t on the {1, 2, 5} x 10^m grid) through paper_1411_5512_b200.ageing,
     against the oracle driven by hand through the same schedule: cfg2's lattice (L = 32, 32 x 2)."""
