@@ -220,28 +220,28 @@ __device__ __forceinline__ uint32_t flip_half(uint32_t u1, uint32_t u2, uint32_t
     return f;
 }
 
-// Heat bath (C-HB): flip iff r < hb[n_u].  hb is increasing in n_u, so with k* the smallest k with r < hb[k] the
-// decision is [n_u >= k*]: a chain of seven predicated assignments from k = 6 down to 0 (the last one taken is k*).
-// n_u = b0 + 2 b1 + 4 b2 from the two full adders; [n_u >= k] are LOP3s of (b2, b1, b0).
-__device__ __forceinline__ uint32_t flip_half_heatbath(uint32_t u1, uint32_t u2, uint32_t u3, uint32_t u4, uint32_t u5,
-                                                       uint32_t u6, uint32_t r, const Thresholds &th)
+// Heat bath (C-HB): flip iff r < hb[n_u].  hb is increasing in n_u, so with k* the smallest k with r < hb[k] the spin flips
+// iff n_u >= k*.  In terms of a_d = j_d ^ n_d and their number n_a (n_u = n_a for s = 0, 6 - n_a for s = 1) the NEW spin is
+// [n_a >= k*] for s = 0 and [n_a >= 7 - k*] for s = 1; with the two full adders (sa, ka), (sb, kb) of the a_d and
+// M(x; a, b) = maj(x, a, b),  A = M(~s; ka, kb), A' = M(s; ka, kb), B = M(~s; sa, sb), B' = M(s; sa, sb):
+//   k* = 0: ~s   1: M(~s; A, B)   2: M(~s; A, B')   3: maj(ka, kb, B)   4: maj(ka, kb, B')   5: M(s; A', B)   6: M(s; A', B')   7: s
+// -- a chain of seven predicated assignments from k = 6 down to 0 (the last one taken is k*).  hb[k] == 2^32 (T = 0,
+// Delta E < 0: certain whatever r) cannot be expressed by the 32-bit compare and rides on hb_always[k].
+__device__ __forceinline__ uint32_t new_spin_half_heatbath(uint32_t s, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t a4, uint32_t a5,
+                                                           uint32_t a6, uint32_t r, const Thresholds &th)
 {
-    const HalfCount h = count_half(u1, u2, u3, u4, u5, u6);
-    const uint32_t b0 = h.sa ^ h.sb, c1 = h.sa & h.sb;
-    const uint32_t b1 = xor3(h.ka, h.kb, c1), b2 = maj3(h.ka, h.kb, c1);
-    const uint32_t ge1 = b2 | b1 | b0, ge2 = b2 | b1, ge3 = b2 | (b1 & b0), ge4 = b2, ge5 = b2 & (b1 | b0), ge6 = b2 & b1;
-    uint32_t f = 0;
-    if (r < th.hb[6]) f = ge6;
-    if (r < th.hb[5]) f = ge5;
-    if (r < th.hb[4]) f = ge4;
-    if (r < th.hb[3]) f = ge3;
-    if (r < th.hb[2]) f = ge2;
-    if (r < th.hb[1]) f = ge1;
-    if (r < th.hb[0]) f = 0xffffffffu;
-    // hb[k] == 2^32 (T = 0, Delta E < 0): certain, whatever r
-    f |= (th.hb_always[6] & ge6) | (th.hb_always[5] & ge5) | (th.hb_always[4] & ge4) | (th.hb_always[3] & ge3) |
-         (th.hb_always[2] & ge2) | (th.hb_always[1] & ge1) | th.hb_always[0];
-    return f;
+    const HalfCount h = count_half_lop3(a1, a2, a3, a4, a5, a6);
+    const uint32_t A = lop3<LUT_MAJ_NA>(s, h.ka, h.kb), A2 = lop3<LUT_MAJ>(s, h.ka, h.kb);
+    const uint32_t B = lop3<LUT_MAJ_NA>(s, h.sa, h.sb), B2 = lop3<LUT_MAJ>(s, h.sa, h.sb);
+    uint32_t n = s;
+    if (r < th.hb[6] || th.hb_always[6]) n = lop3<LUT_MAJ>(s, A2, B2);
+    if (r < th.hb[5] || th.hb_always[5]) n = lop3<LUT_MAJ>(s, A2, B);
+    if (r < th.hb[4] || th.hb_always[4]) n = lop3<LUT_MAJ>(h.ka, h.kb, B2);
+    if (r < th.hb[3] || th.hb_always[3]) n = lop3<LUT_MAJ>(h.ka, h.kb, B);
+    if (r < th.hb[2] || th.hb_always[2]) n = lop3<LUT_MAJ_NA>(s, A, B2);
+    if (r < th.hb[1] || th.hb_always[1]) n = lop3<LUT_MAJ_NA>(s, A, B);
+    if (r < th.hb[0] || th.hb_always[0]) n = ~s;
+    return n;
 }
 
 // 64-bit word <-> halves
@@ -268,13 +268,11 @@ __device__ __forceinline__ uint64_t metropolis_word(uint64_t s, uint64_t n1, uin
 {
     const uint32_t sl = lo32(s), sh = hi32(s);
     if (HB) {
-        const uint32_t fl = flip_half_heatbath(bond_lo(j1) ^ sl ^ lo32(n1), bond_lo(j2) ^ sl ^ lo32(n2),
-                                               bond_lo(j3) ^ sl ^ lo32(n3), bond_lo(j4) ^ sl ^ lo32(n4),
-                                               bond_lo(j5) ^ sl ^ lo32(n5), bond_lo(j6) ^ sl ^ lo32(n6), r_lo, th);
-        const uint32_t fh = flip_half_heatbath(bond_hi(j1) ^ sh ^ hi32(n1), bond_hi(j2) ^ sh ^ hi32(n2),
-                                               bond_hi(j3) ^ sh ^ hi32(n3), bond_hi(j4) ^ sh ^ hi32(n4),
-                                               bond_hi(j5) ^ sh ^ hi32(n5), bond_hi(j6) ^ sh ^ hi32(n6), r_hi, th);
-        return mk64(sl ^ fl, sh ^ fh);
+        const uint32_t nl = new_spin_half_heatbath(sl, bond_lo(j1) ^ lo32(n1), bond_lo(j2) ^ lo32(n2), bond_lo(j3) ^ lo32(n3),
+                                                   bond_lo(j4) ^ lo32(n4), bond_lo(j5) ^ lo32(n5), bond_lo(j6) ^ lo32(n6), r_lo, th);
+        const uint32_t nh = new_spin_half_heatbath(sh, bond_hi(j1) ^ hi32(n1), bond_hi(j2) ^ hi32(n2), bond_hi(j3) ^ hi32(n3),
+                                                   bond_hi(j4) ^ hi32(n4), bond_hi(j5) ^ hi32(n5), bond_hi(j6) ^ hi32(n6), r_hi, th);
+        return mk64(nl, nh);
     }
     if (RARE && !ALWAYS) {
         // In terms of a_d = j_d ^ n_d (J S_nbr = -1 seen from an up spin) and n_a = their number, n_u = n_a for s = 0 and
