@@ -250,7 +250,7 @@ def workload_config(cfg, args, ws):
             "L": cfg.L, "N": cfg.N, "p": cfg.p, "T": cfg.T, "n_replicas": cfg.n_replicas,
             "sweeps_per_step": args.sweeps_per_step,
             "step": "S sweeps = 2S half-sweeps (RESIDENT at L=128: one persistent launch; else one launch per colour) + "
-                    "snapshot + C(t,t_w) + C_4(r=0..L/2, 3 axes) + E + M",
+                    "snapshot + C(t,t_w) + C_4(r=0..L/2, 3 axes) + E + M (ea_snapshot + ea_measure)",
             "l2": "flushed between timed steps (a %d MiB buffer is overwritten); inside a step the %.0f MiB "
                   "lattice is re-swept S times and stays on the chip (spins in shared memory, bonds in L2 for the "
                   "RESIDENT kernel; all of it in L2 for the per-colour kernels), as in the paper's 10^7-sweep runs"
@@ -284,12 +284,8 @@ def run_ours(args, cfg):
 
     def measure_point():
         sim.snapshot(0)
-        out = [sim.autocorr(0)]
-        if cfg.n_replicas == 2:
-            out.append(sim.c4(r_max, with_q=True))
-        out.append(sim.energy())
-        out.append(sim.magnetisation())
-        return out
+        rec = sim.measure(slot=0, r_max=r_max if cfg.n_replicas == 2 else None)  # ea_measure: A, B, q, E, M in one call
+        return [rec[k] for k in ("A", "B", "q", "E", "M") if k in rec]
 
     def step(timed):
         with torch.cuda.stream(stream):

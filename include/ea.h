@@ -168,6 +168,13 @@ ea_status ea_energy(ea_sim *sim, int64_t *E);
 /* M[b] = sum_i S_i,b (C-S14); host array of 64. */
 ea_status ea_magnetisation(ea_sim *sim, int64_t *M);
 
+/* One measure point (the observables the paper took from every stored configuration) in ONE call: the same
+ * numbers as ea_autocorr(slot) / ea_c4(r_max) / ea_energy / ea_magnetisation, but all kernels are enqueued back to back and
+ * the host waits once (five separate calls cost five round trips, ~25 us each -- as much as the kernels at L = 128).
+ * Any of A [64], B [3][r_max+1][32] (+ q [32]), E [64], M [64] may be NULL (skipped); slot / r_max are ignored when A / B is
+ * NULL.  Errors as the separate calls; outputs untouched on error. */
+ea_status ea_measure(ea_sim *sim, int slot, int r_max, int64_t *A, int64_t *B, int64_t *q, int64_t *E, int64_t *M);
+
 /* Canonical packed I/O (host arrays: spins N words, bonds 3N words).
  * ea_set_bonds on a 2-replica sim: EA_ERR_INVALID unless hi half == lo half in every word (checked on the device
  * while packing: after this error the sim's bonds are undefined and must be set again). */

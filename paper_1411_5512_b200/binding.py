@@ -62,6 +62,7 @@ SIGNATURES = {
     "ea_integral_estimator": (_i, [_i, _vp, _vp, _vp, _i, _vp]),
     "ea_energy": (_i, [_vp, _vp]),
     "ea_magnetisation": (_i, [_vp, _vp]),
+    "ea_measure": (_i, [_vp, _i, _i, _vp, _vp, _vp, _vp, _vp]),
     "ea_get_spins": (_i, [_vp, _vp]),
     "ea_set_spins": (_i, [_vp, _vp]),
     "ea_get_bonds": (_i, [_vp, _vp]),
@@ -278,6 +279,24 @@ class Sim:
         M = np.zeros(LANES, dtype=np.int64)
         self._ck(lib().ea_magnetisation(self._h, _ptr(M)))
         return M
+
+    def measure(self, slot=None, r_max=None, energy=True, magnetisation=True):
+        """One measure point in one call (ea_measure): dict with A (if slot is given), B and q (if r_max is given; 2 replicas),
+        E, M -- the same integers as the separate calls."""
+        out = {}
+        A = np.zeros(LANES, dtype=np.int64) if slot is not None else None
+        B = np.zeros((3, int(r_max) + 1, LANES // 2), dtype=np.int64) if r_max is not None else None
+        q = np.zeros(LANES // 2, dtype=np.int64) if r_max is not None else None
+        E = np.zeros(LANES, dtype=np.int64) if energy else None
+        M = np.zeros(LANES, dtype=np.int64) if magnetisation else None
+        nul = C.c_void_p(None)
+        self._ck(lib().ea_measure(self._h, -1 if slot is None else int(slot), 0 if r_max is None else int(r_max),
+                                  nul if A is None else _ptr(A), nul if B is None else _ptr(B), nul if q is None else _ptr(q),
+                                  nul if E is None else _ptr(E), nul if M is None else _ptr(M)))
+        for k, v in (("A", A), ("B", B), ("q", q), ("E", E), ("M", M)):
+            if v is not None:
+                out[k] = v
+        return out
 
     # -- canonical packed I/O -----------------------------------------------------------------------------
     def get_spins(self, out=None):

@@ -622,6 +622,39 @@ ea_status ea_c4(ea_sim *sim, int r_max, int64_t *B, int64_t *q, double *c4_avg)
     return EA_OK;
 }
 
+ea_status ea_measure(ea_sim *sim, int slot, int r_max, int64_t *A, int64_t *B, int64_t *q, int64_t *E, int64_t *M)
+{
+    if (!sim) return EA_ERR_INVALID;
+    if (A) {
+        if (slot < 0 || slot >= sim->n_slots) EA_FAIL(sim, EA_ERR_INVALID, "slot %d out of range [0,%d)", slot, sim->n_slots);
+        if (!sim->slot_set[slot]) EA_FAIL(sim, EA_ERR_STATE, "slot %d holds no snapshot", slot);
+    }
+    if (B || q) {
+        if (!B) EA_FAIL(sim, EA_ERR_INVALID, "q without B");
+        if (sim->n_replicas != 2) EA_FAIL(sim, EA_ERR_STATE, "C_4 needs a 2-replica sim");
+        if (r_max < 0 || r_max > sim->lat.L / 2) EA_FAIL(sim, EA_ERR_INVALID, "r_max %d outside [0, L/2]", r_max);
+    }
+    DeviceGuard g(sim->device);
+    EA_CUDA(sim, fold_ensure_unfolded(sim));
+    // counter regions: [C_4: 3 (r_max + 1) x 32, overlap 32] [A 64] [E 64] [M 64]; all kernels enqueued, then ONE copy and sync
+    const size_t n_r = (size_t)(B ? r_max + 1 : 0), c4_words = B ? (3 * n_r + 1) * 32 : 0;
+    const size_t off_A = (c4_words + 63) & ~(size_t)63, off_E = off_A + 64, off_M = off_E + 64, total = off_M + 64;
+    if (total > sim->n_counters) EA_FAIL(sim, EA_ERR_STATE, "counter space exhausted");
+    if (B) EA_CUDA(sim, launch_count_c4(sim, r_max));
+    if (A) EA_CUDA(sim, launch_count_spins(sim, sim->snaps + (size_t)slot * sim->N, sim->counters + off_A));
+    if (E) EA_CUDA(sim, launch_count_energy(sim, sim->counters + off_E));
+    if (M) EA_CUDA(sim, launch_count_spins(sim, nullptr, sim->counters + off_M));
+    ea_status rc = fetch_counters(sim, total);
+    if (rc != EA_OK) return rc;
+    const unsigned long long *h = sim->h_counters.data();
+    if (B) for (size_t k = 0; k < 3 * n_r * 32; ++k) B[k] = sim->N - 2 * (int64_t)h[k];
+    if (q) for (int b = 0; b < 32; ++b) q[b] = sim->N - 2 * (int64_t)h[3 * n_r * 32 + b];
+    if (A) for (int b = 0; b < 64; ++b) A[b] = sim->N - 2 * (int64_t)h[off_A + b];
+    if (E) for (int b = 0; b < 64; ++b) E[b] = -3 * sim->N + 2 * (int64_t)h[off_E + b];
+    if (M) for (int b = 0; b < 64; ++b) M[b] = sim->N - 2 * (int64_t)h[off_M + b];
+    return EA_OK;
+}
+
 ea_status ea_c4_vectors(ea_sim *sim, int64_t n_vec, const int32_t *dxyz, int64_t *B)
 {
     if (!sim || n_vec < 0 || (n_vec && (!dxyz || !B))) return EA_ERR_INVALID;

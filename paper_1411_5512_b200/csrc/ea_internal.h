@@ -124,8 +124,9 @@ cudaError_t launch_pack_bonds(ea_sim *s, int d, const uint64_t *d_canon, unsigne
 cudaError_t launch_unpack_bonds(ea_sim *s, int d, uint64_t *d_canon);
 
 // observables: per-sample bit counts into s->counters (zeroed by the wrapper)
-cudaError_t launch_count_spins(ea_sim *s, const uint64_t *d_other /* nullable: XOR partner, same layout */);
-cudaError_t launch_count_energy(ea_sim *s);
+// (dst: 64 counters; nullptr = s->counters)
+cudaError_t launch_count_spins(ea_sim *s, const uint64_t *d_other /* nullable: XOR partner, same layout */, unsigned long long *dst = nullptr);
+cudaError_t launch_count_energy(ea_sim *s, unsigned long long *dst = nullptr);
 cudaError_t launch_count_c4(ea_sim *s, int r_max); // counters[(d*(r_max+1)+r)*32+b], then [3*(r_max+1)*32 + b] = overlap
 
 // full-vector C_4 (ea_c4_vectors.cu): per-sample counts of q_i != q_{i+r} for n lattice vectors; host result

@@ -370,23 +370,25 @@ static unsigned grid_for(const ea_sim *s, size_t items)
     return (unsigned)(need < cap ? (need ? need : 1) : cap);
 }
 
-cudaError_t launch_count_spins(ea_sim *s, const uint64_t *d_other)
+cudaError_t launch_count_spins(ea_sim *s, const uint64_t *d_other, unsigned long long *dst)
 {
-    cudaError_t e = cudaMemsetAsync(s->counters, 0, 64 * sizeof(unsigned long long), s->stream);
+    if (!dst) dst = s->counters;
+    cudaError_t e = cudaMemsetAsync(dst, 0, 64 * sizeof(unsigned long long), s->stream);
     if (e != cudaSuccess) return e;
-    k_count_spins<<<grid_for(s, s->N), 256, 0, s->stream>>>(s->lat, s->spins, d_other, s->counters);
+    k_count_spins<<<grid_for(s, s->N), 256, 0, s->stream>>>(s->lat, s->spins, d_other, dst);
     s->count_launch();
     return cudaGetLastError();
 }
 
-cudaError_t launch_count_energy(ea_sim *s)
+cudaError_t launch_count_energy(ea_sim *s, unsigned long long *dst)
 {
-    cudaError_t e = cudaMemsetAsync(s->counters, 0, 64 * sizeof(unsigned long long), s->stream);
+    if (!dst) dst = s->counters;
+    cudaError_t e = cudaMemsetAsync(dst, 0, 64 * sizeof(unsigned long long), s->stream);
     if (e != cudaSuccess) return e;
     if (s->n_replicas == 2)
-        k_count_energy<uint32_t><<<grid_for(s, s->N), 256, 0, s->stream>>>(s->lat, s->spins, (const uint32_t *)s->bonds, s->counters);
+        k_count_energy<uint32_t><<<grid_for(s, s->N), 256, 0, s->stream>>>(s->lat, s->spins, (const uint32_t *)s->bonds, dst);
     else
-        k_count_energy<uint64_t><<<grid_for(s, s->N), 256, 0, s->stream>>>(s->lat, s->spins, (const uint64_t *)s->bonds, s->counters);
+        k_count_energy<uint64_t><<<grid_for(s, s->N), 256, 0, s->stream>>>(s->lat, s->spins, (const uint64_t *)s->bonds, dst);
     s->count_launch();
     return cudaGetLastError();
 }

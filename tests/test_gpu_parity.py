@@ -715,6 +715,34 @@ def test_small_lattice_kernel_auto_choice_and_long_runs():
         binding.Sim(10, 0.5, 0.8, n_replicas=2, kernel="small")  # needs L % 4 == 0
 
 
+@pytest.mark.parametrize("L,n_rep", [(8, 1), (12, 2), (32, 2), (64, 2), (128, 2)])
+def test_measure_point_in_one_call_equals_the_separate_calls_and_the_oracle(L, n_rep):
+    """ea_measure (all observables of a measure point enqueued back to back, one copy, one wait) against ea_autocorr /
+    ea_c4 / ea_energy / ea_magnetisation and, at the sizes the oracle does in seconds, against the oracle."""
+    g, o = make_pair(L, 0.7, 0.8, n_rep, wl.seed_for(9, L), n_slots=1)
+    n0, n1 = (2, 3) if L >= 64 else (5, 20)
+    g.sweep(n0); g.snapshot(0); g.sweep(n1)
+    r_max = L // 2 if n_rep == 2 else None
+    rec = g.measure(slot=0, r_max=r_max)
+    assert np.array_equal(rec["A"], g.autocorr(0)) and np.array_equal(rec["E"], g.energy())
+    assert np.array_equal(rec["M"], g.magnetisation())
+    if n_rep == 2:
+        B, q = g.c4(r_max, with_q=True)
+        assert np.array_equal(rec["B"], B) and np.array_equal(rec["q"], q)
+    part = g.measure(energy=False)                       # subsets: only M
+    assert set(part) == {"M"} and np.array_equal(part["M"], rec["M"])
+    if L <= 64:
+        o.sweep(n0); o.snapshot(0); o.sweep(n1)
+        assert np.array_equal(rec["A"], o.autocorr(0)) and np.array_equal(rec["E"], o.energy())
+        assert np.array_equal(rec["M"], o.magnetisation())
+        if n_rep == 2:
+            assert np.array_equal(rec["B"], o.c4(r_max)) and np.array_equal(rec["q"], o.overlap())
+    if n_rep == 1:
+        with pytest.raises(binding.EAError):
+            g.measure(r_max=2)
+    g.close()
+
+
 def test_randomised_differential_run_of_the_resident_kernels_against_the_per_colour_launches():
     """Seeded random walk through the API on pairs of sims that differ only in the kernel: SMALL (L = 4 .. 32) / RESIDENT
     (L = 128) against SCALAR / ROWS -- random chunking of the sweeps (1 .. 70 per call, so single-launch, graph and
