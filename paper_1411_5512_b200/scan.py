@@ -67,11 +67,8 @@ class Scan:
         """Per point: dict of the per-sample integer observables (E, M, and A for `slot`, B / q for r_max)."""
         out = []
         for s in self.sims:
-            rec = {"t": s.time, "E": s.energy(), "M": s.magnetisation()}
-            if slot is not None:
-                rec["A"] = s.autocorr(slot)
-            if r_max is not None and s.n_replicas == 2:
-                rec["B"], rec["q"] = s.c4(min(r_max, s.L // 2), with_q=True)
+            rec = s.measure(slot=slot, r_max=min(r_max, s.L // 2) if r_max is not None and s.n_replicas == 2 else None)
+            rec["t"] = s.time
             out.append(rec)
         return out
 
