@@ -5,9 +5,10 @@
 // Same update and the same stream contract as every other variant, hence bit-identical.  The lattice is cut into C
 // slabs of L x L x (L / C) sites along z, one CTA per slab:
 //   * C = 1 (L <= 16): one CTA, the colour barrier is __syncthreads();
-//   * C = 2 .. 16 (L = 32: 16 CTAs of 2 planes): one thread-block CLUSTER; a slab's boundary planes are read straight out
-//     of the neighbouring CTA's shared memory (distributed shared memory, ld.shared::cluster) and the colour barrier is
-//     the cluster barrier (barrier.cluster.arrive.release / wait.acquire) -- no global memory traffic between sweeps.
+//   * C = 2 .. 16 (L = 32: 16 CTAs of 2 planes): one thread-block CLUSTER; a thread on a boundary plane PUSHES its new
+//     pair into the halo plane of the neighbouring CTA's shared memory (st.async through distributed shared memory) and the
+//     colour barrier is an mbarrier per CTA that counts its own warps and the bytes its two neighbours pushed -- no global
+//     memory traffic, no cluster-wide barrier and no fence wider than the CTA between sweeps (see PUSH below).
 // Spins AND bond words live in shared memory; global memory is read once at the start and written once at the end.
 // A thread owns one pair of x-adjacent same-colour sites of each colour (one Philox block per pair and sweep, C-A7).
 #include <string.h>
@@ -35,12 +36,6 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank)
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
     return r;
 }
-__device__ __forceinline__ ulonglong2 ld_cluster128(uint32_t addr)
-{
-    ulonglong2 v;
-    asm volatile("ld.shared::cluster.v2.u64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "r"(addr) : "memory");
-    return v;
-}
 __device__ __forceinline__ uint32_t cluster_ctarank()
 {
     uint32_t r;
@@ -66,17 +61,61 @@ __device__ __forceinline__ ulonglong2 lds_v2u64(uint32_t addr)
     asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "r"(addr) : "memory");
     return v;
 }
-__device__ __forceinline__ void lds_bond(uint32_t addr, uint32_t &v) { asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory"); }
-__device__ __forceinline__ void lds_bond(uint32_t addr, uint64_t &v) { asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(addr) : "memory"); }
+// the thread's twelve bond words of one colour: BondT [12 sizeof(BondT) / 16][n_threads] vectors of 16 bytes, so that every
+// load is one conflict-free LDS.128 of the warp
+__device__ __forceinline__ void lds_bonds12(uint32_t addr, uint32_t stride, uint32_t (&j)[12])
+{
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(j[4 * k]), "=r"(j[4 * k + 1]), "=r"(j[4 * k + 2]), "=r"(j[4 * k + 3])
+                     : "r"(addr + k * stride) : "memory");
+}
+__device__ __forceinline__ void lds_bonds12(uint32_t addr, uint32_t stride, uint64_t (&j)[12])
+{
+#pragma unroll
+    for (int k = 0; k < 6; ++k)
+        asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(j[2 * k]), "=l"(j[2 * k + 1]) : "r"(addr + k * stride) : "memory");
+}
 __device__ __forceinline__ void sts_v2u64(uint32_t addr, ulonglong2 v)
 {
     asm volatile("st.shared.v2.u64 [%0], {%1, %2};" ::"r"(addr), "l"(v.x), "l"(v.y) : "memory");
 }
 
+// mbarrier of the push exchange (PUSH): local arrivals of the CTA's warps + the bytes the two neighbours push
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile("{\n"
+                 ".reg .pred p;\n"
+                 "WAIT_%=:\n"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+                 "@!p bra WAIT_%=;\n"
+                 "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// 16 bytes into a neighbouring CTA's shared memory; the bytes are counted on that CTA's mbarrier when they have landed
+__device__ __forceinline__ void st_async_v2u64(uint32_t remote, ulonglong2 v, uint32_t remote_bar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b64 [%0], {%1, %2}, [%3];" ::"r"(remote), "l"(v.x),
+                 "l"(v.y), "r"(remote_bar) : "memory");
+}
+
 // Shared-memory addresses of everything one half-sweep of colour c touches for the thread's pair
 struct SmallAddr {
-    uint32_t own, x0, x1, x2, pm, pp, zm, zp;   // spins: own pair; the row's three other-colour words; y -/+ and z -/+ pairs
-    uint32_t jx, jy, jz, bl0, bl1, by, bz;      // bonds: forward pairs of the own sites; +x bonds of the left neighbours; backward y, z pairs
+    uint32_t own, xa, xe, pm, pp, zm, zp;       // spins: own pair; the other colour's pair at the same place and the row's third
+                                                // other-colour word next to it; y -/+ and z -/+ pairs
+    uint32_t bonds;                             // the thread's bond vectors of this colour
+    uint32_t push_lo, push_hi;                  // PUSH: where the own pair goes in the CTA below / above (shared::cluster addresses)
 };
 
 __device__ __forceinline__ void cluster_barrier()
@@ -84,42 +123,61 @@ __device__ __forceinline__ void cluster_barrier()
     asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
     asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
-// (A neighbour-only barrier -- remote mbarrier arrives on the two z-neighbouring CTAs, release / acquire at cluster scope --
-// was measured SLOWER than the hardware cluster barrier: L = 16 on 4 CTAs 0.81 against 0.67 us per half-sweep, L = 32 on 16
-// CTAs 1.32 against 1.15.  The hardware barrier is split instead: arrive, draw the next random numbers, wait.)
+// (only at the start and the end of the kernel: see PUSH)
 
 // Shared memory of one CTA (nh = L L Lz / 2 words per colour of the slab, pw = L L / 2 words per colour and plane):
 //   spins  uint64 [2][nh]
-//   bonds  BondT  [2][3][nh]
-//   bzh    BondT  [2][pw]      z-bonds of the plane below the slab (the backward z bonds of the slab's first plane)
+//   bonds  BondT  [2][12][n_threads] in vectors of 16 bytes: per colour and thread {jx, jx', jy, jy', jz, jz', bl, bl', by, by',
+//                 bz, bz'} = the forward bonds of the pair's two sites, the +x bonds of their left neighbours, the +y / +z bonds of
+//                 their y - 1 / z - 1 neighbours.  Every bond sits there twice (forward for one colour, backward for the other):
+//                 the addresses never change, so each thread keeps its own copy where one LDS.128 per four words fetches it.
+//   halo   uint64 [2][2][pw]   PUSH: the spin planes below / above the slab, both colours, as the neighbours pushed them
+//   bar    uint64 [2]          PUSH: one mbarrier per colour
+//
+// PUSH (clusters): no cluster barrier in the sweep loop.  barrier.cluster.arrive.release / wait.acquire compile to
+// MEMBAR.ALL.GPU + UCGABAR + CCTL.IVALL (measured ~850 clocks per barrier on 8 CTAs, ~1240 on 16), and so does every other
+// release / acquire at cluster scope (remote mbarrier arrives were slower still).  Instead a thread on a boundary plane
+// stores its new pair into its own slab AND into the facing halo plane of the neighbouring CTA with st.async (STAS), which
+// counts the bytes on that CTA's mbarrier when they have landed; the warps of a CTA arrive on the same mbarrier after
+// their stores.  A half-sweep of colour c completes phase (sweep & 1) of bar[c]; everybody waits on it before the next
+// half-sweep and reads only LOCAL shared memory.  Hazards: a halo word is rewritten two half-sweeps later, which the
+// neighbour starts only after THIS CTA's pushes of the half-sweep between, each made by the thread that read the word.
+// Measured (B200, us per half-sweep, L = 16 / 32): cluster barrier + remote loads 0.59 / 1.03; pushes 0.36 / 0.71.  Not
+// kept: cp.async.bulk of the whole plane by one thread (0.50 / 1.00: the copy starts only after a CTA-wide barrier), two
+// interleaved chains of row classes as in the L = 128 kernel (0.69 at L = 32: a unit's latency, not its issue slots, sets
+// the pace; the pushes cost ~2 clocks per 16-byte packet of the SM-to-SM network whoever overlaps them).
 template <typename BondT, bool ALWAYS, bool RARE, bool HB, bool CLUSTER>
 __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
 {
+    constexpr bool PUSH = CLUSTER;
     extern __shared__ __align__(16) unsigned char smem_small[];
     const unsigned L = a.L, Lh = L / 2, Lz = a.Lz, hp = Lh / 2; // hp: pairs per row
     const unsigned pw = L * Lh, nh = pw * Lz, Nh = pw * L;
     const unsigned rank = CLUSTER ? cluster_ctarank() : 0, C = CLUSTER ? cluster_nctarank() : 1;
     const unsigned z0 = rank * Lz;
     uint64_t *spins_s = (uint64_t *)smem_small;
-    BondT *bonds_s = (BondT *)(spins_s + 2 * nh);
-    BondT *bzh_s = bonds_s + 6 * nh;
-    const BondT *__restrict__ gb = (const BondT *)a.bonds;
     const unsigned tid = threadIdx.x, nthr = blockDim.x;
+    BondT *bonds_s = (BondT *)(spins_s + 2 * nh);
+    uint64_t *halo_s = (uint64_t *)(bonds_s + 24 * nthr);
+    uint64_t *bar_s = halo_s + 4 * pw;
+    const BondT *__restrict__ gb = (const BondT *)a.bonds;
 
     // ---- prologue: the slab (contiguous in every colour / direction plane of the global arrays) ------------------
     for (unsigned v = tid; v < 2 * nh; v += nthr) {
         const unsigned c = v / nh, i = v % nh;
         spins_s[v] = a.spins[(size_t)c * Nh + (size_t)pw * z0 + i];
     }
-    for (unsigned v = tid; v < 6 * nh; v += nthr) {
-        const unsigned cd = v / nh, i = v % nh;
-        bonds_s[v] = gb[(size_t)cd * Nh + (size_t)pw * z0 + i];
-    }
-    {
-        const unsigned zb = (z0 + L - 1) % L;
-        for (unsigned v = tid; v < 2 * pw; v += nthr) {
-            const unsigned c = v / pw, i = v % pw;
-            bzh_s[v] = gb[(size_t)(c * 3 + 2) * Nh + (size_t)pw * zb + i];
+
+    if (PUSH) {
+        for (unsigned v = tid; v < 4 * pw; v += nthr) {
+            const unsigned side = v / (2 * pw), c = (v / pw) & 1u, i = v % pw;
+            const unsigned zh = side ? (z0 + Lz) % L : (z0 + L - 1) % L;
+            halo_s[v] = a.spins[(size_t)c * Nh + (size_t)pw * zh + i];
+        }
+        if (tid == 0) {
+            mbar_init(small_smem_u32(bar_s), nthr / 32);
+            mbar_init(small_smem_u32(bar_s + 1), nthr / 32);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
     }
 
@@ -136,11 +194,10 @@ __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
     const unsigned i_zm = Lh * (y + L * (lo_edge ? Lz - 1 : zl - 1)) + 2 * p;
     const unsigned i_zp = Lh * (y + L * (hi_edge ? 0 : zl + 1)) + 2 * p;
     const uint32_t spins_a = small_smem_u32(spins_s);
-    uint32_t base_zm = spins_a, base_zp = spins_a; // shared::cluster addresses of the spin array that holds the z -/+ neighbour
-    if (CLUSTER) {
-        base_zm = mapa_u32(spins_a, lo_edge ? (rank + C - 1) % C : rank);
-        base_zp = mapa_u32(spins_a, hi_edge ? (rank + 1) % C : rank);
-    }
+    const uint32_t halo_a = small_smem_u32(halo_s), bar_a = small_smem_u32(bar_s);
+    const uint32_t halo_below = PUSH ? mapa_u32(halo_a, (rank + C - 1) % C) : 0, halo_above = PUSH ? mapa_u32(halo_a, (rank + 1) % C) : 0;
+    const uint32_t bar_below = PUSH ? mapa_u32(bar_a, (rank + C - 1) % C) : 0, bar_above = PUSH ? mapa_u32(bar_a, (rank + 1) % C) : 0;
+    const unsigned i_pl = Lh * y + 2 * p; // the pair inside its plane
     const unsigned zg = z0 + zl;
     const uint32_t site_row = L * (y + L * zg);
 
@@ -148,56 +205,80 @@ __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
     // q, q + 1, q + 2 with q = 2p - 1 + S (periodic)
     unsigned Sc[2];
     SmallAddr A[2];
-    const uint32_t bonds_a = small_smem_u32(bonds_s), bzh_a = small_smem_u32(bzh_s);
-    constexpr unsigned BS = sizeof(BondT);
+    const uint32_t bonds_a = small_smem_u32(bonds_s);
+    constexpr unsigned BS = sizeof(BondT), VEC = 16 / BS; // bond words per 16-byte vector
+    const uint32_t bond_stride = 16 * nthr;
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
         Sc[c] = (c ^ y ^ zg) & 1u;
         const unsigned q0 = (2 * p + Sc[c] + Lh - 1) % Lh, q1 = (q0 + 1) % Lh, q2 = (q1 + 1) % Lh;
         const unsigned own_w = c * nh, oth_w = (1 - c) * nh;
         A[c].own = spins_a + (own_w + i0) * 8;
-        A[c].x0 = spins_a + (oth_w + rowb + q0) * 8;
-        A[c].x1 = spins_a + (oth_w + rowb + q1) * 8;
-        A[c].x2 = spins_a + (oth_w + rowb + q2) * 8;
+        A[c].xa = spins_a + (oth_w + i0) * 8;
+        A[c].xe = spins_a + (oth_w + rowb + (Sc[c] ? q2 : q0)) * 8;
         A[c].pm = spins_a + (oth_w + i_ym) * 8;
         A[c].pp = spins_a + (oth_w + i_yp) * 8;
-        A[c].zm = base_zm + (oth_w + i_zm) * 8;
-        A[c].zp = base_zp + (oth_w + i_zp) * 8;
-        const unsigned jc_w = c * 3 * nh, jo_w = (1 - c) * 3 * nh;
-        A[c].jx = bonds_a + (jc_w + i0) * BS;
-        A[c].jy = bonds_a + (jc_w + nh + i0) * BS;
-        A[c].jz = bonds_a + (jc_w + 2 * nh + i0) * BS;
-        A[c].bl0 = bonds_a + (jo_w + rowb + q0) * BS;
-        A[c].bl1 = bonds_a + (jo_w + rowb + q1) * BS;
-        A[c].by = bonds_a + (jo_w + nh + i_ym) * BS;
-        A[c].bz = lo_edge ? bzh_a + ((1 - c) * pw + Lh * y + 2 * p) * BS : bonds_a + (jo_w + 2 * nh + i_zm) * BS;
+        A[c].zm = PUSH && lo_edge ? halo_a + ((1 - c) * pw + i_pl) * 8 : spins_a + (oth_w + i_zm) * 8;
+        A[c].zp = PUSH && hi_edge ? halo_a + ((2 + 1 - c) * pw + i_pl) * 8 : spins_a + (oth_w + i_zp) * 8;
+        A[c].push_lo = halo_below + ((2 + c) * pw + i_pl) * 8; // the slab's first plane is the plane ABOVE the CTA below
+        A[c].push_hi = halo_above + (c * pw + i_pl) * 8;
+        A[c].bonds = bonds_a + c * (12 / VEC) * bond_stride + 16 * tid;
+        if (active) { // the thread's copy of its bonds, straight from the global arrays [2][3][Nh]
+            const size_t g_row = (size_t)Lh * (y + (size_t)L * zg), g_ym = (size_t)Lh * (ym + (size_t)L * zg);
+            const size_t g_zm = (size_t)Lh * (y + (size_t)L * ((zg + L - 1) % L));
+            const BondT *jc = gb + (size_t)c * 3 * Nh, *jo = gb + (size_t)(1 - c) * 3 * Nh;
+            // +x bonds: jx / jx' of the own sites (towards compact q1 / q2), bl / bl' of their left neighbours q0 / q1
+            const BondT jx = jc[g_row + 2 * p], jx2 = jc[g_row + 2 * p + 1], bl = jo[g_row + q0], bl2 = jo[g_row + q1];
+            const bool S = Sc[c];
+            const BondT w[12] = {S ? bl : jx, S ? bl2 : jx2, jc[Nh + g_row + 2 * p], jc[Nh + g_row + 2 * p + 1],
+                                 jc[2 * (size_t)Nh + g_row + 2 * p], jc[2 * (size_t)Nh + g_row + 2 * p + 1],
+                                 S ? jx : bl, S ? jx2 : bl2,
+                                 jo[Nh + g_ym + 2 * p], jo[Nh + g_ym + 2 * p + 1],
+                                 jo[2 * (size_t)Nh + g_zm + 2 * p], jo[2 * (size_t)Nh + g_zm + 2 * p + 1]};
+#pragma unroll
+            for (int k = 0; k < 12; ++k) bonds_s[((size_t)c * (12 / VEC) + k / VEC) * VEC * nthr + (size_t)VEC * tid + k % VEC] = w[k];
+        }
     }
     const uint32_t site0 = site_row + 4 * p + Sc[0], site1 = site_row + 4 * p + Sc[1]; // first site of the pair, colour 0 / 1
 
-    auto half_sweep = [&](const SmallAddr &ad, const uint4 r) {
-        const uint64_t X0 = lds_u64(ad.x0), X1 = lds_u64(ad.x1), X2 = lds_u64(ad.x2);
-        const ulonglong2 own = lds_v2u64(ad.own), Pm = lds_v2u64(ad.pm), Pp = lds_v2u64(ad.pp);
-        const ulonglong2 Zm = CLUSTER ? ld_cluster128(ad.zm) : lds_v2u64(ad.zm);
-        const ulonglong2 Zp = CLUSTER ? ld_cluster128(ad.zp) : lds_v2u64(ad.zp);
-        BondT jxA, jxB, jyA, jyB, jzA, jzB, bl0, bl1, byA, byB, bzA, bzB;
-        lds_bond(ad.jx, jxA); lds_bond(ad.jx + BS, jxB);
-        lds_bond(ad.jy, jyA); lds_bond(ad.jy + BS, jyB);
-        lds_bond(ad.jz, jzA); lds_bond(ad.jz + BS, jzB);
-        lds_bond(ad.bl0, bl0); lds_bond(ad.bl1, bl1);
-        lds_bond(ad.by, byA); lds_bond(ad.by + BS, byB);
-        lds_bond(ad.bz, bzA); lds_bond(ad.bz + BS, bzB);
+    // the thread's own pairs stay in registers between the sweeps (nobody else writes them); shared memory holds the copy
+    // the neighbours read
+    ulonglong2 own_r[2];
+    auto half_sweep = [&](const SmallAddr &ad, const uint4 r, const unsigned c, const bool S) {
+        // the row's other-colour words next to the pair: compact q0, q0 + 1, q0 + 2 with q0 = 2p - 1 + S
+        const ulonglong2 Xa = lds_v2u64(ad.xa);
+        const uint64_t Xe = lds_u64(ad.xe);
+        // first word: x neighbours Xa.x and (S ? Xa.y : Xe); second word: Xa.y and (S ? Xe : Xa.x).  The thread's x-bond
+        // words are stored in that order (the six terms of the local field are symmetric: only the pairing matters).
+        const uint64_t A2 = S ? Xa.y : Xe, B2 = S ? Xe : Xa.x;
+        const ulonglong2 own = own_r[c], Pm = lds_v2u64(ad.pm), Pp = lds_v2u64(ad.pp);
+        const ulonglong2 Zm = lds_v2u64(ad.zm), Zp = lds_v2u64(ad.zp);
+        BondT j[12];
+        lds_bonds12(ad.bonds, bond_stride, j);
+        const BondT xA1 = j[0], xB1 = j[1], jyA = j[2], jyB = j[3], jzA = j[4], jzB = j[5], xA2 = j[6], xB2 = j[7], byA = j[8],
+                    byB = j[9], bzA = j[10], bzB = j[11];
         ulonglong2 out;
-        out.x = metropolis_word<BondT, ALWAYS, RARE, HB>(own.x, X1, X0, Pp.x, Pm.x, Zp.x, Zm.x, jxA, bl0, jyA, byA, jzA, bzA, r.x, r.y, a.th);
-        out.y = metropolis_word<BondT, ALWAYS, RARE, HB>(own.y, X2, X1, Pp.y, Pm.y, Zp.y, Zm.y, jxB, bl1, jyB, byB, jzB, bzB, r.z, r.w, a.th);
+        out.x = metropolis_word<BondT, ALWAYS, RARE, HB>(own.x, Xa.x, A2, Pp.x, Pm.x, Zp.x, Zm.x, xA1, xA2, jyA, byA, jzA, bzA, r.x, r.y, a.th);
+        out.y = metropolis_word<BondT, ALWAYS, RARE, HB>(own.y, Xa.y, B2, Pp.y, Pm.y, Zp.y, Zm.y, xB1, xB2, jyB, byB, jzB, bzB, r.z, r.w, a.th);
         sts_v2u64(ad.own, out);
+        own_r[c] = out;
+        if (PUSH) {
+            if (lo_edge) st_async_v2u64(ad.push_lo, out, bar_below + 8 * c);
+            if (hi_edge) st_async_v2u64(ad.push_hi, out, bar_above + 8 * c);
+        }
     };
 
     // end of a half-sweep: arrive at the colour barrier, draw the next random numbers meanwhile, wait
-    auto barrier_begin = [&]() {
-        if (CLUSTER) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    const uint32_t tx_bytes = 2 * pw * 8; // what the two neighbours push per half-sweep
+    auto barrier_begin = [&](const unsigned c) {
+        if (PUSH) {
+            __syncwarp();
+            if (tid == 0) mbar_arrive_expect_tx(bar_a + 8 * c, tx_bytes);
+            else if ((tid & 31u) == 0) mbar_arrive(bar_a + 8 * c);
+        }
     };
-    auto barrier_end = [&]() {
-        if (CLUSTER) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+    auto barrier_end = [&](const unsigned c, const uint32_t parity) {
+        if (PUSH) mbar_wait(bar_a + 8 * c, parity);
         else __syncthreads();
     };
 
@@ -206,17 +287,24 @@ __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
     uint4 r = sweep_random4(g, site0);
     if (CLUSTER) cluster_barrier(); else __syncthreads(); // every CTA of the cluster has its slab in place
 
+    own_r[0] = own_r[1] = make_ulonglong2(0, 0);
+    if (active) {
+        own_r[0] = lds_v2u64(A[0].own);
+        own_r[1] = lds_v2u64(A[1].own);
+    }
+    auto draw = [&](const uint64_t t, const uint32_t colour) {
+        sweep_rng_set_time(g, t, colour);
+        return sweep_random4(g, colour ? site1 : site0);
+    };
     for (uint32_t sw = 0; sw < a.n_half / 2; ++sw) { // n_half is even: colour 0 then colour 1 of sweep t0 + sw
-        if (active) half_sweep(A[0], r);
-        barrier_begin();
-        sweep_rng_set_time(g, a.t0 + sw, 1u);
-        r = sweep_random4(g, site1);
-        barrier_end();
-        if (active) half_sweep(A[1], r);
-        barrier_begin();
-        sweep_rng_set_time(g, a.t0 + sw + 1, 0u);
-        r = sweep_random4(g, site0);
-        barrier_end();
+        if (active) half_sweep(A[0], r, 0, Sc[0]);
+        barrier_begin(0);
+        r = draw(a.t0 + sw, 1u);
+        barrier_end(0, sw & 1u);
+        if (active) half_sweep(A[1], r, 1, Sc[1]);
+        barrier_begin(1);
+        r = draw(a.t0 + sw + 1, 0u);
+        barrier_end(1, sw & 1u);
     }
     if (CLUSTER) cluster_barrier(); // nobody leaves while a neighbour may still read its shared memory
 
@@ -233,13 +321,14 @@ __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
 static size_t small_smem_bytes(int L, int Lz, int bond_bytes)
 {
     const size_t pw = (size_t)L * L / 2, nh = pw * Lz;
-    return 2 * nh * 8 + 6 * nh * bond_bytes + 2 * pw * bond_bytes;
+    const size_t threads = ((size_t)L * L * Lz / 4 + 31) / 32 * 32;
+    return 2 * nh * 8 + 24 * threads * bond_bytes + 4 * pw * 8 + 16; // spins, bonds, halo, bar
 }
 
 // Cluster size C (1, 2, 4, 8, 16; L % C == 0) for a lattice of side L: every slab must fit one CTA (at most 512 pairs =
 // threads, and the shared memory of one SM); among those the one with the smallest estimated half-sweep time -- warps per
-// sub-partition x ~300 clocks per pair, plus ~40 clocks for __syncthreads() or ~450 for the cluster barrier (measured:
-// L = 16 on one CTA 1.93 us, L = 32 on 8 CTAs 1.84 us).  0 if there is none.
+// sub-partition x ~300 clocks per pair, plus ~40 clocks for __syncthreads() or ~450 for the exchange between CTAs.  0 if
+// there is none.
 int small_cluster_size(int L, int n_replicas)
 {
     if (L < 4 || L % 4 || L > 64) return 0;
