@@ -27,21 +27,20 @@ class Scan:
             self.sims.append(binding.Sim(pt["L"], pt["p"], pt["T"], n_replicas=pt.get("n_replicas", 2),
                                          seed=pt.get("seed", 0), n_slots=pt.get("n_slots", 1),
                                          kernel=pt.get("kernel", "auto"), device=device))
-        # Which points share launches (measured on B200, 2000-sweep calls, us per sweep of ALL points):
-        #   L <= 16: every point alone on its stream -- AUTO runs SMALL (lattice in the shared memory of one CTA / cluster, one
-        #            launch per call): L = 16: 1.47 (16 points) / 2.00 (64) against 5.19 / 5.92 for the fused launches;
-        #   L = 32:  SMALL takes a 16-CTA cluster per point, so few run at once: 4.11 / 6.17 / 20.6 with 8 / 16 / 64 points
-        #            against 5.94 / 6.94 / 14.7 fused (ea_batch_*: one launch per colour for all points) -> fuse from 32 points;
+        # Which points share launches (measured on B200, 2000-sweep calls, us per sweep of ALL points): none, unless asked.
+        #   L <= 32: every point alone on its stream -- AUTO runs SMALL (lattice in the shared memory of one CTA / cluster, one
+        #            launch per call): L = 16: 0.89 (16 points) / 1.40 (64) against 5.19 / 5.99 for the fused launches
+        #            (ea_batch_*: one launch per colour for all points); L = 32: 2.9 / 4.3 / 7.2 / 14.3 / 27.3 with 8 / 16 / 32 /
+        #            64 / 128 points against - / 6.9 / 9.0 / 14.6 / 30.1 fused;
         #   L = 64:  streams of graph replays (10.2 for 8 points against 14 fused).
-        # fused=True / False overrides.
+        # fused=True fuses every group of one shape (L in 16, 32, 64); "auto" and False do not.
         self.batches, self._solo = [], list(self.sims)
         groups = {}
         for s in self.sims:
             if s.n_samples == binding.LANES and s.L in (16, 32, 64):
                 groups.setdefault((s.L, s.n_replicas), []).append(s)
         for (L, _), members in groups.items():
-            fuse = fused is True or (fused == "auto" and L == 32 and len(members) >= 32)
-            if fuse and len(members) > 1:
+            if fused is True and len(members) > 1:
                 self.batches.append(binding.Batch(members))
                 self._solo = [s for s in self._solo if s not in members]
 
