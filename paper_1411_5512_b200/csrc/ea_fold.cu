@@ -1,9 +1,8 @@
-// ea_fold.cu -- mixed multispin coding with M < 64 samples per word (III):
-// "one can simply reduce the number of samples to M = 2^m (m < 6) by storing 64/M spins from different positions
-// per sample in a multispin.  A simple way is to split the system into 64/M equal parts along one dimension and
-// assign spins at the same relative positions to the bits {i, i + M, i + 2M, ...} in the same multispin.  This
-// effectively makes it look and work like a smaller system with the caveat, that when coupling over the 'periodic
-// boundary' one has to rotate the bits of the multispin variable by M positions."
+// ea_fold.cu -- mixed multispin coding with M < 64 samples per word (III).  The paper's
+// recipe, restated: with M = 2^m < 64 samples, a word carries 64/M sites of every sample -- the lattice is cut into 64/M
+// equal parts along one dimension and the sites at the same relative position of each part share a word (bits i, i + M,
+// i + 2M, ... belong to sample i).  The sweep then runs on a lattice 64/M times smaller, except across the cut, where the
+// neighbouring word has to be rotated by M bits.
 //
 // Here: K = 64/M slabs along z, folded lattice L x L x Lz (Lz = L/K, even so that folded and physical colour agree);
 // bit j + M k of folded word (x, y, z') = sample j at physical site (x, y, z' + k Lz).  The +z neighbour of the top
