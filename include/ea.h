@@ -122,7 +122,7 @@ ea_status ea_get_time(const ea_sim *sim, uint64_t *t); /* completed sweeps since
 ea_status ea_set_time(ea_sim *sim, uint64_t t);
 ea_status ea_set_temperature(ea_sim *sim, double T);   /* recomputes the thresholds               */
 ea_status ea_get_thresholds(const ea_sim *sim, uint64_t thr[3]); /* thr[n_u], n_u = 0,1,2 (C-A4)  */
-ea_status ea_set_dynamics(ea_sim *sim, int dynamics);  /* ea_dynamics (not with n_samples < 64)                */
+ea_status ea_set_dynamics(ea_sim *sim, int dynamics);  /* ea_dynamics                                          */
 ea_status ea_get_dynamics(const ea_sim *sim, int *dynamics);
 ea_status ea_get_thresholds_heatbath(const ea_sim *sim, uint64_t thr[7]); /* thr[n_u], n_u = 0..6 (C-HB)     */
 ea_status ea_set_kernel(ea_sim *sim, int kernel);      /* EA_ERR_INVALID if not valid for this L  */

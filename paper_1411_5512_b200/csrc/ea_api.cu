@@ -463,8 +463,6 @@ ea_status ea_set_dynamics(ea_sim *sim, int dynamics)
 {
     if (!sim) return EA_ERR_INVALID;
     if (dynamics != EA_DYN_METROPOLIS && dynamics != EA_DYN_HEATBATH) EA_FAIL(sim, EA_ERR_INVALID, "unknown dynamics %d", dynamics);
-    if (dynamics == EA_DYN_HEATBATH && sim->n_samples < EA_LANES)
-        EA_FAIL(sim, EA_ERR_STATE, "heat bath is not available with n_samples < 64");
     if (dynamics != sim->dynamics) {
         DeviceGuard g(sim->device);
         destroy_graph(sim); // the captured launches are of the other rule's kernels

@@ -138,10 +138,26 @@ __device__ __forceinline__ uint64_t flip_word_masks(uint64_t s, uint64_t n1, uin
     return f;
 }
 
+// Heat bath (reading C-HB): flip with probability hb[n_u], n_u = 0..6 unsatisfied bonds, hb increasing in n_u.  With the
+// level masks m_k (bit set <=> that sample's number is below hb[k], nested: m_0 <= ... <= m_6 bitwise) the flip word is
+// m_{n_u} = OR_k (m_k & [n_u >= k]); n_u = d0 + 2 d1 + 4 d2 from the two full adders.
+__device__ __forceinline__ uint64_t flip_word_masks_heatbath(uint64_t s, uint64_t n1, uint64_t n2, uint64_t n3, uint64_t n4,
+                                                             uint64_t n5, uint64_t n6, uint64_t j1, uint64_t j2, uint64_t j3,
+                                                             uint64_t j4, uint64_t j5, uint64_t j6, const uint64_t (&m)[7])
+{
+    const uint64_t u1 = j1 ^ s ^ n1, u2 = j2 ^ s ^ n2, u3 = j3 ^ s ^ n3, u4 = j4 ^ s ^ n4, u5 = j5 ^ s ^ n5, u6 = j6 ^ s ^ n6;
+    const uint64_t sa = u1 ^ u2 ^ u3, ka = (u1 & u2) | (u3 & (u1 | u2));
+    const uint64_t sb = u4 ^ u5 ^ u6, kb = (u4 & u5) | (u6 & (u4 | u5));
+    const uint64_t d0 = sa ^ sb, c0 = sa & sb;
+    const uint64_t d1 = ka ^ kb ^ c0, d2 = (ka & kb) | (c0 & (ka | kb));
+    const uint64_t ge1 = d0 | d1 | d2, ge2 = d1 | d2, ge3 = d2 | (d1 & d0), ge4 = d2, ge5 = d2 & (d1 | d0), ge6 = d2 & d1;
+    return m[0] | (m[1] & ge1) | (m[2] & ge2) | (m[3] & ge3) | (m[4] & ge4) | (m[5] & ge5) | (m[6] & ge6);
+}
+
 // one thread = two x-adjacent folded words of one colour (L % 4 == 0)
 // MT = M as a compile-time constant (shifts and the slab loop unroll), or 0: taken from the arguments.
 // POW2: L is a power of two (index arithmetic by shifts).
-template <int MT, bool POW2, bool ALWAYS>
+template <int MT, bool POW2, bool ALWAYS, bool HB = false>
 __global__ void __launch_bounds__(256) k_sweep_fold(const FoldSweepArgs a)
 {
     const FoldGeom f = a.f;
@@ -198,8 +214,31 @@ __global__ void __launch_bounds__(256) k_sweep_fold(const FoldSweepArgs a)
     // two words are one pair of the stream contract C-A7)
     const uint64_t time = (a.d_time ? *a.d_time : a.t) + a.t_offset;
     const SweepRng g = make_sweep_rng(a.seed, time, (uint32_t)a.colour);
-    uint64_t m0a = 0, m1a = 0, m2a = 0, m0b = 0, m1b = 0, m2b = 0; // word 0 (a), word 1 (b)
     uint64_t glo = f.g_lo, ghi = f.g_hi;                           // the slab's group bits, shifted by M per slab
+    if (HB) {
+        uint64_t ma[7], mb[7]; // word 0 (a), word 1 (b)
+#pragma unroll
+        for (int l = 0; l < 7; ++l) ma[l] = mb[l] = a.th.hb_always[l] ? ~(uint64_t)0 : 0; // hb[l] == 2^32 (T = 0): certain
+        for (int kk = 0; kk < K; ++kk) {
+            const uint32_t site0 = (4 * k + s) + L * (y + L * (z + kk * Lz));
+            const uint4 r = sweep_random4(g, site0);
+#pragma unroll
+            for (int l = 0; l < 7; ++l) {
+                if (r.x < a.th.hb[l]) ma[l] |= glo;
+                if (r.y < a.th.hb[l]) ma[l] |= ghi;
+                if (r.z < a.th.hb[l]) mb[l] |= glo;
+                if (r.w < a.th.hb[l]) mb[l] |= ghi;
+            }
+            glo <<= M;
+            ghi <<= M;
+        }
+        ulonglong2 out;
+        out.x = own.x ^ flip_word_masks_heatbath(own.x, np0, nm0, Yp.x, Ym.x, Zp.x, Zm.x, jx.x, jm0, jy.x, by.x, jz.x, bz.x, ma);
+        out.y = own.y ^ flip_word_masks_heatbath(own.y, np1, nm1, Yp.y, Ym.y, Zp.y, Zm.y, jx.y, jm1, jy.y, by.y, jz.y, bz.y, mb);
+        *(ulonglong2 *)(a.own + i0) = out;
+        return;
+    }
+    uint64_t m0a = 0, m1a = 0, m2a = 0, m0b = 0, m1b = 0, m2b = 0; // word 0 (a), word 1 (b)
 #pragma unroll(MT ? (64 / (MT ? MT : 1) <= 8 ? 64 / (MT ? MT : 1) : 4) : 1)
     for (int kk = 0; kk < K; ++kk) {
         const uint32_t site0 = (4 * k + s) + L * (y + L * (z + kk * Lz));
@@ -319,7 +358,9 @@ cudaError_t launch_half_sweep_fold(ea_sim *s, int parity, uint64_t t, const uint
     a.th = s->th;
     const bool always = a.th.always[0] | a.th.always[1] | a.th.always[2];
     const unsigned grid = blocks_for(a.f.Nhf / 2, 256);
-    if (always || s->lat.log2L < 0) { // T = inf or L not a power of two: the generic kernel
+    if (s->dynamics == EA_DYN_HEATBATH) { // the generic kernel with seven level masks
+        k_sweep_fold<0, false, false, true><<<grid, 256, 0, st>>>(a);
+    } else if (always || s->lat.log2L < 0) { // T = inf or L not a power of two: the generic kernel
         if (always) k_sweep_fold<0, false, true><<<grid, 256, 0, st>>>(a);
         else k_sweep_fold<0, false, false><<<grid, 256, 0, st>>>(a);
     } else {

@@ -622,15 +622,21 @@ def _used(mask64, n):
     return [b for b in range(n) if (mask64 >> b) & 1]
 
 
-@pytest.mark.parametrize("L,M,n_rep,T,sweeps", [(8, 32, 2, 0.8, 40), (8, 16, 2, 2.0, 40), (16, 8, 2, 0.8, 40), (16, 32, 1, 0.8, 20),
-                                                 (16, 16, 1, float("inf"), 6), (32, 4, 2, 0.8, 36), (64, 2, 2, 2.0, 6),
-                                                 (12, 32, 2, 0.0, 20), (128, 32, 2, 0.8, 4), (128, 1, 1, 0.8, 4)])
-def test_folded_sim_is_the_used_lanes_of_the_64_sample_trajectory(L, M, n_rep, T, sweeps):
+@pytest.mark.parametrize("L,M,n_rep,T,sweeps,dyn", [
+    (8, 32, 2, 0.8, 40, "metropolis"), (8, 16, 2, 2.0, 40, "metropolis"), (16, 8, 2, 0.8, 40, "metropolis"),
+    (16, 32, 1, 0.8, 20, "metropolis"), (16, 16, 1, float("inf"), 6, "metropolis"), (32, 4, 2, 0.8, 36, "metropolis"),
+    (64, 2, 2, 2.0, 6, "metropolis"), (12, 32, 2, 0.0, 20, "metropolis"), (128, 32, 2, 0.8, 4, "metropolis"),
+    (128, 1, 1, 0.8, 4, "metropolis"),
+    (8, 32, 2, 0.8, 40, "heatbath"), (16, 8, 2, 2.0, 30, "heatbath"), (16, 16, 1, float("inf"), 6, "heatbath"),
+    (12, 32, 2, 0.0, 20, "heatbath"), (32, 4, 1, 1.1, 12, "heatbath"), (128, 32, 2, 0.8, 3, "heatbath")])
+def test_folded_sim_is_the_used_lanes_of_the_64_sample_trajectory(L, M, n_rep, T, sweeps, dyn):
     """A sim with n_samples = M < 64 stores 64/M z-slabs per word and rotates by M at the seam; by C-M its samples
     are lanes of the 64-sample definition, so the ORACLE AS IT STANDS (64 lanes, same seed) is the reference:
-    spin words and bond words masked to the used lanes, and every observable on the used lanes."""
+    spin words and bond words masked to the used lanes, and every observable on the used lanes.  Both update rules."""
     g = binding.Sim(L, 0.6, T, n_replicas=n_rep, seed=wl.seed_for(2, L + M), n_slots=1, n_samples=M)
     o = Oracle(L, 0.6, T, n_replicas=n_rep, seed=wl.seed_for(2, L + M), n_slots=1)
+    g.set_dynamics(dyn)
+    o.set_dynamics(dyn)
     assert g.kernel == binding.EA_KERNEL_FOLD
     mask = np.uint64(g.lane_mask)
     assert np.array_equal(g.get_bonds(), o.get_bonds() & mask)
@@ -671,8 +677,6 @@ def test_folded_sim_set_state_and_argument_errors():
     assert np.array_equal(g.get_spins(), spins & mask) and np.array_equal(g.get_bonds(), bonds & mask)
     g.sweep(5); o.sweep(5)
     assert np.array_equal(g.get_spins(), o.get_spins() & mask)
-    with pytest.raises(binding.EAError):
-        g.set_dynamics("heatbath")
     with pytest.raises(binding.EAError):
         g.kernel = "rows"
     for bad in ((10, 32, 2), (16, 3, 2), (16, 1, 2), (8, 8, 2), (16, 128, 2)):   # L % 4, M not 2^m, M < 2 replicas, L M / 64 odd, M > 64
