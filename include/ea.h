@@ -64,8 +64,8 @@ typedef enum {
     EA_KERNEL_ROWS_PERSISTENT = 6, /* ROWS with a grid barrier per colour, one launch per ea_sweep (L = 16, 32, 64);
                                      measured slower than the graph replays, never chosen by AUTO */
     EA_KERNEL_SMALL = 7   /* small lattices (L % 4 == 0, L <= 32): spins and bonds resident in the shared memory of one
-                             CTA (L <= 16) or of one thread-block cluster (L = 32: 16 CTAs, neighbouring planes read
-                             through distributed shared memory, cluster barrier per colour); one launch per ea_sweep.
+                             CTA (L <= 8) or of one thread-block cluster (L = 32: 16 CTAs; boundary planes pushed into
+                             the neighbouring CTA's shared memory, an mbarrier per colour); one launch per ea_sweep.
                              AUTO uses it for ea_sweep(n >= 2); shorter calls go as per-colour launches */
 } ea_kernel;
 

@@ -698,8 +698,8 @@ def test_rows_persistent_long_run_matches_the_graph_replays():
 
 
 def test_small_lattice_kernel_auto_choice_and_long_runs():
-    """SMALL (lattice resident in the shared memory of one CTA, or of one thread-block cluster with the neighbouring planes
-    read through distributed shared memory): AUTO picks it for L = 8, 16, 32; launches of 2, 3 and n sweeps (ea_sweep(1)
+    """SMALL (lattice resident in the shared memory of one CTA, or of one thread-block cluster with the boundary planes
+    pushed into the neighbouring CTA's shared memory): AUTO picks it for L = 8, 16, 32; launches of 2, 3 and n sweeps (ea_sweep(1)
     goes as per-colour launches) against the per-colour kernels over cfg1's, cfg2's and a longer horizon; both bond
     widths.  (The oracle follows the first sweeps in the every-kernel test and in the cfg1 / cfg2 tests.)"""
     for L, n_rep, n in ((8, 1, 1000), (16, 2, 3000), (32, 2, 3000), (32, 1, 500), (24, 2, 500)):
