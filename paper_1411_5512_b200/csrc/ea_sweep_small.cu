@@ -2,15 +2,16 @@
 // small lattices of the paper's scans (L = 8 .. 32: PAPER.md:134 and BASELINE configs 1-2), where a kernel launch
 // per colour costs far more than the half-sweep itself.
 //
-// Same update and the same stream contract as every other variant, hence bit-identical.  The lattice is cut into C
-// slabs of L x L x (L / C) sites along z, one CTA per slab:
-//   * C = 1 (L <= 16): one CTA, the colour barrier is __syncthreads();
-//   * C = 2 .. 16 (L = 32: 16 CTAs of 2 planes): one thread-block CLUSTER; a thread on a boundary plane PUSHES its new
-//     pair into the halo plane of the neighbouring CTA's shared memory (st.async through distributed shared memory) and the
-//     colour barrier is an mbarrier per CTA that counts its own warps and the bytes its two neighbours pushed -- no global
-//     memory traffic, no cluster-wide barrier and no fence wider than the CTA between sweeps (see PUSH below).
+// Same update and the same stream contract as every other variant, hence bit-identical.  The lattice is cut into
+// C = Cy x Cz blocks of L x (L / Cy) x (L / Cz) sites (whole x rows), one CTA per block:
+//   * C = 1 (L <= 8): one CTA, the colour barrier is __syncthreads();
+//   * C = 2 .. 16 (L = 32: 16 slabs of 2 planes; L = 20, 24: 4 x 4 blocks): one thread-block CLUSTER; a thread on a face of
+//     its block PUSHES its new pair into the halo of the neighbouring CTA's shared memory (st.async through distributed
+//     shared memory) and the colour barrier is an mbarrier per CTA that counts its own warps and the bytes its neighbours
+//     pushed -- no global memory traffic, no cluster-wide barrier and no fence wider than the CTA between sweeps (PUSH below).
 // Spins AND bond words live in shared memory; global memory is read once at the start and written once at the end.
 // A thread owns one pair of x-adjacent same-colour sites of each colour (one Philox block per pair and sweep, C-A7).
+#include <stdlib.h>
 #include <string.h>
 
 #include "ea_internal.h"
@@ -24,7 +25,8 @@ struct SmallArgs {
     uint64_t seed;
     uint64_t t0;         // first sweep index
     uint32_t n_half;     // half-sweeps to run
-    int L, Lz;           // side; planes per CTA (L / cluster size)
+    int L, Ly, Lz;       // side; rows and planes per CTA
+    int Cy, Cz;          // CTAs along y and z (Cy Cz = cluster size; rank = ry + Cy rz)
     Thresholds th;
 };
 
@@ -115,7 +117,8 @@ struct SmallAddr {
     uint32_t own, xa, xe, pm, pp, zm, zp;       // spins: own pair; the other colour's pair at the same place and the row's third
                                                 // other-colour word next to it; y -/+ and z -/+ pairs
     uint32_t bonds;                             // the thread's bond vectors of this colour
-    uint32_t push_lo, push_hi;                  // PUSH: where the own pair goes in the CTA below / above (shared::cluster addresses)
+    uint32_t push_zlo, push_zhi, push_ylo, push_yhi; // PUSH: where the own pair goes in the CTA below / above along z and y
+                                                // (shared::cluster addresses)
 };
 
 __device__ __forceinline__ void cluster_barrier()
@@ -125,14 +128,15 @@ __device__ __forceinline__ void cluster_barrier()
 }
 // (only at the start and the end of the kernel: see PUSH)
 
-// Shared memory of one CTA (nh = L L Lz / 2 words per colour of the slab, pw = L L / 2 words per colour and plane):
-//   spins  uint64 [2][nh]
+// Shared memory of one CTA (Ly x Lz rows of Lh = L / 2 words per colour; nh = Lh Ly Lz words per colour of the block):
+//   spins  uint64 [2][Lz][Ly][Lh]
 //   bonds  BondT  [2][12][n_threads] in vectors of 16 bytes: per colour and thread {jx, jx', jy, jy', jz, jz', bl, bl', by, by',
 //                 bz, bz'} = the forward bonds of the pair's two sites, the +x bonds of their left neighbours, the +y / +z bonds of
 //                 their y - 1 / z - 1 neighbours.  Every bond sits there twice (forward for one colour, backward for the other):
 //                 the addresses never change, so each thread keeps its own copy where one LDS.128 per four words fetches it.
-//   halo   uint64 [2][2][pw]   PUSH: the spin planes below / above the slab, both colours, as the neighbours pushed them
-//   bar    uint64 [2]          PUSH: one mbarrier per colour
+//   zhalo  uint64 [2][2][Ly][Lh]  PUSH: the faces below / above the block along z, both colours, as the neighbours pushed them
+//   yhalo  uint64 [2][2][Lz][Lh]  PUSH, Cy > 1 (YSPLIT): the same along y
+//   bar    uint64 [2]             PUSH: one mbarrier per colour
 //
 // PUSH (clusters): no cluster barrier in the sweep loop.  barrier.cluster.arrive.release / wait.acquire compile to
 // MEMBAR.ALL.GPU + UCGABAR + CCTL.IVALL (measured ~850 clocks per barrier on 8 CTAs, ~1240 on 16), and so does every other
@@ -145,34 +149,42 @@ __device__ __forceinline__ void cluster_barrier()
 // Measured (B200, us per half-sweep, L = 16 / 32): cluster barrier + remote loads 0.59 / 1.03; pushes 0.36 / 0.71.  Not
 // kept: cp.async.bulk of the whole plane by one thread (0.50 / 1.00: the copy starts only after a CTA-wide barrier), two
 // interleaved chains of row classes as in the L = 128 kernel (0.69 at L = 32: a unit's latency, not its issue slots, sets
-// the pace; the pushes cost ~2 clocks per 16-byte packet of the SM-to-SM network whoever overlaps them).
-template <typename BondT, bool ALWAYS, bool RARE, bool HB, bool CLUSTER>
+// the pace).  The number of pushed pairs does not matter either (see small_shape).
+template <typename BondT, bool ALWAYS, bool RARE, bool HB, bool CLUSTER, bool YSPLIT>
 __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
 {
     constexpr bool PUSH = CLUSTER;
     extern __shared__ __align__(16) unsigned char smem_small[];
-    const unsigned L = a.L, Lh = L / 2, Lz = a.Lz, hp = Lh / 2; // hp: pairs per row
-    const unsigned pw = L * Lh, nh = pw * Lz, Nh = pw * L;
-    const unsigned rank = CLUSTER ? cluster_ctarank() : 0, C = CLUSTER ? cluster_nctarank() : 1;
-    const unsigned z0 = rank * Lz;
-    uint64_t *spins_s = (uint64_t *)smem_small;
+    const unsigned L = a.L, Lh = L / 2, Ly = a.Ly, Lz = a.Lz, hp = Lh / 2; // hp: pairs per row
+    const unsigned Cy = a.Cy, Cz = a.Cz;
+    const unsigned pz = Ly * Lh, py = Lz * Lh;  // words per colour of one z face (a plane of the block) / one y face
+    const unsigned nh = pz * Lz, Nh = L * L * Lh;
+    const unsigned rank = CLUSTER ? cluster_ctarank() : 0;
+    const unsigned ry = rank % Cy, rz = rank / Cy, y0 = ry * Ly, z0 = rz * Lz;
+    const bool split_y = YSPLIT, split_z = PUSH && (!YSPLIT || Cz > 1); // YSPLIT: Cy > 1 (compiled out of the slab variant)
+    uint64_t *spins_s = (uint64_t *)smem_small;                // [2][Lz][Ly][Lh]
     const unsigned tid = threadIdx.x, nthr = blockDim.x;
     BondT *bonds_s = (BondT *)(spins_s + 2 * nh);
-    uint64_t *halo_s = (uint64_t *)(bonds_s + 24 * nthr);
-    uint64_t *bar_s = halo_s + 4 * pw;
+    uint64_t *zhalo_s = (uint64_t *)(bonds_s + 24 * nthr);     // [2 sides][2 colours][Ly][Lh]
+    uint64_t *yhalo_s = zhalo_s + 4 * pz;                      // [2 sides][2 colours][Lz][Lh]
+    uint64_t *bar_s = yhalo_s + 4 * py;
     const BondT *__restrict__ gb = (const BondT *)a.bonds;
 
-    // ---- prologue: the slab (contiguous in every colour / direction plane of the global arrays) ------------------
+    // ---- prologue: the block (whole x rows) and the four faces around it ------------------------------------------
     for (unsigned v = tid; v < 2 * nh; v += nthr) {
-        const unsigned c = v / nh, i = v % nh;
-        spins_s[v] = a.spins[(size_t)c * Nh + (size_t)pw * z0 + i];
+        const unsigned c = v / nh, i = v % nh, x = i % Lh, yl = (i / Lh) % Ly, zl = i / pz;
+        spins_s[v] = a.spins[(size_t)c * Nh + (size_t)Lh * ((y0 + yl) + (size_t)L * (z0 + zl)) + x];
     }
-
     if (PUSH) {
-        for (unsigned v = tid; v < 4 * pw; v += nthr) {
-            const unsigned side = v / (2 * pw), c = (v / pw) & 1u, i = v % pw;
+        for (unsigned v = tid; v < 4 * pz; v += nthr) {
+            const unsigned side = v / (2 * pz), c = (v / pz) & 1u, i = v % pz, x = i % Lh, yl = i / Lh;
             const unsigned zh = side ? (z0 + Lz) % L : (z0 + L - 1) % L;
-            halo_s[v] = a.spins[(size_t)c * Nh + (size_t)pw * zh + i];
+            zhalo_s[v] = a.spins[(size_t)c * Nh + (size_t)Lh * ((y0 + yl) + (size_t)L * zh) + x];
+        }
+        for (unsigned v = tid; v < 4 * py; v += nthr) {
+            const unsigned side = v / (2 * py), c = (v / py) & 1u, i = v % py, x = i % Lh, zl = i / Lh;
+            const unsigned yh = side ? (y0 + Ly) % L : (y0 + L - 1) % L;
+            yhalo_s[v] = a.spins[(size_t)c * Nh + (size_t)Lh * (yh + (size_t)L * (z0 + zl)) + x];
         }
         if (tid == 0) {
             mbar_init(small_smem_u32(bar_s), nthr / 32);
@@ -181,24 +193,28 @@ __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
         }
     }
 
-    // ---- the thread's pair: (p, y, zl) -> compact words 2p, 2p + 1 of row (y, zl), both colours -------------------
-    const unsigned n_pairs = hp * L * Lz;
+    // ---- the thread's pair: (p, yl, zl) -> compact words 2p, 2p + 1 of row (yl, zl) of the block, both colours -----
+    const unsigned n_pairs = hp * Ly * Lz;
     const bool active = tid < n_pairs;
-    const unsigned p = tid % hp, y = (tid / hp) % L, zl = active ? tid / (hp * L) : 0;
-    const unsigned ym = y == 0 ? L - 1 : y - 1, yp = y + 1 == L ? 0 : y + 1;
-    const unsigned i0 = Lh * (y + L * zl) + 2 * p;          // own words (and the other colour's words of the same position)
-    const unsigned rowb = Lh * (y + L * zl);
-    const unsigned i_ym = Lh * (ym + L * zl) + 2 * p, i_yp = Lh * (yp + L * zl) + 2 * p;
-    // z neighbours: inside the slab, or the facing plane of the neighbouring CTA (C = 1: the slab wraps onto itself)
-    const bool lo_edge = zl == 0, hi_edge = zl + 1 == Lz;
-    const unsigned i_zm = Lh * (y + L * (lo_edge ? Lz - 1 : zl - 1)) + 2 * p;
-    const unsigned i_zp = Lh * (y + L * (hi_edge ? 0 : zl + 1)) + 2 * p;
+    const unsigned p = tid % hp, yl = (tid / hp) % Ly, zl = active ? tid / (hp * Ly) : 0;
+    const unsigned y = y0 + yl, zg = z0 + zl;                       // global row
+    const unsigned ym = y == 0 ? L - 1 : y - 1;
+    const unsigned rowb = Lh * (yl + Ly * zl), i0 = rowb + 2 * p;   // own words (and the other colour's words of the same position)
+    // y / z neighbours: inside the block, or the facing halo (the neighbouring CTA's face); an unsplit direction wraps
+    const bool ylo = yl == 0, yhi = yl + 1 == Ly, zlo = zl == 0, zhi = zl + 1 == Lz;
+    const unsigned i_ym = Lh * ((ylo ? Ly - 1 : yl - 1) + Ly * zl) + 2 * p, i_yp = Lh * ((yhi ? 0 : yl + 1) + Ly * zl) + 2 * p;
+    const unsigned i_zm = Lh * (yl + Ly * (zlo ? Lz - 1 : zl - 1)) + 2 * p, i_zp = Lh * (yl + Ly * (zhi ? 0 : zl + 1)) + 2 * p;
+    const unsigned i_zf = Lh * yl + 2 * p, i_yf = Lh * zl + 2 * p;  // the pair inside a z face / a y face
     const uint32_t spins_a = small_smem_u32(spins_s);
-    const uint32_t halo_a = small_smem_u32(halo_s), bar_a = small_smem_u32(bar_s);
-    const uint32_t halo_below = PUSH ? mapa_u32(halo_a, (rank + C - 1) % C) : 0, halo_above = PUSH ? mapa_u32(halo_a, (rank + 1) % C) : 0;
-    const uint32_t bar_below = PUSH ? mapa_u32(bar_a, (rank + C - 1) % C) : 0, bar_above = PUSH ? mapa_u32(bar_a, (rank + 1) % C) : 0;
-    const unsigned i_pl = Lh * y + 2 * p; // the pair inside its plane
-    const unsigned zg = z0 + zl;
+    const uint32_t zhalo_a = small_smem_u32(zhalo_s), yhalo_a = small_smem_u32(yhalo_s), bar_a = small_smem_u32(bar_s);
+    // the four neighbouring CTAs of the cluster (rank = ry + Cy rz)
+    const unsigned r_zlo = ry + Cy * ((rz + Cz - 1) % Cz), r_zhi = ry + Cy * ((rz + 1) % Cz);
+    const unsigned r_ylo = (ry + Cy - 1) % Cy + Cy * rz, r_yhi = (ry + 1) % Cy + Cy * rz;
+    const uint32_t zhalo_zlo = PUSH ? mapa_u32(zhalo_a, r_zlo) : 0, zhalo_zhi = PUSH ? mapa_u32(zhalo_a, r_zhi) : 0;
+    const uint32_t yhalo_ylo = PUSH ? mapa_u32(yhalo_a, r_ylo) : 0, yhalo_yhi = PUSH ? mapa_u32(yhalo_a, r_yhi) : 0;
+    const uint32_t bar_zlo = PUSH ? mapa_u32(bar_a, r_zlo) : 0, bar_zhi = PUSH ? mapa_u32(bar_a, r_zhi) : 0;
+    const uint32_t bar_ylo = PUSH ? mapa_u32(bar_a, r_ylo) : 0, bar_yhi = PUSH ? mapa_u32(bar_a, r_yhi) : 0;
+    const bool push_zlo = split_z && zlo, push_zhi = split_z && zhi, push_ylo = split_y && ylo, push_yhi = split_y && yhi;
     const uint32_t site_row = L * (y + L * zg);
 
     // per colour c: x-phase S = (c ^ y ^ z) & 1; the three other-colour words of the row next to the pair are compact
@@ -216,12 +232,14 @@ __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
         A[c].own = spins_a + (own_w + i0) * 8;
         A[c].xa = spins_a + (oth_w + i0) * 8;
         A[c].xe = spins_a + (oth_w + rowb + (Sc[c] ? q2 : q0)) * 8;
-        A[c].pm = spins_a + (oth_w + i_ym) * 8;
-        A[c].pp = spins_a + (oth_w + i_yp) * 8;
-        A[c].zm = PUSH && lo_edge ? halo_a + ((1 - c) * pw + i_pl) * 8 : spins_a + (oth_w + i_zm) * 8;
-        A[c].zp = PUSH && hi_edge ? halo_a + ((2 + 1 - c) * pw + i_pl) * 8 : spins_a + (oth_w + i_zp) * 8;
-        A[c].push_lo = halo_below + ((2 + c) * pw + i_pl) * 8; // the slab's first plane is the plane ABOVE the CTA below
-        A[c].push_hi = halo_above + (c * pw + i_pl) * 8;
+        A[c].pm = push_ylo ? yhalo_a + ((1 - c) * py + i_yf) * 8 : spins_a + (oth_w + i_ym) * 8;
+        A[c].pp = push_yhi ? yhalo_a + ((2 + 1 - c) * py + i_yf) * 8 : spins_a + (oth_w + i_yp) * 8;
+        A[c].zm = push_zlo ? zhalo_a + ((1 - c) * pz + i_zf) * 8 : spins_a + (oth_w + i_zm) * 8;
+        A[c].zp = push_zhi ? zhalo_a + ((2 + 1 - c) * pz + i_zf) * 8 : spins_a + (oth_w + i_zp) * 8;
+        A[c].push_zlo = zhalo_zlo + ((2 + c) * pz + i_zf) * 8; // the block's first plane is the face ABOVE the CTA below
+        A[c].push_zhi = zhalo_zhi + (c * pz + i_zf) * 8;
+        A[c].push_ylo = yhalo_ylo + ((2 + c) * py + i_yf) * 8;
+        A[c].push_yhi = yhalo_yhi + (c * py + i_yf) * 8;
         A[c].bonds = bonds_a + c * (12 / VEC) * bond_stride + 16 * tid;
         if (active) { // the thread's copy of its bonds, straight from the global arrays [2][3][Nh]
             const size_t g_row = (size_t)Lh * (y + (size_t)L * zg), g_ym = (size_t)Lh * (ym + (size_t)L * zg);
@@ -263,13 +281,15 @@ __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
         sts_v2u64(ad.own, out);
         own_r[c] = out;
         if (PUSH) {
-            if (lo_edge) st_async_v2u64(ad.push_lo, out, bar_below + 8 * c);
-            if (hi_edge) st_async_v2u64(ad.push_hi, out, bar_above + 8 * c);
+            if (push_zlo) st_async_v2u64(ad.push_zlo, out, bar_zlo + 8 * c);
+            if (push_zhi) st_async_v2u64(ad.push_zhi, out, bar_zhi + 8 * c);
+            if (push_ylo) st_async_v2u64(ad.push_ylo, out, bar_ylo + 8 * c);
+            if (push_yhi) st_async_v2u64(ad.push_yhi, out, bar_yhi + 8 * c);
         }
     };
 
     // end of a half-sweep: arrive at the colour barrier, draw the next random numbers meanwhile, wait
-    const uint32_t tx_bytes = 2 * pw * 8; // what the two neighbours push per half-sweep
+    const uint32_t tx_bytes = (split_z ? 2 * pz * 8 : 0) + (split_y ? 2 * py * 8 : 0); // what the neighbours push per half-sweep
     auto barrier_begin = [&](const unsigned c) {
         if (PUSH) {
             __syncwarp();
@@ -308,48 +328,66 @@ __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
     }
     if (CLUSTER) cluster_barrier(); // nobody leaves while a neighbour may still read its shared memory
 
-    // ---- epilogue: the slab back to global ---------------------------------------------------------------------------
+    // ---- epilogue: the block back to global ---------------------------------------------------------------------------
     for (unsigned v = tid; v < 2 * nh; v += nthr) {
-        const unsigned c = v / nh, i = v % nh;
-        a.spins[(size_t)c * Nh + (size_t)pw * z0 + i] = spins_s[v];
+        const unsigned c = v / nh, i = v % nh, x = i % Lh, yl_ = (i / Lh) % Ly, zl_ = i / pz;
+        a.spins[(size_t)c * Nh + (size_t)Lh * ((y0 + yl_) + (size_t)L * (z0 + zl_)) + x] = spins_s[v];
     }
 }
 
 // ---------------------------------------------------------------------------------------------
 // Host side
 // ---------------------------------------------------------------------------------------------
-static size_t small_smem_bytes(int L, int Lz, int bond_bytes)
+struct SmallShape {
+    int Cy, Cz;   // CTAs along y and z; 0: no valid shape
+    int C() const { return Cy * Cz; }
+};
+
+static size_t small_smem_bytes(int L, int Ly, int Lz, int bond_bytes)
 {
-    const size_t pw = (size_t)L * L / 2, nh = pw * Lz;
-    const size_t threads = ((size_t)L * L * Lz / 4 + 31) / 32 * 32;
-    return 2 * nh * 8 + 24 * threads * bond_bytes + 4 * pw * 8 + 16; // spins, bonds, halo, bar
+    const size_t Lh = L / 2, nh = Lh * Ly * Lz, pz = Ly * Lh, py = Lz * Lh;
+    const size_t threads = ((size_t)(L / 4) * Ly * Lz + 31) / 32 * 32;
+    return 2 * nh * 8 + 24 * threads * bond_bytes + 4 * pz * 8 + 4 * py * 8 + 16; // spins, bonds, z and y halos, bar
 }
 
-// Cluster size C (1, 2, 4, 8, 16; L % C == 0) for a lattice of side L: every slab must fit one CTA (at most 512 pairs =
-// threads, and the shared memory of one SM); among those the one with the smallest estimated half-sweep time -- warps per
-// sub-partition x ~300 clocks per pair, plus ~40 clocks for __syncthreads() or ~450 for the exchange between CTAs.  0 if
-// there is none.
-int small_cluster_size(int L, int n_replicas)
+// The cluster (Cy x Cz CTAs, 1 .. 16, blocks of L x L/Cy x L/Cz sites) for a lattice of side L: every block must fit one
+// CTA (at most 512 pairs = threads, and the shared memory of one SM); among those the one with the smallest estimated
+// half-sweep time -- warps per sub-partition x ~300 clocks per pair, plus ~40 clocks for __syncthreads() or ~450 for the
+// exchange between CTAs (measured: whatever the number of pushed pairs -- L = 32 as 1 x 16, 2 x 8, 4 x 4 blocks: 0.72 / 0.75 /
+// 0.76 us; the y split costs a little for its extra predicated pushes).  What the y split buys is sixteen CTAs for sides
+// that are no power of two (L = 20: 0.59 -> 0.38 us, L = 24: 0.66 -> 0.52).  Cy = 0 if there is none.
+static SmallShape small_shape(int L, int n_replicas)
 {
-    if (L < 4 || L % 4 || L > 64) return 0;
-    const int bond_bytes = n_replicas == 2 ? 4 : 8;
-    int best = 0;
+    SmallShape best = {0, 0};
+    if (L < 4 || L % 4 || L > 64) return best;
+    static const int forced_cy = [] { const char *e = getenv("EA_SMALL_CY"); return e ? atoi(e) : 0; }();
+    static const int forced_cz = [] { const char *e = getenv("EA_SMALL_CZ"); return e ? atoi(e) : 0; }();
+    const int bond_bytes = n_replicas == 2 ? 4 : 8, hp = L / 4;
     long best_cost = 0;
-    for (int C = 1; C <= 16; C *= 2) {
-        if (L % C) continue;
-        const int Lz = L / C;
-        const long pairs = (long)L * L * Lz / 4;
-        if (pairs > 512 || small_smem_bytes(L, Lz, bond_bytes) > 200 * 1024) continue;
-        const long cost = (pairs + 127) / 128 * 300 + (C > 1 ? 450 : 40);
-        if (!best || cost < best_cost) { best = C; best_cost = cost; }
-    }
+    for (int C = 1; C <= 16; C *= 2)
+        for (int Cy = 1; Cy <= C; Cy *= 2) {
+            const int Cz = C / Cy;
+            if (L % Cy || L % Cz) continue;
+            if (forced_cy && forced_cz && (Cy != forced_cy || Cz != forced_cz)) continue;
+            const int Ly = L / Cy, Lz = L / Cz;
+            const long pairs = (long)hp * Ly * Lz;
+            if (pairs > 512 || small_smem_bytes(L, Ly, Lz, bond_bytes) > 200 * 1024) continue;
+            const long cost = (pairs + 127) / 128 * 300 + (Cy * Cz == 1 ? 40 : Cy == 1 ? 450 : 510);
+            if (!best.Cy || cost < best_cost) { best.Cy = Cy; best.Cz = Cz; best_cost = cost; } // ties: the smaller cluster
+        }
     return best;
 }
 
-template <typename BondT, bool ALWAYS, bool RARE, bool HB, bool CLUSTER>
+int small_cluster_size(int L, int n_replicas)
+{
+    const SmallShape sh = small_shape(L, n_replicas);
+    return sh.Cy ? sh.C() : 0;
+}
+
+template <typename BondT, bool ALWAYS, bool RARE, bool HB, bool CLUSTER, bool YSPLIT>
 static cudaError_t launch_small_kernel(const SmallArgs &a, int C, unsigned threads, size_t smem, cudaStream_t st)
 {
-    auto kern = k_sweep_small<BondT, ALWAYS, RARE, HB, CLUSTER>;
+    auto kern = k_sweep_small<BondT, ALWAYS, RARE, HB, CLUSTER, YSPLIT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     if (C > 8 && (e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1)) != cudaSuccess) return e;
@@ -369,34 +407,36 @@ static cudaError_t launch_small_kernel(const SmallArgs &a, int C, unsigned threa
     return cudaLaunchKernelEx(&cfg, kern, a);
 }
 
-template <typename BondT, bool CLUSTER>
+template <typename BondT, bool CLUSTER, bool YSPLIT>
 static cudaError_t launch_small_typed(ea_sim *s, const SmallArgs &a, int C, unsigned threads, size_t smem, cudaStream_t st)
 {
     const Thresholds &th = s->th;
-    if (s->dynamics == EA_DYN_HEATBATH) return launch_small_kernel<BondT, false, false, true, CLUSTER>(a, C, threads, smem, st);
+    if (s->dynamics == EA_DYN_HEATBATH) return launch_small_kernel<BondT, false, false, true, CLUSTER, YSPLIT>(a, C, threads, smem, st);
     const bool always = th.always[0] | th.always[1] | th.always[2];
     const bool rare = !always && th.thr[2] < 0x04000000u; // as in the persistent L = 128 kernel
-    return always ? launch_small_kernel<BondT, true, false, false, CLUSTER>(a, C, threads, smem, st)
-           : rare ? launch_small_kernel<BondT, false, true, false, CLUSTER>(a, C, threads, smem, st)
-                  : launch_small_kernel<BondT, false, false, false, CLUSTER>(a, C, threads, smem, st);
+    return always ? launch_small_kernel<BondT, true, false, false, CLUSTER, YSPLIT>(a, C, threads, smem, st)
+           : rare ? launch_small_kernel<BondT, false, true, false, CLUSTER, YSPLIT>(a, C, threads, smem, st)
+                  : launch_small_kernel<BondT, false, false, false, CLUSTER, YSPLIT>(a, C, threads, smem, st);
 }
 
 bool small_supported(const ea_sim *s, std::string *why)
 {
     auto no = [&](const char *msg) { if (why) *why = msg; return false; };
-    const int C = small_cluster_size(s->lat.L, s->n_replicas);
-    if (!C) return no("small-lattice kernel: L must be a multiple of 4 whose slabs fit one thread-block cluster (L <= 32)");
+    const SmallShape sh = small_shape(s->lat.L, s->n_replicas);
+    const int C = sh.Cy ? sh.C() : 0;
+    if (!C) return no("small-lattice kernel: L must be a multiple of 4 whose blocks fit one thread-block cluster (L <= 32)");
+    const int Ly = s->lat.L / sh.Cy, Lz = s->lat.L / sh.Cz;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) return no("small-lattice kernel: cudaGetDeviceProperties failed");
     if (prop.major < 9 && C > 1) return no("small-lattice kernel: the device has no thread-block clusters");
-    const size_t smem = small_smem_bytes(s->lat.L, s->lat.L / C, s->bond_bytes());
+    const size_t smem = small_smem_bytes(s->lat.L, Ly, Lz, s->bond_bytes());
     if (prop.sharedMemPerBlockOptin < smem) return no("small-lattice kernel: the device has too little shared memory per CTA");
     if (C > 1) { // can the device co-schedule one cluster of this shape at all (MIG slices, small parts)?
-        auto kern = k_sweep_small<uint32_t, false, true, false, true>;
+        auto kern = k_sweep_small<uint32_t, false, true, false, true, false>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
             (C > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess))
             return no("small-lattice kernel: the device rejects the cluster configuration");
-        const unsigned pairs = (unsigned)((size_t)s->lat.L * s->lat.L * (s->lat.L / C) / 4);
+        const unsigned pairs = (unsigned)((size_t)(s->lat.L / 4) * Ly * Lz);
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof(cfg));
         cfg.gridDim = dim3((unsigned)C);
@@ -420,8 +460,10 @@ bool small_supported(const ea_sim *s, std::string *why)
 // n sweeps starting at sweep index t0, one launch.  Asynchronous.
 cudaError_t launch_sweeps_small(ea_sim *s, uint64_t t0, uint32_t n, cudaStream_t st)
 {
-    const int L = s->lat.L, C = small_cluster_size(L, s->n_replicas);
-    if (!C) return cudaErrorInvalidConfiguration;
+    const int L = s->lat.L;
+    const SmallShape sh = small_shape(L, s->n_replicas);
+    if (!sh.Cy) return cudaErrorInvalidConfiguration;
+    const int C = sh.C();
     SmallArgs a;
     a.spins = s->spins;
     a.bonds = s->bonds;
@@ -429,17 +471,23 @@ cudaError_t launch_sweeps_small(ea_sim *s, uint64_t t0, uint32_t n, cudaStream_t
     a.t0 = t0;
     a.n_half = 2 * n;
     a.L = L;
-    a.Lz = L / C;
+    a.Ly = L / sh.Cy;
+    a.Lz = L / sh.Cz;
+    a.Cy = sh.Cy;
+    a.Cz = sh.Cz;
     a.th = s->th;
-    const unsigned pairs = (unsigned)((size_t)L * L * a.Lz / 4), threads = (pairs + 31) / 32 * 32;
-    const size_t smem = small_smem_bytes(L, a.Lz, s->bond_bytes());
+    const unsigned pairs = (unsigned)((size_t)(L / 4) * a.Ly * a.Lz), threads = (pairs + 31) / 32 * 32;
+    const size_t smem = small_smem_bytes(L, a.Ly, a.Lz, s->bond_bytes());
     cudaError_t e;
-    if (C > 1)
-        e = s->n_replicas == 2 ? launch_small_typed<uint32_t, true>(s, a, C, threads, smem, st)
-                               : launch_small_typed<uint64_t, true>(s, a, C, threads, smem, st);
+    if (sh.Cy > 1)
+        e = s->n_replicas == 2 ? launch_small_typed<uint32_t, true, true>(s, a, C, threads, smem, st)
+                               : launch_small_typed<uint64_t, true, true>(s, a, C, threads, smem, st);
+    else if (C > 1)
+        e = s->n_replicas == 2 ? launch_small_typed<uint32_t, true, false>(s, a, C, threads, smem, st)
+                               : launch_small_typed<uint64_t, true, false>(s, a, C, threads, smem, st);
     else
-        e = s->n_replicas == 2 ? launch_small_typed<uint32_t, false>(s, a, C, threads, smem, st)
-                               : launch_small_typed<uint64_t, false>(s, a, C, threads, smem, st);
+        e = s->n_replicas == 2 ? launch_small_typed<uint32_t, false, false>(s, a, C, threads, smem, st)
+                               : launch_small_typed<uint64_t, false, false>(s, a, C, threads, smem, st);
     if (e == cudaSuccess) s->count_launch();
     return e;
 }

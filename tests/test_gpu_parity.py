@@ -702,7 +702,7 @@ def test_small_lattice_kernel_auto_choice_and_long_runs():
     pushed into the neighbouring CTA's shared memory): AUTO picks it for L = 8, 16, 32; launches of 2, 3 and n sweeps (ea_sweep(1)
     goes as per-colour launches) against the per-colour kernels over cfg1's, cfg2's and a longer horizon; both bond
     widths.  (The oracle follows the first sweeps in the every-kernel test and in the cfg1 / cfg2 tests.)"""
-    for L, n_rep, n in ((8, 1, 1000), (16, 2, 3000), (32, 2, 3000), (32, 1, 500), (24, 2, 500)):
+    for L, n_rep, n in ((8, 1, 1000), (16, 2, 3000), (32, 2, 3000), (32, 1, 500), (24, 2, 500), (20, 1, 500)):
         ref = "rows" if L in (16, 32) else "vec2"
         a = binding.Sim(L, 0.5, 0.8, n_replicas=n_rep, seed=wl.seed_for(2, L), n_slots=0, kernel=ref)
         b = binding.Sim(L, 0.5, 0.8, n_replicas=n_rep, seed=wl.seed_for(2, L), n_slots=0)
