@@ -262,7 +262,7 @@ __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
     // the thread's own pairs stay in registers between the sweeps (nobody else writes them); shared memory holds the copy
     // the neighbours read
     ulonglong2 own_r[2];
-    auto half_sweep = [&](const SmallAddr &ad, const uint4 r, const unsigned c, const bool S) {
+    auto half_sweep = [&](const SmallAddr &ad, const uint4 r, const unsigned c, const bool S, const BondT (&j)[12]) {
         // the row's other-colour words next to the pair: compact q0, q0 + 1, q0 + 2 with q0 = 2p - 1 + S
         const ulonglong2 Xa = lds_v2u64(ad.xa);
         const uint64_t Xe = lds_u64(ad.xe);
@@ -271,8 +271,6 @@ __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
         const uint64_t A2 = S ? Xa.y : Xe, B2 = S ? Xe : Xa.x;
         const ulonglong2 own = own_r[c], Pm = lds_v2u64(ad.pm), Pp = lds_v2u64(ad.pp);
         const ulonglong2 Zm = lds_v2u64(ad.zm), Zp = lds_v2u64(ad.zp);
-        BondT j[12];
-        lds_bonds12(ad.bonds, bond_stride, j);
         const BondT xA1 = j[0], xB1 = j[1], jyA = j[2], jyB = j[3], jzA = j[4], jzB = j[5], xA2 = j[6], xB2 = j[7], byA = j[8],
                     byB = j[9], bzA = j[10], bzB = j[11];
         ulonglong2 out;
@@ -312,18 +310,25 @@ __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
         own_r[0] = lds_v2u64(A[0].own);
         own_r[1] = lds_v2u64(A[1].own);
     }
+    // The bond words do not depend on the exchange: those of the next half-sweep are fetched while the barrier completes, so
+    // that only the spin loads queue on the load pipe when all warps start the half-sweep together (a trace showed ~600 clocks
+    // from the first load to the last operand at L = 32, against ~500 of logic).
+    BondT j[12];
+    lds_bonds12(A[0].bonds, bond_stride, j);
     auto draw = [&](const uint64_t t, const uint32_t colour) {
         sweep_rng_set_time(g, t, colour);
         return sweep_random4(g, colour ? site1 : site0);
     };
     for (uint32_t sw = 0; sw < a.n_half / 2; ++sw) { // n_half is even: colour 0 then colour 1 of sweep t0 + sw
-        if (active) half_sweep(A[0], r, 0, Sc[0]);
+        if (active) half_sweep(A[0], r, 0, Sc[0], j);
         barrier_begin(0);
         r = draw(a.t0 + sw, 1u);
+        lds_bonds12(A[1].bonds, bond_stride, j);
         barrier_end(0, sw & 1u);
-        if (active) half_sweep(A[1], r, 1, Sc[1]);
+        if (active) half_sweep(A[1], r, 1, Sc[1], j);
         barrier_begin(1);
         r = draw(a.t0 + sw + 1, 0u);
+        lds_bonds12(A[0].bonds, bond_stride, j);
         barrier_end(1, sw & 1u);
     }
     if (CLUSTER) cluster_barrier(); // nobody leaves while a neighbour may still read its shared memory
