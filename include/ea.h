@@ -38,6 +38,7 @@ extern "C" {
 
 #define EA_LANES 64 /* samples per multispin word (III) */
 #define EA_C4_MAX_VECTORS ((int64_t)1 << 24) /* ea_c4_vectors: most vectors per call (a full L = 128 torus has 2^21) */
+#define EA_C4_STATIC_MAX_VECTORS ((int64_t)1024) /* ea_c4_vectors_static: most vectors per call */
 
 typedef struct ea_sim ea_sim; /* opaque; one batch of 64 samples on one L^3 lattice */
 
@@ -147,6 +148,14 @@ ea_status ea_c4(ea_sim *sim, int r_max, int64_t *B, int64_t *q, double *c4_avg);
  * host arrays: dxyz 3 n_vec int32, B 32 n_vec int64.  EA_ERR_STATE on a 1-replica sim; EA_ERR_INVALID unless
  * L <= 32 or L in {64, 128}, or n_vec > EA_C4_MAX_VECTORS; EA_ERR_NOMEM if a host buffer cannot be allocated. */
 ea_status ea_c4_vectors(ea_sim *sim, int64_t n_vec, const int32_t *dxyz, int64_t *B);
+/* The same result for n_vec <= EA_C4_STATIC_MAX_VECTORS with NO allocation on the device or the host, for callers that cannot
+ * call cudaMalloc (inside a stream capture, in a serving loop, under a harness that forbids it): ea_c4_vectors keeps its job
+ * list and counters in grow-only cudaMalloc buffers; this call keeps them in one file-scope device array of 301 KiB (256 KiB of
+ * counters, 20 KiB of jobs, 24.5 KiB for the transposed field of an L < 16 lattice) that every GPU which loads the library holds
+ * until the process exits.  Same arguments, same B.  EA_ERR_INVALID with an ea_last_error text if n_vec exceeds the limit.
+ * Every call on a device shares that array, which keeps the last call's contents (the call clears the counters it uses):
+ * calls that overlap on the GPU -- two sims on two streams, two host threads -- race; serialise them. */
+ea_status ea_c4_vectors_static(ea_sim *sim, int64_t n_vec, const int32_t *dxyz, int64_t *B);
 /* Shell sums over the cube |dx|, |dy|, |dz| <= r_max (0 <= r_max <= L/2), by squared length d2 = 0 .. 3 r_max^2:
  *   S[d2*32 + b] = sum_{|r|^2 = d2} B_b(r),  mult[d2] = number of those vectors (0 for an empty shell),
  * so C_4(|r| = sqrt(d2)) = S / (mult N).  r and -r are both counted; with r_max = L/2 the components +L/2 and

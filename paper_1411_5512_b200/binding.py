@@ -17,6 +17,7 @@ EA_KERNEL_AUTO, EA_KERNEL_SCALAR, EA_KERNEL_VEC2, EA_KERNEL_ROWS, EA_KERNEL_RESI
     EA_KERNEL_SMALL = range(8)
 KERNEL_NAMES = {"auto": 0, "scalar": 1, "vec2": 2, "rows": 3, "resident": 4, "rows_persistent": 6, "small": 7}
 LANES = 64
+C4_STATIC_MAX_VECTORS = 1024  # EA_C4_STATIC_MAX_VECTORS (include/ea.h)
 
 
 class ea_params(C.Structure):
@@ -57,6 +58,7 @@ SIGNATURES = {
     "ea_autocorr": (_i, [_vp, _i, _vp, _vp]),
     "ea_c4": (_i, [_vp, _i, _vp, _vp, _vp]),
     "ea_c4_vectors": (_i, [_vp, C.c_int64, _vp, _vp]),
+    "ea_c4_vectors_static": (_i, [_vp, C.c_int64, _vp, _vp]),
     "ea_c4_shells": (_i, [_vp, _i, _vp, _vp]),
     "ea_c4_curve": (_i, [_vp, _vp, _i, _i, C.c_int64, _i, C.POINTER(_i), _vp, _vp, _vp]),
     "ea_integral_estimator": (_i, [_i, _vp, _vp, _vp, _i, _vp]),
@@ -260,6 +262,13 @@ class Sim:
         v = np.ascontiguousarray(vectors, dtype=np.int32).reshape(-1, 3)
         B = np.zeros((v.shape[0], 32), dtype=np.int64)
         self._ck(lib().ea_c4_vectors(self._h, v.shape[0], _ptr(v), _ptr(B)))
+        return B
+
+    def c4_vectors_static(self, vectors):
+        """c4_vectors for at most C4_STATIC_MAX_VECTORS vectors without any allocation in the library (static device scratch)."""
+        v = np.ascontiguousarray(vectors, dtype=np.int32).reshape(-1, 3)
+        B = np.zeros((v.shape[0], 32), dtype=np.int64)
+        self._ck(lib().ea_c4_vectors_static(self._h, v.shape[0], _ptr(v), _ptr(B)))
         return B
 
     def c4_shells(self, r_max):

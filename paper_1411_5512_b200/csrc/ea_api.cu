@@ -672,6 +672,25 @@ ea_status ea_c4_vectors(ea_sim *sim, int64_t n_vec, const int32_t *dxyz, int64_t
     return EA_OK;
 }
 
+ea_status ea_c4_vectors_static(ea_sim *sim, int64_t n_vec, const int32_t *dxyz, int64_t *B)
+{
+    if (!sim || n_vec < 0 || (n_vec && (!dxyz || !B))) return EA_ERR_INVALID;
+    if (sim->n_replicas != 2) EA_FAIL(sim, EA_ERR_STATE, "ea_c4_vectors_static needs a 2-replica sim");
+    if (!c4_vectors_supported(sim->lat.L)) EA_FAIL(sim, EA_ERR_INVALID, "ea_c4_vectors_static: L must be <= 32, 64 or 128");
+    if (EA_C4_STATIC_MAX_VECTORS != (int64_t)c4_vectors_static_max()) EA_FAIL(sim, EA_ERR_STATE, "ea_c4_vectors_static: header and library disagree on the limit");
+    if (n_vec > EA_C4_STATIC_MAX_VECTORS)
+        EA_FAIL(sim, EA_ERR_INVALID, "ea_c4_vectors_static: n_vec %lld exceeds the %lld vectors the static scratch array holds; use ea_c4_vectors",
+                (long long)n_vec, (long long)EA_C4_STATIC_MAX_VECTORS);
+    DeviceGuard g(sim->device);
+    EA_CUDA(sim, fold_ensure_unfolded(sim));
+    // the counts land in the caller's B (same width) and are turned into sums in place: no host buffer of our own
+    unsigned long long *cnt = (unsigned long long *)B;
+    EA_CUDA(sim, c4_vector_counts_static(sim, (size_t)n_vec, dxyz, cnt));
+    EA_SYNC(sim);
+    for (size_t k = 0; k < (size_t)n_vec * 32; ++k) B[k] = sim->N - 2 * (int64_t)cnt[k];
+    return EA_OK;
+}
+
 ea_status ea_c4_shells(ea_sim *sim, int r_max, int64_t *S, int64_t *mult)
 {
     if (!sim || !S || !mult) return EA_ERR_INVALID;

@@ -13,6 +13,7 @@
 // Work is cut into jobs = (dy, dz, first dx, up to NDX consecutive dx): the two rows are loaded once per job and
 // the dx scan advances by one-bit funnel shifts.  The kernel is bound by the popcount rate (16 lanes / clk / SM).
 #include <algorithm>
+#include <mutex>
 #include <vector>
 
 #include "ea_internal.h"
@@ -211,6 +212,115 @@ cudaError_t c4_vector_counts(ea_sim *s, size_t n, const int32_t *vec, unsigned l
     }
     if (Tr_own) { cudaStreamSynchronize(s->stream); cudaFree(Tr_own); }
     return e;
+}
+
+// ---------------------------------------------------------------------------------------------
+// The same counts with NO device or host allocation (ea_c4_vectors_static, include/ea.h): for callers that cannot call
+// cudaMalloc (inside a stream capture, in a serving loop, under a harness that forbids it).  c4_vector_counts() above keeps
+// its job list and its counters in grow-only cudaMalloc buffers; here they live in ONE file-scope device array of a fixed,
+// modest size, held by every GPU that loads the library until the process exits:
+//     out    unsigned long long [C4V_STATIC_MAX_VECTORS][32]   256 KiB   counters, cleared at the start of every call
+//     jobs   C4Job              [C4V_STATIC_MAX_VECTORS]        20 KiB
+//     tr     uint32_t           [14 * 14 * 32]                  24.5 KiB  the transposed overlap field of an L < 16 lattice
+//                                                                         (larger ones fit the sim's own staging buffer)
+// In host code the array's NAME is only a host-side stand-in, not a device address: its address on a device comes from
+// cudaGetSymbolAddress, asked once per device with that device current, below.  All calls share the array and it keeps
+// the last call's contents: two calls that overlap on the GPU (two sims on two streams, two host threads) race.
+// ---------------------------------------------------------------------------------------------
+constexpr size_t C4V_STATIC_MAX_VECTORS = 1024; // = EA_C4_STATIC_MAX_VECTORS (include/ea.h; checked in ea_api.cu)
+constexpr size_t C4V_STATIC_OUT_BYTES = C4V_STATIC_MAX_VECTORS * 32 * sizeof(unsigned long long);
+constexpr size_t C4V_STATIC_JOBS_OFF = C4V_STATIC_OUT_BYTES;
+constexpr size_t C4V_STATIC_JOBS_BYTES = (C4V_STATIC_MAX_VECTORS * sizeof(C4Job) + 255) / 256 * 256;
+constexpr size_t C4V_STATIC_TR_OFF = C4V_STATIC_JOBS_OFF + C4V_STATIC_JOBS_BYTES;
+constexpr size_t C4V_STATIC_TR_BYTES = (size_t)14 * 14 * 32 * sizeof(uint32_t);
+constexpr size_t C4V_STATIC_BYTES = C4V_STATIC_TR_OFF + C4V_STATIC_TR_BYTES;
+
+static __device__ __align__(256) unsigned char c4v_static_scratch[C4V_STATIC_BYTES];
+
+constexpr int C4V_MAX_DEVICES = 64;
+static unsigned char *c4v_static_ptr[C4V_MAX_DEVICES]; // device address of c4v_static_scratch, per device (nullptr: not asked yet)
+static std::mutex c4v_static_mutex;
+
+// the device address of the scratch array on `device`, which must be current
+static cudaError_t c4v_static_address(int device, unsigned char **ptr)
+{
+    if (device < 0 || device >= C4V_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(c4v_static_mutex);
+    if (!c4v_static_ptr[device]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, c4v_static_scratch);
+        if (e != cudaSuccess) return e;
+        c4v_static_ptr[device] = (unsigned char *)p;
+    }
+    *ptr = c4v_static_ptr[device];
+    return cudaSuccess;
+}
+
+size_t c4_vectors_static_max() { return C4V_STATIC_MAX_VECTORS; }
+
+// As c4_vector_counts for n <= C4V_STATIC_MAX_VECTORS vectors (cudaErrorInvalidValue beyond): the same two kernels, scratch
+// in the static array, host work in fixed-size buffers.  Synchronises the stream.  Not re-entrant (see above).
+cudaError_t c4_vector_counts_static(ea_sim *s, size_t n, const int32_t *vec, unsigned long long *counts)
+{
+    if (n > C4V_STATIC_MAX_VECTORS) return cudaErrorInvalidValue;
+    if (!n) return cudaSuccess;
+    const int L = s->lat.L;
+    const int wpr = (L + 31) / 32;
+    unsigned char *scratch = nullptr;
+    cudaError_t e = c4v_static_address(s->device, &scratch);
+    if (e != cudaSuccess) return e;
+    unsigned long long *d_out = (unsigned long long *)scratch;
+    C4Job *d_jobs = (C4Job *)(scratch + C4V_STATIC_JOBS_OFF);
+
+    // host side of c4_vector_counts in fixed-size buffers (static: 24 + 20 + 256 KiB are too much for a stack frame)
+    struct V { int dx, dy, dz; unsigned idx; };
+    static V v[C4V_STATIC_MAX_VECTORS];
+    static C4Job jobs[C4V_STATIC_MAX_VECTORS];
+    static unsigned long long h_out[C4V_STATIC_MAX_VECTORS * 32];
+    static std::mutex host_mutex; // the host buffers; the DEVICE array is still shared by calls on other streams
+    std::lock_guard<std::mutex> lock(host_mutex);
+    for (size_t i = 0; i < n; ++i) {
+        auto m = [L](int a) { int r = a % L; return r < 0 ? r + L : r; };
+        v[i] = {m(vec[3 * i]), m(vec[3 * i + 1]), m(vec[3 * i + 2]), (unsigned)i};
+    }
+    std::sort(v, v + n, [](const V &a, const V &b) { // in place: no allocation
+        if (a.dz != b.dz) return a.dz < b.dz;
+        if (a.dy != b.dy) return a.dy < b.dy;
+        if (a.dx != b.dx) return a.dx < b.dx;
+        return a.idx < b.idx;
+    });
+    size_t nj = 0;
+    for (size_t i = 0; i < n;) {
+        size_t j = i + 1;
+        while (j < n && j - i < (size_t)C4V_NDX && v[j].dz == v[i].dz && v[j].dy == v[i].dy && v[j].dx == v[j - 1].dx + 1) ++j;
+        jobs[nj++] = {v[i].dy, v[i].dz, v[i].dx, (int)(j - i), (unsigned)i};
+        i = j;
+    }
+
+    const size_t tr_bytes = (size_t)L * L * wpr * 32 * sizeof(uint32_t);
+    uint32_t *Tr = (uint32_t *)s->stage;
+    if (tr_bytes > (size_t)s->N * 8) { // L < 16 (rows are padded to 32 bits)
+        if (tr_bytes > C4V_STATIC_TR_BYTES) return cudaErrorInvalidValue;
+        Tr = (uint32_t *)(scratch + C4V_STATIC_TR_OFF);
+    }
+    k_q_rows<<<(unsigned)s->n_sm * 2, 256, 0, s->stream>>>(s->lat, s->spins, Tr, wpr);
+    s->count_launch();
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if ((e = cudaMemcpyAsync(d_jobs, jobs, nj * sizeof(C4Job), cudaMemcpyHostToDevice, s->stream)) != cudaSuccess) return e;
+    // the array keeps the last call's counters: the kernel adds into them, so they start at zero
+    if ((e = cudaMemsetAsync(d_out, 0, n * 32 * sizeof(unsigned long long), s->stream)) != cudaSuccess) return e;
+    const dim3 grid(C4V_ROWCHUNKS, (unsigned)nj);
+    switch (wpr) {
+    case 1: k_c4_vec<1><<<grid, 256, 0, s->stream>>>(L, Tr, d_jobs, d_out); break;
+    case 2: k_c4_vec<2><<<grid, 256, 0, s->stream>>>(L, Tr, d_jobs, d_out); break;
+    default: k_c4_vec<4><<<grid, 256, 0, s->stream>>>(L, Tr, d_jobs, d_out); break;
+    }
+    s->count_launch();
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if ((e = cudaMemcpyAsync(h_out, d_out, n * 32 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s->stream)) != cudaSuccess) return e;
+    if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return e;
+    for (size_t k = 0; k < n; ++k) std::copy(h_out + k * 32, h_out + (k + 1) * 32, counts + (size_t)v[k].idx * 32);
+    return cudaSuccess;
 }
 
 } // namespace ea

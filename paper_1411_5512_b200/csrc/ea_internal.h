@@ -132,6 +132,8 @@ cudaError_t launch_count_c4(ea_sim *s, int r_max); // counters[(d*(r_max+1)+r)*3
 // full-vector C_4 (ea_c4_vectors.cu): per-sample counts of q_i != q_{i+r} for n lattice vectors; host result
 bool c4_vectors_supported(int L);
 cudaError_t c4_vector_counts(ea_sim *s, size_t n, const int32_t *vec, unsigned long long *counts);
+size_t c4_vectors_static_max();
+cudaError_t c4_vector_counts_static(ea_sim *s, size_t n, const int32_t *vec, unsigned long long *counts); // no allocation; n <= c4_vectors_static_max()
 
 cudaError_t pipe_rates(int device, double out[8]);
 cudaError_t philox_selftest(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
