@@ -151,7 +151,7 @@ __device__ __forceinline__ void cluster_barrier()
 // interleaved chains of row classes as in the L = 128 kernel (0.69 at L = 32: a unit's latency, not its issue slots, sets
 // the pace).  The number of pushed pairs does not matter either (see small_shape).
 template <typename BondT, bool ALWAYS, bool RARE, bool HB, bool CLUSTER, bool YSPLIT>
-__global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
+__global__ void __launch_bounds__(CLUSTER ? 512 : 128, 1) k_sweep_small(const SmallArgs a)
 {
     constexpr bool PUSH = CLUSTER;
     extern __shared__ __align__(16) unsigned char smem_small[];
@@ -276,7 +276,7 @@ __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
         ulonglong2 out;
         out.x = metropolis_word<BondT, ALWAYS, RARE, HB>(own.x, Xa.x, A2, Pp.x, Pm.x, Zp.x, Zm.x, xA1, xA2, jyA, byA, jzA, bzA, r.x, r.y, a.th);
         out.y = metropolis_word<BondT, ALWAYS, RARE, HB>(own.y, Xa.y, B2, Pp.y, Pm.y, Zp.y, Zm.y, xB1, xB2, jyB, byB, jzB, bzB, r.z, r.w, a.th);
-        sts_v2u64(ad.own, out);
+        if (active) sts_v2u64(ad.own, out);
         own_r[c] = out;
         if (PUSH) {
             if (push_zlo) st_async_v2u64(ad.push_zlo, out, bar_zlo + 8 * c);
@@ -319,6 +319,25 @@ __global__ void __launch_bounds__(512, 1) k_sweep_small(const SmallArgs a)
         sweep_rng_set_time(g, t, colour);
         return sweep_random4(g, colour ? site1 : site0);
     };
+    if (!CLUSTER && !HB) {
+        // one CTA, one warp per sub-partition: nothing to overlap with but the warp's own instructions.  The next numbers
+        // are drawn in the same basic block as the loads and the logic of the current half-sweep (no branch around the
+        // update: only the store is predicated), so that the Philox chain fills the load and dependency latencies
+        // (L = 8: 0.30 -> 0.25 us per half-sweep with 64-bit bond words, 0.28 -> 0.24 with 32-bit ones; the heat bath's seven
+        // predicated levels did not gain).  Up to 255 registers: the one-CTA kernel never has more than 128 threads.
+        BondT j1[12];
+#pragma unroll 1
+        for (uint32_t sw = 0; sw < a.n_half / 2; ++sw) {
+            const uint4 r1 = draw(a.t0 + sw, 1u);
+            lds_bonds12(A[1].bonds, bond_stride, j1);
+            half_sweep(A[0], r, 0, Sc[0], j);
+            __syncthreads();
+            r = draw(a.t0 + sw + 1, 0u);
+            lds_bonds12(A[0].bonds, bond_stride, j);
+            half_sweep(A[1], r1, 1, Sc[1], j1);
+            __syncthreads();
+        }
+    } else
     for (uint32_t sw = 0; sw < a.n_half / 2; ++sw) { // n_half is even: colour 0 then colour 1 of sweep t0 + sw
         if (active) half_sweep(A[0], r, 0, Sc[0], j);
         barrier_begin(0);
@@ -376,7 +395,7 @@ static SmallShape small_shape(int L, int n_replicas)
             if (forced_cy && forced_cz && (Cy != forced_cy || Cz != forced_cz)) continue;
             const int Ly = L / Cy, Lz = L / Cz;
             const long pairs = (long)hp * Ly * Lz;
-            if (pairs > 512 || small_smem_bytes(L, Ly, Lz, bond_bytes) > 200 * 1024) continue;
+            if (pairs > (C == 1 ? 128 : 512) || small_smem_bytes(L, Ly, Lz, bond_bytes) > 200 * 1024) continue; // launch bounds
             const long cost = (pairs + 127) / 128 * 300 + (Cy * Cz == 1 ? 40 : Cy == 1 ? 450 : 510);
             if (!best.Cy || cost < best_cost) { best.Cy = Cy; best.Cz = Cz; best_cost = cost; } // ties: the smaller cluster
         }
@@ -418,7 +437,10 @@ static cudaError_t launch_small_typed(ea_sim *s, const SmallArgs &a, int C, unsi
     const Thresholds &th = s->th;
     if (s->dynamics == EA_DYN_HEATBATH) return launch_small_kernel<BondT, false, false, true, CLUSTER, YSPLIT>(a, C, threads, smem, st);
     const bool always = th.always[0] | th.always[1] | th.always[2];
-    const bool rare = !always && th.thr[2] < 0x04000000u; // as in the persistent L = 128 kernel
+    // The warp-level branch around the energy-raising levels (RARE, as in the persistent L = 128 kernel) saves alu issue
+    // slots, which only bind with four warps per sub-partition (L = 32: 0.65 against 0.70 us); with one or two the
+    // branch-free predicated levels schedule better (L = 8: 0.18 against 0.27 us, L = 16: 0.30 against 0.35, L = 24: 0.44 / 0.47)
+    const bool rare = threads > 256 && !always && th.thr[2] < 0x04000000u;
     return always ? launch_small_kernel<BondT, true, false, false, CLUSTER, YSPLIT>(a, C, threads, smem, st)
            : rare ? launch_small_kernel<BondT, false, true, false, CLUSTER, YSPLIT>(a, C, threads, smem, st)
                   : launch_small_kernel<BondT, false, false, false, CLUSTER, YSPLIT>(a, C, threads, smem, st);
