@@ -128,6 +128,10 @@ ea_status ea_get_dynamics(const ea_sim *sim, int *dynamics);
 ea_status ea_get_thresholds_heatbath(const ea_sim *sim, uint64_t thr[7]); /* thr[n_u], n_u = 0..6 (C-HB)     */
 ea_status ea_set_kernel(ea_sim *sim, int kernel);      /* EA_ERR_INVALID if not valid for this L  */
 ea_status ea_get_kernel(const ea_sim *sim, int *kernel); /* the variant AUTO resolved to          */
+/* How many sims the caller advances at the same time on this device (a scan), n >= 1; default 1.  Results
+ * never depend on it: the library only chooses between code paths tuned for one sim alone on the device (latency) and
+ * for many sims sharing its SMs (issue slots) -- today in the small-lattice kernel.  EA_ERR_INVALID if n < 1. */
+ea_status ea_set_concurrency_hint(ea_sim *sim, int n_concurrent_sims);
 ea_status ea_synchronize(ea_sim *sim);                 /* wait for the sim's stream               */
 /* Kernels this sim has launched on the device since ea_create (a CUDA-graph replay counts its kernel nodes). */
 ea_status ea_get_launch_count(const ea_sim *sim, uint64_t *n);

@@ -51,6 +51,7 @@ SIGNATURES = {
     "ea_get_dynamics": (_i, [_vp, C.POINTER(_i)]),
     "ea_get_thresholds_heatbath": (_i, [_vp, C.POINTER(_u64)]),
     "ea_set_kernel": (_i, [_vp, _i]),
+    "ea_set_concurrency_hint": (_i, [_vp, _i]),
     "ea_get_kernel": (_i, [_vp, C.POINTER(_i)]),
     "ea_synchronize": (_i, [_vp]),
     "ea_get_launch_count": (_i, [_vp, C.POINTER(_u64)]),
@@ -238,6 +239,10 @@ class Sim:
     @kernel.setter
     def kernel(self, k):
         self._ck(lib().ea_set_kernel(self._h, KERNEL_NAMES[k] if isinstance(k, str) else int(k)))
+
+    def set_concurrency_hint(self, n_concurrent_sims):
+        """How many sims the caller advances at the same time on this device (never changes a result)."""
+        self._ck(lib().ea_set_concurrency_hint(self._h, int(n_concurrent_sims)))
 
     # -- observables ----------------------------------------------------------------------------------
     def snapshot(self, slot):

@@ -485,6 +485,14 @@ ea_status ea_get_thresholds_heatbath(const ea_sim *sim, uint64_t thr[7])
     return EA_OK;
 }
 
+ea_status ea_set_concurrency_hint(ea_sim *sim, int n_concurrent_sims)
+{
+    if (!sim) return EA_ERR_INVALID;
+    if (n_concurrent_sims < 1) EA_FAIL(sim, EA_ERR_INVALID, "ea_set_concurrency_hint: n_concurrent_sims %d < 1", n_concurrent_sims);
+    sim->n_concurrent = n_concurrent_sims;
+    return EA_OK;
+}
+
 ea_status ea_set_kernel(ea_sim *sim, int kernel)
 {
     if (!sim) return EA_ERR_INVALID;

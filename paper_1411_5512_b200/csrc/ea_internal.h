@@ -26,6 +26,7 @@ struct ea_sim {
     cudaStream_t stream = nullptr;
     int kernel = EA_KERNEL_SCALAR; // resolved variant
     int dynamics = EA_DYN_METROPOLIS;
+    int n_concurrent = 1;         // ea_set_concurrency_hint
     uint64_t thr_hb[7] = {0, 0, 0, 0, 0, 0, 0};
 
     bool own_ws = false, own_stream = false;

@@ -440,7 +440,10 @@ static cudaError_t launch_small_typed(ea_sim *s, const SmallArgs &a, int C, unsi
     // The warp-level branch around the energy-raising levels (RARE, as in the persistent L = 128 kernel) saves alu issue
     // slots, which only bind with four warps per sub-partition (L = 32: 0.65 against 0.70 us); with one or two the
     // branch-free predicated levels schedule better (L = 8: 0.18 against 0.27 us, L = 16: 0.30 against 0.35, L = 24: 0.44 / 0.47)
-    const bool rare = threads > 256 && !always && th.thr[2] < 0x04000000u;
+    // -- unless many sims share the SMs (ea_set_concurrency_hint), which makes the issue slots bind again (64 points of
+    // L = 16: 1.40 against 1.62 us per sweep of all of them).
+    const bool shared = (long)s->n_concurrent * C > s->n_sm;
+    const bool rare = (threads > 256 || shared) && !always && th.thr[2] < 0x04000000u;
     return always ? launch_small_kernel<BondT, true, false, false, CLUSTER, YSPLIT>(a, C, threads, smem, st)
            : rare ? launch_small_kernel<BondT, false, true, false, CLUSTER, YSPLIT>(a, C, threads, smem, st)
                   : launch_small_kernel<BondT, false, false, false, CLUSTER, YSPLIT>(a, C, threads, smem, st);

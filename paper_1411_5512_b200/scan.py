@@ -29,11 +29,13 @@ class Scan:
                                          kernel=pt.get("kernel", "auto"), device=device))
         # Which points share launches (measured on B200, 2000-sweep calls, us per sweep of ALL points): none, unless asked.
         #   L <= 32: every point alone on its stream -- AUTO runs SMALL (lattice in the shared memory of one CTA / cluster, one
-        #            launch per call): L = 16: 0.89 (16 points) / 1.40 (64) against 5.19 / 5.99 for the fused launches
-        #            (ea_batch_*: one launch per colour for all points); L = 32: 2.9 / 4.3 / 7.2 / 14.3 / 27.3 with 8 / 16 / 32 /
-        #            64 / 128 points against - / 6.9 / 9.0 / 14.6 / 30.1 fused;
+        #            launch per call): L = 16: 0.82 (16 points) / 1.41 (64) against 5.19 / 5.99 for the fused launches
+        #            (ea_batch_*: one launch per colour for all points); L = 32: 3.9 / 13.1 / 24.9 with 16 / 64 / 128 points
+        #            against 6.9 / 14.6 / 30.1 fused;
         #   L = 64:  streams of graph replays (10.2 for 8 points against 14 fused).
         # fused=True fuses every group of one shape (L in 16, 32, 64); "auto" and False do not.
+        for s in self.sims:
+            s.set_concurrency_hint(len(self.sims))   # many sims share the SMs: throughput-oriented code paths
         self.batches, self._solo = [], list(self.sims)
         groups = {}
         for s in self.sims:

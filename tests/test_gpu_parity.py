@@ -719,6 +719,27 @@ def test_small_lattice_kernel_auto_choice_and_long_runs():
         binding.Sim(10, 0.5, 0.8, n_replicas=2, kernel="small")  # needs L % 4 == 0
 
 
+def test_concurrency_hint_never_changes_a_result():
+    """ea_set_concurrency_hint only picks between code paths of the small-lattice kernel (branch-free levels for one sim
+    alone, the warp-level branch when many sims share the SMs): same trajectory, against the oracle and each other."""
+    for L, n_rep, T in ((8, 1, 0.8), (16, 2, 0.8), (24, 2, 0.8), (32, 2, 0.8)):
+        a = binding.Sim(L, 0.5, T, n_replicas=n_rep, seed=wl.seed_for(4, L), n_slots=0)
+        b = binding.Sim(L, 0.5, T, n_replicas=n_rep, seed=wl.seed_for(4, L), n_slots=0)
+        o = Oracle(L, 0.5, T, n_replicas=n_rep, seed=wl.seed_for(4, L), n_slots=0)
+        b.set_concurrency_hint(1000)
+        assert a.kernel == b.kernel == binding.EA_KERNEL_SMALL
+        for n in (2, 7, 31):
+            a.sweep(n); b.sweep(n); o.sweep(n)
+            sa, sb = a.get_spins(), b.get_spins()
+            assert np.array_equal(sa, sb) and np.array_equal(sa, o.get_spins()), "L=%d after %d sweeps" % (L, a.time)
+        b.set_concurrency_hint(1)
+        a.sweep(200); b.sweep(200)
+        assert np.array_equal(a.get_spins(), b.get_spins())
+        with pytest.raises(binding.EAError):
+            b.set_concurrency_hint(0)
+        a.close(); b.close()
+
+
 @pytest.mark.parametrize("L,n_rep", [(8, 1), (12, 2), (32, 2), (64, 2), (128, 2)])
 def test_measure_point_in_one_call_equals_the_separate_calls_and_the_oracle(L, n_rep):
     """ea_measure (all observables of a measure point enqueued back to back, one copy, one wait) against ea_autocorr /
