@@ -118,13 +118,14 @@ __global__ void __launch_bounds__(256) k_count_spins(Lattice lat, const uint64_t
 }
 
 // cnt_b over the 3N words j_d(i) ^ sigma_i ^ sigma_{i+e_d} (unsatisfied bonds, C-A2): energy.
-template <typename BondT>
+// POW2: L is a power of two -- coordinates by shifts and masks (the divisions by run-time L cost more than the counting)
+template <typename BondT, bool POW2>
 __global__ void __launch_bounds__(256) k_count_energy(Lattice lat, const uint64_t *__restrict__ spins,
                                                       const BondT *__restrict__ bonds, unsigned long long *out)
 {
-    const unsigned lane = threadIdx.x & 31, N = 2 * lat.Nh;
+    const unsigned lane = threadIdx.x & 31, Nh = lat.Nh, N = 2 * Nh;
     const unsigned stride = gridDim.x * blockDim.x;
-    const unsigned L = lat.L;
+    const unsigned L = lat.L, Lh = lat.Lh;
     Csa8 acc;
     LaneCounter k8;
     for (unsigned base = blockIdx.x * blockDim.x; base < N; base += 8 * stride) { // eight sites = three groups of eight words
@@ -134,15 +135,29 @@ __global__ void __launch_bounds__(256) k_count_energy(Lattice lat, const uint64_
             const unsigned e = base + j * stride + threadIdx.x;
             u[0][j] = u[1][j] = u[2][j] = 0;
             if (e < N) {
-                Coord q = coord_of(lat, e);
-                unsigned i = e - q.c * lat.Nh, x = 2 * q.xh + ((q.c ^ (q.y + q.z)) & 1u);
-                unsigned xp = (x + 1 == L) ? 0 : x + 1, yp = (q.y + 1 == L) ? 0 : q.y + 1, zp = (q.z + 1 == L) ? 0 : q.z + 1;
-                uint64_t sg = spins[e];
-                const BondT *J = bonds + (size_t)q.c * 3 * lat.Nh;
-                BondT j0 = J[i], j1 = J[lat.Nh + i], j2 = J[2 * lat.Nh + i];
-                u[0][j] = mk64(bond_lo(j0), bond_hi(j0)) ^ sg ^ spins[flat_of(lat, xp, q.y, q.z)];
-                u[1][j] = mk64(bond_lo(j1), bond_hi(j1)) ^ sg ^ spins[flat_of(lat, x, yp, q.z)];
-                u[2][j] = mk64(bond_lo(j2), bond_hi(j2)) ^ sg ^ spins[flat_of(lat, x, q.y, zp)];
+                const unsigned c = e >= Nh, i = e - c * Nh;
+                unsigned xh, y, z;
+                if (POW2) {
+                    xh = i & (Lh - 1);
+                    const unsigned row = i >> lat.log2Lh;
+                    y = row & (L - 1);
+                    z = row >> lat.log2L;
+                } else {
+                    xh = i % Lh;
+                    const unsigned row = i / Lh;
+                    y = row % L;
+                    z = row / L;
+                }
+                // the +x / +y / +z neighbours have the other colour: compact x = xh + S (S = row phase of colour c), same xh
+                const unsigned S = (c ^ (y + z)) & 1u, xn = xh + S == Lh ? 0 : xh + S;
+                const unsigned yp = y + 1 == L ? 0 : y + 1, zp = z + 1 == L ? 0 : z + 1;
+                const uint64_t *oth = spins + (1 - c) * Nh;
+                const uint64_t sg = spins[e];
+                const BondT *J = bonds + (size_t)c * 3 * Nh;
+                const BondT j0 = J[i], j1 = J[Nh + i], j2 = J[2 * Nh + i];
+                u[0][j] = mk64(bond_lo(j0), bond_hi(j0)) ^ sg ^ oth[i - xh + xn];
+                u[1][j] = mk64(bond_lo(j1), bond_hi(j1)) ^ sg ^ oth[Lh * (yp + L * z) + xh];
+                u[2][j] = mk64(bond_lo(j2), bond_hi(j2)) ^ sg ^ oth[Lh * (y + L * zp) + xh];
             }
         }
 #pragma unroll
@@ -385,10 +400,15 @@ cudaError_t launch_count_energy(ea_sim *s, unsigned long long *dst)
     if (!dst) dst = s->counters;
     cudaError_t e = cudaMemsetAsync(dst, 0, 64 * sizeof(unsigned long long), s->stream);
     if (e != cudaSuccess) return e;
-    if (s->n_replicas == 2)
-        k_count_energy<uint32_t><<<grid_for(s, s->N), 256, 0, s->stream>>>(s->lat, s->spins, (const uint32_t *)s->bonds, dst);
-    else
-        k_count_energy<uint64_t><<<grid_for(s, s->N), 256, 0, s->stream>>>(s->lat, s->spins, (const uint64_t *)s->bonds, dst);
+    const bool pow2 = s->lat.log2L >= 0 && s->lat.log2Lh >= 0;
+    const unsigned grid = grid_for(s, s->N);
+    if (s->n_replicas == 2) {
+        if (pow2) k_count_energy<uint32_t, true><<<grid, 256, 0, s->stream>>>(s->lat, s->spins, (const uint32_t *)s->bonds, dst);
+        else k_count_energy<uint32_t, false><<<grid, 256, 0, s->stream>>>(s->lat, s->spins, (const uint32_t *)s->bonds, dst);
+    } else {
+        if (pow2) k_count_energy<uint64_t, true><<<grid, 256, 0, s->stream>>>(s->lat, s->spins, (const uint64_t *)s->bonds, dst);
+        else k_count_energy<uint64_t, false><<<grid, 256, 0, s->stream>>>(s->lat, s->spins, (const uint64_t *)s->bonds, dst);
+    }
     s->count_launch();
     return cudaGetLastError();
 }
