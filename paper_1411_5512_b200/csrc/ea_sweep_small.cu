@@ -384,6 +384,7 @@ static SmallShape small_shape(int L, int n_replicas)
 {
     SmallShape best = {0, 0};
     if (L < 4 || L % 4 || L > 64) return best;
+    // EA_SMALL_CY / EA_SMALL_CZ (both set): the shape, for measurements like the ones quoted above; shapes that do not fit are skipped
     static const int forced_cy = [] { const char *e = getenv("EA_SMALL_CY"); return e ? atoi(e) : 0; }();
     static const int forced_cz = [] { const char *e = getenv("EA_SMALL_CZ"); return e ? atoi(e) : 0; }();
     const int bond_bytes = n_replicas == 2 ? 4 : 8, hp = L / 4;
