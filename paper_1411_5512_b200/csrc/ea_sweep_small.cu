@@ -12,7 +12,6 @@
 // Spins AND bond words live in shared memory; global memory is read once at the start and written once at the end.
 // A thread owns one pair of x-adjacent same-colour sites of each colour (one Philox block per pair and sweep, C-A7).
 #include <stdlib.h>
-#include <string.h>
 
 #include "ea_internal.h"
 #include "ea_sweep_common.cuh"
@@ -42,12 +41,6 @@ __device__ __forceinline__ uint32_t cluster_ctarank()
 {
     uint32_t r;
     asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ uint32_t cluster_nctarank()
-{
-    uint32_t r;
-    asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
     return r;
 }
 // shared-memory loads by 32-bit shared address (precomputed once per thread: the sweep loop holds no index arithmetic)
@@ -261,7 +254,7 @@ __global__ void __launch_bounds__(CLUSTER ? 512 : 128, 1) k_sweep_small(const Sm
 
     // the thread's own pairs stay in registers between the sweeps (nobody else writes them); shared memory holds the copy
     // the neighbours read
-    ulonglong2 own_r[2];
+    ulonglong2 own_r[2] = {};
     auto half_sweep = [&](const SmallAddr &ad, const uint4 r, const unsigned c, const bool S, const BondT (&j)[12]) {
         // the row's other-colour words next to the pair: compact q0, q0 + 1, q0 + 2 with q0 = 2p - 1 + S
         const ulonglong2 Xa = lds_v2u64(ad.xa);
@@ -305,7 +298,6 @@ __global__ void __launch_bounds__(CLUSTER ? 512 : 128, 1) k_sweep_small(const Sm
     uint4 r = sweep_random4(g, site0);
     if (CLUSTER) cluster_barrier(); else __syncthreads(); // every CTA of the cluster has its slab in place
 
-    own_r[0] = own_r[1] = make_ulonglong2(0, 0);
     if (active) {
         own_r[0] = lds_v2u64(A[0].own);
         own_r[1] = lds_v2u64(A[1].own);
@@ -416,8 +408,7 @@ static cudaError_t launch_small_kernel(const SmallArgs &a, int C, unsigned threa
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     if (C > 8 && (e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1)) != cudaSuccess) return e;
-    cudaLaunchConfig_t cfg;
-    memset(&cfg, 0, sizeof(cfg));
+    cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)C);
     cfg.blockDim = dim3(threads);
     cfg.dynamicSmemBytes = smem;
@@ -468,8 +459,7 @@ bool small_supported(const ea_sim *s, std::string *why)
             (C > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess))
             return no("small-lattice kernel: the device rejects the cluster configuration");
         const unsigned pairs = (unsigned)((size_t)(s->lat.L / 4) * Ly * Lz);
-        cudaLaunchConfig_t cfg;
-        memset(&cfg, 0, sizeof(cfg));
+        cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3((unsigned)C);
         cfg.blockDim = dim3((pairs + 31) / 32 * 32);
         cfg.dynamicSmemBytes = smem;
