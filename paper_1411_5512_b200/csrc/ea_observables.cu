@@ -60,18 +60,47 @@ __device__ __forceinline__ void flush_counts(const LaneCounter &k, unsigned long
     }
 }
 
-// Carry-save front end of the per-sample counters: eight 64-sample words go through seven 3:2 compressors (Harley-Seal)
-// into bit-sliced ones / twos / fours planes kept per thread; only the "eights" word they emit -- and, once at the end,
-// the three planes -- pays for the 32 x 32 bit transposition and the POPC: one transposition per eight words, not eight.
-struct Csa8 {
-    uint64_t ones = 0, twos = 0, fours = 0;
+// Bit-sliced (vertical) per-sample counter.  Eight 64-sample words go through seven 3:2 compressors (Harley-Seal) into
+// ones / twos / fours planes kept per thread; the "eights" word they emit ripples through four more planes (weights 8 ..
+// 64) with half adders, so that nothing pays for the 32 x 32 bit transposition and the POPC until a thread has taken 120
+// words (or is done): seven planes are drained at once instead of one transposition per eight words.
+struct VCounter {
+    uint64_t ones = 0, twos = 0, fours = 0, hi[4] = {0, 0, 0, 0}; // hi[k]: weight 8 << k
+    unsigned n_words = 0;                                         // taken since the last drain (thread-uniform in a warp)
     static __device__ __forceinline__ void csa(uint64_t &h, uint64_t &l, uint64_t a, uint64_t b, uint64_t c)
     {
         h = mk64(lop3<LUT_MAJ>(lo32(a), lo32(b), lo32(c)), lop3<LUT_MAJ>(hi32(a), hi32(b), hi32(c)));
         l = mk64(lop3<LUT_XOR3>(lo32(a), lo32(b), lo32(c)), lop3<LUT_XOR3>(hi32(a), hi32(b), hi32(c)));
     }
-    __device__ __forceinline__ uint64_t add8(const uint64_t (&x)[8]) // returns the eights word
+    // weights x planes -> counts of the lane's two samples; planes cleared
+    __device__ __forceinline__ void drain(LaneCounter &k, unsigned lane)
     {
+        LaneCounter t;
+        unsigned lo = 0, hi_ = 0;
+#pragma unroll
+        for (int l = 3; l >= 0; --l) {
+            t.lo = t.hi = 0;
+            t.add64(hi[l], lane);
+            lo = 2 * lo + t.lo;
+            hi_ = 2 * hi_ + t.hi;
+            hi[l] = 0;
+        }
+        const uint64_t low[3] = {fours, twos, ones};
+#pragma unroll
+        for (int l = 0; l < 3; ++l) {
+            t.lo = t.hi = 0;
+            t.add64(low[l], lane);
+            lo = 2 * lo + t.lo;
+            hi_ = 2 * hi_ + t.hi;
+        }
+        ones = twos = fours = 0;
+        n_words = 0;
+        k.lo += lo;
+        k.hi += hi_;
+    }
+    __device__ __forceinline__ void add8(const uint64_t (&x)[8], LaneCounter &k, unsigned lane)
+    {
+        if (n_words > 127 - 8) drain(k, lane); // the planes hold counts up to 127
         uint64_t tA, tB, tC, tD, fA, fB, e;
         csa(tA, ones, ones, x[0], x[1]);
         csa(tB, ones, ones, x[2], x[3]);
@@ -80,20 +109,15 @@ struct Csa8 {
         csa(tD, ones, ones, x[6], x[7]);
         csa(fB, twos, twos, tC, tD);
         csa(e, fours, fours, fA, fB);
-        return e;
+#pragma unroll
+        for (int l = 0; l < 4; ++l) { // half adders: the carry out of the last plane is zero by the bound above
+            const uint64_t c = hi[l] & e;
+            hi[l] ^= e;
+            e = c;
+        }
+        n_words += 8;
     }
 };
-
-// weights 8 (eights words), then the planes once: lo / hi = counts of samples lane and lane + 32
-__device__ __forceinline__ void csa_finish(const Csa8 &a, const LaneCounter &k8, unsigned lane, LaneCounter &out)
-{
-    LaneCounter k1, k2, k4;
-    k1.add64(a.ones, lane);
-    k2.add64(a.twos, lane);
-    k4.add64(a.fours, lane);
-    out.lo = 8 * k8.lo + 4 * k4.lo + 2 * k2.lo + k1.lo;
-    out.hi = 8 * k8.hi + 4 * k4.hi + 2 * k2.hi + k1.hi;
-}
 
 // cnt_b over all N words of sigma ^ other (other may be null): autocorrelation / magnetisation.
 __global__ void __launch_bounds__(256) k_count_spins(Lattice lat, const uint64_t *__restrict__ spins,
@@ -101,8 +125,8 @@ __global__ void __launch_bounds__(256) k_count_spins(Lattice lat, const uint64_t
 {
     const unsigned lane = threadIdx.x & 31, N = 2 * lat.Nh;
     const unsigned stride = gridDim.x * blockDim.x;
-    Csa8 acc;
-    LaneCounter k8;
+    VCounter acc;
+    LaneCounter k;
     for (unsigned base = blockIdx.x * blockDim.x; base < N; base += 8 * stride) { // block-uniform trip count
         uint64_t w[8];
 #pragma unroll
@@ -110,10 +134,9 @@ __global__ void __launch_bounds__(256) k_count_spins(Lattice lat, const uint64_t
             const unsigned e = base + j * stride + threadIdx.x;
             w[j] = e < N ? (other ? (spins[e] ^ other[e]) : spins[e]) : 0;
         }
-        k8.add64(acc.add8(w), lane);
+        acc.add8(w, k, lane);
     }
-    LaneCounter k;
-    csa_finish(acc, k8, lane, k);
+    acc.drain(k, lane);
     flush_counts(k, out, true);
 }
 
@@ -126,8 +149,8 @@ __global__ void __launch_bounds__(256) k_count_energy(Lattice lat, const uint64_
     const unsigned lane = threadIdx.x & 31, Nh = lat.Nh, N = 2 * Nh;
     const unsigned stride = gridDim.x * blockDim.x;
     const unsigned L = lat.L, Lh = lat.Lh;
-    Csa8 acc;
-    LaneCounter k8;
+    VCounter acc;
+    LaneCounter k;
     for (unsigned base = blockIdx.x * blockDim.x; base < N; base += 8 * stride) { // eight sites = three groups of eight words
         uint64_t u[3][8];
 #pragma unroll
@@ -161,10 +184,9 @@ __global__ void __launch_bounds__(256) k_count_energy(Lattice lat, const uint64_
             }
         }
 #pragma unroll
-        for (int d = 0; d < 3; ++d) k8.add64(acc.add8(u[d]), lane);
+        for (int d = 0; d < 3; ++d) acc.add8(u[d], k, lane);
     }
-    LaneCounter k;
-    csa_finish(acc, k8, lane, k);
+    acc.drain(k, lane);
     flush_counts(k, out, true);
 }
 
@@ -379,9 +401,11 @@ static cudaError_t launch_c4_fast(ea_sim *s, int r_max)
     return cudaGetLastError();
 }
 
+// Counting kernels: every thread ends with the transposition of its seven planes, so threads are few and long -- two
+// CTAs of 256 threads per SM (L = 128: 28 words per thread) unless the lattice has fewer words than that
 static unsigned grid_for(const ea_sim *s, size_t items)
 {
-    size_t need = (items + 255) / 256, cap = (size_t)s->n_sm * 8;
+    size_t need = (items + 255) / 256, cap = (size_t)s->n_sm * 2;
     return (unsigned)(need < cap ? (need ? need : 1) : cap);
 }
 
