@@ -719,6 +719,29 @@ def test_small_lattice_kernel_auto_choice_and_long_runs():
         binding.Sim(10, 0.5, 0.8, n_replicas=2, kernel="small")  # needs L % 4 == 0
 
 
+def test_many_concurrent_small_sims_match_the_per_colour_kernels():
+    """Stress of the cluster exchange: 40 sims of L = 32 (sixteen-CTA clusters, nine fit the device at a time) and 40 of
+    L = 16 advance at once on their own streams, 400 sweeps in calls of uneven length; every one must equal the same sim
+    run alone through the per-colour kernels."""
+    sims = []
+    for k in range(80):
+        L = 32 if k < 40 else 16
+        sims.append(binding.Sim(L, 0.5 + 0.005 * (k % 40), 0.8 if k % 3 else 2.0, n_replicas=2, seed=wl.seed_for(6, k), n_slots=0))
+        assert sims[-1].kernel == binding.EA_KERNEL_SMALL
+        if k % 2:
+            sims[-1].set_concurrency_hint(80)
+    for n in (3, 120, 2, 275):
+        for s in sims:
+            s.sweep(n)                 # asynchronous: the launches of all sims are in flight together
+    for k, s in enumerate(sims):
+        L = 32 if k < 40 else 16
+        ref = binding.Sim(L, 0.5 + 0.005 * (k % 40), 0.8 if k % 3 else 2.0, n_replicas=2, seed=wl.seed_for(6, k), n_slots=0, kernel="rows")
+        ref.sweep(400)
+        assert np.array_equal(s.get_spins(), ref.get_spins()), "sim %d (L = %d)" % (k, L)
+        ref.close()
+        s.close()
+
+
 def test_concurrency_hint_never_changes_a_result():
     """ea_set_concurrency_hint only picks between code paths of the small-lattice kernel (branch-free levels for one sim
     alone, the warp-level branch when many sims share the SMs): same trajectory, against the oracle and each other."""
